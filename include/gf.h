@@ -1,0 +1,176 @@
+/*
+ * gf.h — C ABI of libgf.so: SU(3) lattice gauge fixing by checkerboard local updates on one B200.
+ *
+ * The operations are those of Schroeck & Vogt, "Coulomb, Landau and Maximally Abelian Gauge Fixing
+ * in Lattice QCD with Multi-GPUs" (arxiv 1212.5221; line numbers below refer to the text of the
+ * paper as PAPER.md).  Every entry point enqueues hand-written sm_100a CUDA kernels; there is no
+ * CPU fallback: without a CUDA device gf_create fails with GF_ECUDA.
+ *
+ * Conventions common to all calls
+ *   - Return value: 0 = GF_OK, 1 = GF_NOT_CONVERGED (gf_run only), < 0 = error.  No exception or
+ *     abort crosses the ABI.  gf_last_error(ctx) returns a ctx-owned, NUL-terminated description of
+ *     the last error (valid until the next call on that ctx).
+ *   - A context owns all of its device memory.  The caller owns every pointer it passes in; the
+ *     library never keeps a caller pointer beyond the call.
+ *   - One context per stream, not thread-safe.  Kernels are enqueued on the cudaStream_t given to
+ *     gf_create (NULL = the legacy default stream).  gf_set_links, gf_get_*, gf_measure, gf_run and
+ *     gf_anneal(with history) synchronise that stream before returning; gf_sweep, gf_half_sweep,
+ *     gf_reunitarize and gf_coulomb_finalize only enqueue.
+ *   - Host-side link layout ("StandardPattern", Sec. 4.2.1; mu = 0 is the temporal
+ *     direction): links[t][x][y][z][mu][i][j][c], c = 0 real / 1 imaginary, i.e. real
+ *     offset ((((((t*Nx + x)*Ny + y)*Nz + z)*4 + mu)*3 + i)*3 + j)*2 + c.  mu = 1,2,3 are x,y,z.
+ *     Gauge transforms use [t][x][y][z][i][j][c].
+ *   - All four extents must be even and >= 2 (the red/black colouring of PAPER.md:293 fn. 3 is
+ *     inconsistent under periodic boundaries otherwise); Nx*Ny*Nz*Nt < 2^32.
+ */
+#ifndef GF_H_
+#define GF_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gf_ctx gf_ctx; /* opaque */
+
+/* return codes */
+#define GF_OK 0
+#define GF_NOT_CONVERGED 1
+#define GF_EINVAL (-1) /* bad argument (odd extent, unknown gauge/algo, NULL pointer, ...) */
+#define GF_ENOMEM (-2) /* device or host allocation failed */
+#define GF_ECUDA (-3)  /* a CUDA runtime call or kernel launch failed; see gf_last_error */
+#define GF_ESTATE (-4) /* call not valid in this state (e.g. no links set, transform not tracked) */
+
+/* precision policy (Sec. 4.5) */
+#define GF_SP 0 /* float links, float Step 1 and Step 2; reductions and reunitarisation in double */
+#define GF_DP 1 /* everything in double */
+#define GF_MP 2 /* float links and Step 2; Step 1 (gauge-update calculation) in double */
+
+/* gauge (Sec. 2.1) */
+#define GF_LANDAU 0  /* Eq. (4), all four directions */
+#define GF_COULOMB 1 /* Eq. (4) restricted to mu = 1,2,3; every time-slice is its own problem */
+#define GF_MAG 2     /* maximally Abelian gauge, functional Eq. (11) */
+
+/* Step-1 update rule (Secs. 2.2.3-2.3) */
+#define GF_OR 0    /* overrelaxation g -> g^omega "to first order" = Fig. A.11; param = omega in [1,2) */
+#define GF_SR 1    /* stochastic relaxation: g^2 with probability param = p, else g */
+#define GF_SA 2    /* simulated-annealing heatbath at temperature param = T */
+#define GF_MICRO 3 /* microcanonical step g -> g^2; param ignored */
+
+/* gf_create flags */
+#define GF_FLAG_TRACK_TRANSFORM 1u /* accumulate g(x) so that gf_get_gauge_transform / Coulomb finalisation work */
+
+/*
+ * gf_create — allocate a context for an Nx*Ny*Nz*Nt periodic lattice (BASELINE.json north_star:
+ * gf_create(Nx,Ny,Nz,Nt,precision)).  recon = 18 stores full links, recon = 12 stores the first two
+ * rows and rebuilds the third as (u x v)^* on load.  Device storage is parity-split
+ * structure-of-arrays in 16-byte vectors.  cuda_stream: a cudaStream_t or NULL.
+ * Errors: GF_EINVAL (extents, precision, recon), GF_ECUDA (no device), GF_ENOMEM.
+ */
+int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int recon, unsigned flags,
+              void* cuda_stream);
+int gf_destroy(gf_ctx* ctx);
+
+/*
+ * gf_set_links / gf_get_links — copy a whole configuration in / out in StandardPattern.
+ * links: host pointer (is_device = 0) or device pointer (is_device = 1) to Nt*Nx*Ny*Nz*4*18 reals of
+ * elem_bytes = 4 (float) or 8 (double), independent of the context's precision (converted on the
+ * way).  gf_set_links resets the accumulated gauge transform to the identity.  With recon = 12 the
+ * third row returned by gf_get_links is the reconstructed one.  Synchronous.
+ */
+int gf_set_links(gf_ctx* ctx, const void* links, int elem_bytes, int is_device);
+int gf_get_links(gf_ctx* ctx, void* links, int elem_bytes, int is_device);
+
+/*
+ * gf_get_gauge_transform — the accumulated g(x) with U_now = g(x) U_set g(x+mu)^dagger (Eq. (1),
+ * PAPER.md:25), layout [t][x][y][z][i][j][c].  Needs GF_FLAG_TRACK_TRANSFORM (else GF_ESTATE).
+ */
+int gf_get_gauge_transform(gf_ctx* ctx, void* g, int elem_bytes, int is_device);
+
+/*
+ * gf_sweep — one sweep of Alg. 1: the even half-sweep then the odd one.  For every
+ * site x of the active parity: gather U_mu(x), U_mu(x-mu); for the SU(2) subgroups (0,1),(0,2),(1,2)
+ * find g (Step 1, rule `algo`) and rotate U_mu(x) <- g U_mu(x), U_mu(x-mu) <- U_mu(x-mu) g^dagger
+ * (Step 2).  Parity is (t+x+y+z)&1 for Landau/MAG and (x+y+z)&1 in every time-slice
+ * for Coulomb, whose sweeps touch spatial links only.
+ * seed / sweep_index key the counter-based Philox4x32-10 generator (PAPER.md:249 fn. 2) as
+ * counter = (lexicographic site index, sweep_index, subgroup | purpose << 8, trial), key = seed;
+ * they are ignored by GF_OR and GF_MICRO.  Asynchronous.
+ * gf_half_sweep does one parity only (parity 0 = even, 1 = odd).
+ */
+int gf_sweep(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t sweep_index);
+int gf_half_sweep(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t sweep_index,
+                  int parity);
+
+/*
+ * gf_measure — gauge functional F (Eq. (4), N_d = 3 for Coulomb; Eq. (11) PAPER.md:102 for
+ * MAG) and gauge precision theta (Eq. (7); MAG: sum over the three subgroups of
+ * |X^s_12|^2 / (N_c V), R11), reduced on the device in double with a fixed summation order
+ * (bit-reproducible).  theta_slice: NULL or Nt doubles receiving theta of every time-slice
+ * (V -> Nx*Ny*Nz), the Coulomb stopping quantity.  Synchronous.
+ */
+int gf_measure(gf_ctx* ctx, int gauge, double* F, double* theta, double* theta_slice);
+
+typedef struct {
+    int sweeps;   /* sweeps performed */
+    double F;     /* functional at the last check */
+    double theta; /* stopping quantity at the last check: theta, or max_t theta_t for Coulomb */
+} gf_result;
+
+/*
+ * gf_run — Alg. 1's outer loop: sweep (sweep s uses sweep_index first_sweep_index + s)
+ * until the stopping quantity < eps, checked after every check_every-th sweep and after the last one,
+ * or until max_sweeps.  reunit_every > 0 reprojects all links (and the tracked transform) onto SU(3)
+ * after every reunit_every-th sweep.  hist: NULL or room for
+ * 3 * (max_sweeps / check_every + 1) doubles, filled with (sweep, F, theta) per check.
+ * For Coulomb with a tracked transform the temporal links are finalised before returning
+ * (PAPER.md:448).  Returns GF_OK if converged, GF_NOT_CONVERGED otherwise.  Synchronous.
+ */
+int gf_run(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t first_sweep_index,
+           int max_sweeps, double eps, int check_every, int reunit_every, gf_result* out, double* hist);
+
+/*
+ * gf_anneal — simulated annealing schedule: n_steps heatbath sweeps at
+ * T_k = T_hi - k (T_hi - T_lo)/(n_steps - 1), each followed by n_micro microcanonical sweeps; every
+ * sweep consumes one sweep index starting at first_sweep_index.  *next_sweep_index (may be NULL)
+ * receives the first unused index.  Asynchronous.
+ */
+int gf_anneal(gf_ctx* ctx, int gauge, double T_hi, double T_lo, int n_steps, int n_micro, uint64_t seed,
+              uint32_t first_sweep_index, uint32_t* next_sweep_index);
+
+/*
+ * gf_reunitarize — reproject every link (and the tracked transform) onto SU(3): Gram-Schmidt on rows
+ * 0,1 in double, third row (u x v)^* (R20).  Asynchronous.
+ */
+int gf_reunitarize(gf_ctx* ctx);
+
+/*
+ * gf_coulomb_finalize — apply the accumulated g to the temporal links,
+ * U_0(x,t) <- g(x,t) U_0(x,t) g(x,t+1)^dagger.  Idempotent: only the part of g not yet
+ * applied is used.  Called implicitly by gf_run(Coulomb), gf_get_links and by Landau/MAG calls that
+ * follow Coulomb sweeps.  Needs GF_FLAG_TRACK_TRANSFORM (else GF_ESTATE).  Asynchronous.
+ */
+int gf_coulomb_finalize(gf_ctx* ctx);
+
+/* gf_sync — wait for everything enqueued on the context's stream. */
+int gf_sync(gf_ctx* ctx);
+
+/*
+ * gf_kernel_time_ms — device time (CUDA events on the context's stream) of the half-sweep kernels
+ * launched since the last call with reset != 0: *total_ms receives their summed duration, *launches
+ * their count.  Timing is off until gf_kernel_timing(ctx, 1).  Used by bench.py for the roofline.
+ */
+int gf_kernel_timing(gf_ctx* ctx, int enable);
+int gf_kernel_time_ms(gf_ctx* ctx, double* total_ms, int* launches, int reset);
+
+/* bytes of device memory held by the context */
+int64_t gf_device_bytes(const gf_ctx* ctx);
+
+const char* gf_last_error(const gf_ctx* ctx);
+const char* gf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GF_H_ */

@@ -1,0 +1,277 @@
+// aux_kernels.cuh — everything on the path that is not the half-sweep itself:
+//   layout conversion StandardPattern <-> device store (gf_set_links / gf_get_links),
+//   F / theta reductions, reunitarisation (a10),
+//   Coulomb finalisation of the temporal links (a12).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "layout.cuh"
+#include "su3.cuh"
+#include "sweep.cuh"
+
+namespace gf {
+
+struct Dims {
+    int Nt, Nx, Ny, Nz;
+};
+
+// lexicographic site index s = ((t*Nx + x)*Ny + y)*Nz + z  ->  parity, checkerboard index
+GF_DEV void site_to_cb(const Dims& d, int64_t s, int& par, int& cb) {
+    int64_t rem = s;
+    const int z = (int)(rem % d.Nz); rem /= d.Nz;
+    const int y = (int)(rem % d.Ny); rem /= d.Ny;
+    const int x = (int)(rem % d.Nx);
+    const int t = (int)(rem / d.Nx);
+    par = (t + x + y + z) & 1;
+    cb = (int)(s >> 1);
+}
+
+// ---- StandardPattern (AoS, element type E) -> device store (R, RECON) ------------------------
+// one thread per link (site, mu); src points at the first link of site `site0`
+template <class E, class R, int RECON>
+__global__ void convert_in_kernel(const E* __restrict__ src, char* links, Dims d, int64_t site0, int64_t nsites) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nsites * 4) return;
+    const int64_t s = site0 + (i >> 2);
+    const int mu = (int)(i & 3);
+    const int64_t Vh = (int64_t)d.Nt * d.Nx * d.Ny * d.Nz / 2;
+    int par, cb;
+    site_to_cb(d, s, par, cb);
+    Mat<R> m;
+    const E* p = src + i * 18;
+#pragma unroll
+    for (int k = 0; k < 18; ++k) m.v[k] = (R)p[k];
+    global_put<R, RECON>(links + Layout<R, RECON>::link_offset(par, mu, Vh), Vh, cb, m);
+}
+template <class E, class R, int RECON>
+__global__ void convert_out_kernel(E* __restrict__ dst, const char* links, Dims d, int64_t site0, int64_t nsites) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nsites * 4) return;
+    const int64_t s = site0 + (i >> 2);
+    const int mu = (int)(i & 3);
+    const int64_t Vh = (int64_t)d.Nt * d.Nx * d.Ny * d.Nz / 2;
+    int par, cb;
+    site_to_cb(d, s, par, cb);
+    Mat<R> m;
+    global_get<R, RECON>(links + Layout<R, RECON>::link_offset(par, mu, Vh), Vh, cb, m);
+    E* p = dst + i * 18;
+#pragma unroll
+    for (int k = 0; k < 18; ++k) p[k] = (E)m.v[k];
+}
+// one-matrix-per-site field (tracked transform), always 18 reals
+template <class E, class R>
+__global__ void field_out_kernel(E* __restrict__ dst, const char* field, Dims d, int64_t site0, int64_t nsites) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nsites) return;
+    const int64_t s = site0 + i;
+    const int64_t Vh = (int64_t)d.Nt * d.Nx * d.Ny * d.Nz / 2;
+    int par, cb;
+    site_to_cb(d, s, par, cb);
+    Mat<R> m;
+    global_get<R, 18>(field + Layout<R, 18>::site_offset(par, Vh), Vh, cb, m);
+    E* p = dst + i * 18;
+#pragma unroll
+    for (int k = 0; k < 18; ++k) p[k] = (E)m.v[k];
+}
+template <class R>
+__global__ void field_identity_kernel(char* field, int64_t Vh) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 2 * Vh) return;
+    const int par = (int)(i / Vh);
+    const int cb = (int)(i % Vh);
+    Mat<R> m;
+    set_identity(m);
+    global_put<R, 18>(field + Layout<R, 18>::site_offset(par, Vh), Vh, cb, m);
+}
+
+// ---- reunitarisation: Gram-Schmidt on rows 0,1 in double, row 2 = (u x v)^* ------------------
+GF_DEV void gram_schmidt(Mat<double>& m) {
+    double nu = 0.0;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) nu += m.v[RE(0, j)] * m.v[RE(0, j)] + m.v[IM(0, j)] * m.v[IM(0, j)];
+    nu = 1.0 / sqrt(nu);
+#pragma unroll
+    for (int j = 0; j < 3; ++j) { m.v[RE(0, j)] *= nu; m.v[IM(0, j)] *= nu; }
+    double pr = 0.0, pi = 0.0;   // u^dagger v
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        pr += m.v[RE(0, j)] * m.v[RE(1, j)] + m.v[IM(0, j)] * m.v[IM(1, j)];
+        pi += m.v[RE(0, j)] * m.v[IM(1, j)] - m.v[IM(0, j)] * m.v[RE(1, j)];
+    }
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        const double ur = m.v[RE(0, j)], ui = m.v[IM(0, j)];
+        m.v[RE(1, j)] -= pr * ur - pi * ui;
+        m.v[IM(1, j)] -= pr * ui + pi * ur;
+    }
+    double nv = 0.0;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) nv += m.v[RE(1, j)] * m.v[RE(1, j)] + m.v[IM(1, j)] * m.v[IM(1, j)];
+    nv = 1.0 / sqrt(nv);
+#pragma unroll
+    for (int j = 0; j < 3; ++j) { m.v[RE(1, j)] *= nv; m.v[IM(1, j)] *= nv; }
+    reconstruct_row2(m);
+}
+
+// nmats matrices stored as planes [slot][chunk][cb] with `slot_bytes` = RECON*sizeof(R)*Vh between slots
+template <class R, int RECON>
+__global__ void reunit_kernel(char* base, int64_t Vh, int nslots) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (int64_t)nslots * Vh) return;
+    const int slot = (int)(i / Vh);
+    const int cb = (int)(i % Vh);
+    char* p0 = base + (int64_t)slot * Layout<R, RECON>::LINK_BYTES * Vh;
+    Mat<R> m;
+    global_get<R, RECON>(p0, Vh, cb, m);   // RECON=12: row 2 rebuilt here, overwritten below
+    Mat<double> w;
+#pragma unroll
+    for (int k = 0; k < 18; ++k) w.v[k] = (double)m.v[k];
+    gram_schmidt(w);
+#pragma unroll
+    for (int k = 0; k < 18; ++k) m.v[k] = (R)w.v[k];
+    global_put<R, RECON>(p0, Vh, cb, m);
+}
+
+// ---- F and theta ---------------------------------------------------------------------------
+// grid = (ceil(Vsh / block), Nt, 2): one thread per site of parity blockIdx.z in time-slice
+// blockIdx.y.  Each block writes one (F-term, theta-term) pair; slice_reduce_kernel sums them in a
+// fixed order, so results are bit-reproducible.  All arithmetic in double (BASELINE.json).
+GF_DEV double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+GF_DEV void block_sum2(double& a, double& b) {
+    __shared__ double sa[32], sb[32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    a = warp_sum(a);
+    b = warp_sum(b);
+    if (lane == 0) { sa[w] = a; sb[w] = b; }
+    __syncthreads();
+    if (w == 0) {
+        a = lane < nw ? sa[lane] : 0.0;
+        b = lane < nw ? sb[lane] : 0.0;
+        a = warp_sum(a);
+        b = warp_sum(b);
+    }
+}
+
+template <class R, int RECON, int GAUGE>
+__global__ void measure_kernel(const char* links, Dims d, double* partial) {
+    typedef Layout<R, RECON> L;
+    constexpr int MU0 = (GAUGE == GAUGE_COULOMB) ? 1 : 0;
+    const int Nzh = d.Nz >> 1;
+    const int Vsh = d.Nx * d.Ny * Nzh;
+    const int64_t Vh = (int64_t)d.Nt * Vsh;
+    const int t = blockIdx.y, par = blockIdx.z;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double f_term = 0.0, th_term = 0.0;
+    if (i < Vsh) {
+        const int cb = t * Vsh + i;
+        int rem = i;
+        const int zh = rem % Nzh; rem /= Nzh;
+        const int y = rem % d.Ny;
+        const int x = rem / d.Ny;
+        const int r = (t + x + y + par) & 1;
+        const int sy = Nzh, sx = Nzh * d.Ny, st = Vsh;
+        int cbn[4];
+        cbn[0] = cb + (t ? -st : (d.Nt - 1) * st);
+        cbn[1] = cb + (x ? -sx : (d.Nx - 1) * sx);
+        cbn[2] = cb + (y ? -sy : (d.Ny - 1) * sy);
+        cbn[3] = r ? cb : (zh ? cb - 1 : cb + Nzh - 1);
+        Mat<double> K;
+        Herm<double> M[3];
+        if (GAUGE == GAUGE_MAG) { set_zero(M[0]); set_zero(M[1]); set_zero(M[2]); }
+        else set_zero(K);
+#pragma unroll
+        for (int mu = MU0; mu < 4; ++mu) {
+            Mat<R> U;
+            global_get<R, RECON>(links + L::link_offset(par, mu, Vh), Vh, cb, U);
+            if (GAUGE == GAUGE_MAG) {
+#pragma unroll
+                for (int k = 0; k < 3; ++k)
+                    f_term += (double)U.v[RE(k, k)] * (double)U.v[RE(k, k)] + (double)U.v[IM(k, k)] * (double)U.v[IM(k, k)];
+                mag_acc_up<0>(M[0], U); mag_acc_up<1>(M[1], U); mag_acc_up<2>(M[2], U);
+            } else {
+                f_term += (double)U.v[RE(0, 0)] + (double)U.v[RE(1, 1)] + (double)U.v[RE(2, 2)];
+                acc_plain(K, U);
+            }
+            global_get<R, RECON>(links + L::link_offset(1 - par, mu, Vh), Vh, cbn[mu], U);
+            if (GAUGE == GAUGE_MAG) { mag_acc_down<0>(M[0], U); mag_acc_down<1>(M[1], U); mag_acc_down<2>(M[2], U); }
+            else acc_dagger(K, U);
+        }
+        if (GAUGE == GAUGE_MAG) {
+            // theta: sum over the three subgroups of |X^s_12|^2 = E_s^2 + F_s^2 (R11)
+            const int SI[3] = {0, 0, 1}, SJ[3] = {1, 2, 2};
+#pragma unroll
+            for (int s = 0; s < 3; ++s) {
+                const double E = M[SI[s]].o[2 * s + 1] - M[SJ[s]].o[2 * s + 1];
+                const double F = M[SI[s]].o[2 * s] - M[SJ[s]].o[2 * s];
+                th_term += E * E + F * F;
+            }
+        } else {
+            // Delta = traceless[(K - K^dag)/2i] (Eqs. (6)); tr[Delta Delta^dag] (Eq. (7))
+            double sum = 0.0, tr = 0.0;
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+#pragma unroll
+                for (int b = 0; b < 3; ++b) {
+                    const double xr = K.v[RE(a, b)] - K.v[RE(b, a)];
+                    const double xi = K.v[IM(a, b)] + K.v[IM(b, a)];
+                    sum += 0.25 * (xr * xr + xi * xi);
+                    if (a == b) tr += 0.5 * xi;   // (X/2i)_aa = Im-part
+                }
+            th_term = sum - tr * tr / 3.0;
+        }
+    }
+    block_sum2(f_term, th_term);
+    if (threadIdx.x == 0) {
+        const int64_t b = ((int64_t)(t * 2 + par)) * gridDim.x + blockIdx.x;
+        partial[2 * b] = f_term;
+        partial[2 * b + 1] = th_term;
+    }
+}
+
+// one block per time-slice: out[t] = sum of F terms, out[Nt + t] = sum of theta terms
+__global__ void slice_reduce_kernel(const double* partial, int blocks_per_slice, int Nt, double* out) {
+    const int t = blockIdx.x;
+    double a = 0.0, b = 0.0;
+    for (int k = threadIdx.x; k < blocks_per_slice; k += blockDim.x) {
+        a += partial[2 * ((int64_t)t * blocks_per_slice + k)];
+        b += partial[2 * ((int64_t)t * blocks_per_slice + k) + 1];
+    }
+    block_sum2(a, b);
+    if (threadIdx.x == 0) { out[t] = a; out[Nt + t] = b; }
+}
+
+// ---- Coulomb finalisation: U_0(x) <- R(x) U_0(x) R(x+t)^dag, R = g_tot g_applied^dag -----------
+template <class R, int RECON>
+__global__ void coulomb_finalize_kernel(char* links, const char* gtot, const char* gapp, Dims d) {
+    const int Nzh = d.Nz >> 1;
+    const int Vsh = d.Nx * d.Ny * Nzh;
+    const int64_t Vh = (int64_t)d.Nt * Vsh;
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 2 * Vh) return;
+    const int par = (int)(i / Vh);
+    const int cb = (int)(i % Vh);
+    const int t = cb / Vsh;
+    const int cbf = cb + ((t == d.Nt - 1) ? -(d.Nt - 1) * Vsh : Vsh);   // x + t_hat, other parity
+    Mat<R> U, Ga, Gb, T, O;
+    global_get<R, 18>(gtot + Layout<R, 18>::site_offset(par, Vh), Vh, cb, Ga);
+    global_get<R, 18>(gtot + Layout<R, 18>::site_offset(1 - par, Vh), Vh, cbf, Gb);
+    if (gapp) {
+        Mat<R> P;
+        global_get<R, 18>(gapp + Layout<R, 18>::site_offset(par, Vh), Vh, cb, P);
+        mul_right_dagger<3>(Ga, P, T); Ga = T;
+        global_get<R, 18>(gapp + Layout<R, 18>::site_offset(1 - par, Vh), Vh, cbf, P);
+        mul_right_dagger<3>(Gb, P, T); Gb = T;
+    }
+    char* p0 = links + Layout<R, RECON>::link_offset(par, 0, Vh);
+    global_get<R, RECON>(p0, Vh, cb, U);
+    mul_left<3>(Ga, U, T);
+    mul_right_dagger<3>(T, Gb, O);
+    global_put<R, RECON>(p0, Vh, cb, O);
+}
+
+}  // namespace gf

@@ -1,0 +1,585 @@
+// gf_api.cu — the C ABI of include/gf.h: context, dispatch and the run loops.
+// Host code only orchestrates; every step of the path runs in the kernels of sweep.cuh /
+// aux_kernels.cuh.  There is no CPU fallback.
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/gf.h"
+#include "aux_kernels.cuh"
+#include "sweep.cuh"
+
+using namespace gf;
+
+namespace gf {
+// one explicit instantiation per translation unit sweep_<prec><recon>.cu
+extern template cudaError_t launch_sweep<float, float, 18>(const SweepArgs&, int, bool, int, cudaStream_t);
+extern template cudaError_t launch_sweep<float, float, 12>(const SweepArgs&, int, bool, int, cudaStream_t);
+extern template cudaError_t launch_sweep<float, double, 18>(const SweepArgs&, int, bool, int, cudaStream_t);
+extern template cudaError_t launch_sweep<float, double, 12>(const SweepArgs&, int, bool, int, cudaStream_t);
+extern template cudaError_t launch_sweep<double, double, 18>(const SweepArgs&, int, bool, int, cudaStream_t);
+extern template cudaError_t launch_sweep<double, double, 12>(const SweepArgs&, int, bool, int, cudaStream_t);
+}  // namespace gf
+
+struct gf_ctx {
+    int Nx, Ny, Nz, Nt;
+    int precision, recon;
+    unsigned flags;
+    cudaStream_t stream;
+    int64_t V, Vh;
+    size_t real_bytes;      // 4 | 8
+    char* links;            // device link store
+    char* gtot;             // tracked transform (18 reals/site) or nullptr
+    char* gapplied;         // part of gtot already applied to the temporal links (Coulomb) or nullptr
+    bool have_links;
+    bool temporal_stale;    // Coulomb sweeps ran since the temporal links were last finalised
+    // reductions
+    double* partial;        // per-block partial sums
+    int meas_block, meas_gx;
+    double* slice_dev;      // [2*Nt]
+    double* slice_host;     // pinned [2*Nt]
+    // host<->device staging for gf_set_links / gf_get_*
+    void* staging;
+    size_t staging_bytes;
+    int64_t device_bytes;
+    int block_override;     // 0 = default CTA size
+    // kernel timing (gf_kernel_timing)
+    bool timing;
+    std::vector<cudaEvent_t> ev;   // pairs (start, stop)
+    size_t ev_used;
+    char err[512];
+};
+
+static int fail(gf_ctx* c, int code, const char* fmt, ...) {
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof(c->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+#define CU(call)                                                                                     \
+    do {                                                                                             \
+        cudaError_t e_ = (call);                                                                     \
+        if (e_ != cudaSuccess)                                                                       \
+            return fail(ctx, e_ == cudaErrorMemoryAllocation ? GF_ENOMEM : GF_ECUDA, "%s: %s (%s:%d)", #call, \
+                        cudaGetErrorString(e_), __FILE__, __LINE__);                                 \
+    } while (0)
+
+static Dims dims_of(const gf_ctx* c) {
+    Dims d = {c->Nt, c->Nx, c->Ny, c->Nz};
+    return d;
+}
+static int64_t link_store_bytes(const gf_ctx* c) { return (int64_t)8 * c->recon * c->real_bytes * c->Vh; }
+static int64_t field_store_bytes(const gf_ctx* c) { return (int64_t)2 * 18 * c->real_bytes * c->Vh; }
+
+// dispatch on (storage type, RECON)
+#define DISPATCH_RR(ctx, FN, ...)                                                  \
+    do {                                                                           \
+        if ((ctx)->real_bytes == 4) {                                              \
+            if ((ctx)->recon == 18) { FN(float, 18, __VA_ARGS__); }                \
+            else { FN(float, 12, __VA_ARGS__); }                                   \
+        } else {                                                                   \
+            if ((ctx)->recon == 18) { FN(double, 18, __VA_ARGS__); }               \
+            else { FN(double, 12, __VA_ARGS__); }                                  \
+        }                                                                          \
+    } while (0)
+
+extern "C" {
+
+const char* gf_version(void) { return "gf 0.1 (sm_100a)"; }
+
+const char* gf_last_error(const gf_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+int64_t gf_device_bytes(const gf_ctx* ctx) { return ctx ? ctx->device_bytes : 0; }
+
+int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int recon, unsigned flags,
+              void* cuda_stream) {
+    if (!out) return GF_EINVAL;
+    *out = nullptr;
+    const int n[4] = {Nx, Ny, Nz, Nt};
+    for (int k = 0; k < 4; ++k)
+        if (n[k] < 2 || (n[k] & 1)) return GF_EINVAL;
+    const double vol = (double)Nx * Ny * Nz * Nt;
+    if (vol >= 4294967296.0) return GF_EINVAL;
+    if (precision != GF_SP && precision != GF_DP && precision != GF_MP) return GF_EINVAL;
+    if (recon != 18 && recon != 12) return GF_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0) return GF_ECUDA;   // no CPU fallback
+    gf_ctx* ctx = new (std::nothrow) gf_ctx();
+    if (!ctx) return GF_ENOMEM;
+    ctx->Nx = Nx; ctx->Ny = Ny; ctx->Nz = Nz; ctx->Nt = Nt;
+    ctx->precision = precision; ctx->recon = recon; ctx->flags = flags;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    ctx->V = (int64_t)Nx * Ny * Nz * Nt;
+    ctx->Vh = ctx->V / 2;
+    ctx->real_bytes = (precision == GF_DP) ? 8 : 4;
+    ctx->links = ctx->gtot = ctx->gapplied = nullptr;
+    ctx->have_links = false; ctx->temporal_stale = false;
+    ctx->partial = nullptr; ctx->slice_dev = nullptr; ctx->slice_host = nullptr;
+    ctx->staging = nullptr; ctx->staging_bytes = 0;
+    ctx->device_bytes = 0; ctx->block_override = 0;
+    ctx->timing = false; ctx->ev_used = 0;
+    ctx->err[0] = 0;
+
+    cudaError_t e = cudaMalloc((void**)&ctx->links, (size_t)link_store_bytes(ctx));
+    if (e == cudaSuccess) ctx->device_bytes += link_store_bytes(ctx);
+    if (e == cudaSuccess && (flags & GF_FLAG_TRACK_TRANSFORM)) {
+        e = cudaMalloc((void**)&ctx->gtot, (size_t)field_store_bytes(ctx));
+        if (e == cudaSuccess) ctx->device_bytes += field_store_bytes(ctx);
+    }
+    ctx->meas_block = 128;
+    const int Vsh = Nx * Ny * (Nz / 2);
+    ctx->meas_gx = (Vsh + ctx->meas_block - 1) / ctx->meas_block;
+    const size_t npart = (size_t)ctx->meas_gx * Nt * 2;
+    if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->partial, npart * 2 * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->slice_dev, (size_t)2 * Nt * sizeof(double));
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->slice_host, (size_t)2 * Nt * sizeof(double));
+    if (e != cudaSuccess) {
+        const int code = (e == cudaErrorMemoryAllocation) ? GF_ENOMEM : GF_ECUDA;
+        gf_destroy(ctx);
+        cudaGetLastError();
+        return code;
+    }
+    ctx->device_bytes += (int64_t)(npart * 2 + 2 * Nt) * sizeof(double);
+    *out = ctx;
+    return GF_OK;
+}
+
+int gf_destroy(gf_ctx* ctx) {
+    if (!ctx) return GF_OK;
+    cudaStreamSynchronize(ctx->stream);
+    cudaFree(ctx->links);
+    cudaFree(ctx->gtot);
+    cudaFree(ctx->gapplied);
+    cudaFree(ctx->partial);
+    cudaFree(ctx->slice_dev);
+    cudaFree(ctx->staging);
+    if (ctx->slice_host) cudaFreeHost(ctx->slice_host);
+    for (cudaEvent_t ev : ctx->ev) cudaEventDestroy(ev);
+    delete ctx;
+    return GF_OK;
+}
+
+int gf_sync(gf_ctx* ctx) {
+    if (!ctx) return GF_EINVAL;
+    CU(cudaStreamSynchronize(ctx->stream));
+    return GF_OK;
+}
+
+static int ensure_staging(gf_ctx* ctx, size_t bytes) {
+    if (ctx->staging_bytes >= bytes) return GF_OK;
+    if (ctx->staging) {
+        CU(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->staging);
+        ctx->device_bytes -= (int64_t)ctx->staging_bytes;
+        ctx->staging = nullptr; ctx->staging_bytes = 0;
+    }
+    CU(cudaMalloc(&ctx->staging, bytes));
+    ctx->staging_bytes = bytes;
+    ctx->device_bytes += (int64_t)bytes;
+    return GF_OK;
+}
+
+static const int64_t STAGE_SITES = 1 << 18;   // sites per host<->device staging chunk
+
+#define CONVERT_IN(R, RECON, E, src, s0, ns)                                                            \
+    convert_in_kernel<E, R, RECON><<<(unsigned)(((ns) * 4 + 255) / 256), 256, 0, ctx->stream>>>(        \
+        (const E*)(src), ctx->links, dims_of(ctx), (s0), (ns))
+#define CONVERT_OUT(R, RECON, E, dst, s0, ns)                                                           \
+    convert_out_kernel<E, R, RECON><<<(unsigned)(((ns) * 4 + 255) / 256), 256, 0, ctx->stream>>>(       \
+        (E*)(dst), ctx->links, dims_of(ctx), (s0), (ns))
+
+static int reset_transform(gf_ctx* ctx) {
+    if (ctx->gtot) {
+        const unsigned g = (unsigned)((2 * ctx->Vh + 255) / 256);
+        if (ctx->real_bytes == 4) field_identity_kernel<float><<<g, 256, 0, ctx->stream>>>(ctx->gtot, ctx->Vh);
+        else field_identity_kernel<double><<<g, 256, 0, ctx->stream>>>(ctx->gtot, ctx->Vh);
+        CU(cudaGetLastError());
+    }
+    if (ctx->gapplied) {
+        CU(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->gapplied);
+        ctx->gapplied = nullptr;
+        ctx->device_bytes -= field_store_bytes(ctx);
+    }
+    ctx->temporal_stale = false;
+    return GF_OK;
+}
+
+int gf_set_links(gf_ctx* ctx, const void* links, int elem_bytes, int is_device) {
+    if (!ctx) return GF_EINVAL;
+    if (!links || (elem_bytes != 4 && elem_bytes != 8)) return fail(ctx, GF_EINVAL, "gf_set_links: bad arguments");
+    const int64_t link_elems = 4 * 18;
+    if (is_device) {
+        if (elem_bytes == 4) DISPATCH_RR(ctx, CONVERT_IN, float, links, (int64_t)0, ctx->V);
+        else DISPATCH_RR(ctx, CONVERT_IN, double, links, (int64_t)0, ctx->V);
+        CU(cudaGetLastError());
+    } else {
+        const int64_t chunk = ctx->V < STAGE_SITES ? ctx->V : STAGE_SITES;
+        int rc = ensure_staging(ctx, (size_t)(chunk * link_elems * elem_bytes));
+        if (rc) return rc;
+        for (int64_t s0 = 0; s0 < ctx->V; s0 += chunk) {
+            const int64_t ns = (ctx->V - s0 < chunk) ? ctx->V - s0 : chunk;
+            const char* src = (const char*)links + s0 * link_elems * elem_bytes;
+            CU(cudaMemcpyAsync(ctx->staging, src, (size_t)(ns * link_elems * elem_bytes), cudaMemcpyHostToDevice,
+                               ctx->stream));
+            if (elem_bytes == 4) DISPATCH_RR(ctx, CONVERT_IN, float, ctx->staging, s0, ns);
+            else DISPATCH_RR(ctx, CONVERT_IN, double, ctx->staging, s0, ns);
+            CU(cudaGetLastError());
+        }
+    }
+    int rc = reset_transform(ctx);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->have_links = true;
+    return GF_OK;
+}
+
+int gf_get_links(gf_ctx* ctx, void* links, int elem_bytes, int is_device) {
+    if (!ctx) return GF_EINVAL;
+    if (!links || (elem_bytes != 4 && elem_bytes != 8)) return fail(ctx, GF_EINVAL, "gf_get_links: bad arguments");
+    if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_get_links: no links set");
+    if (ctx->temporal_stale && ctx->gtot) {
+        int rc = gf_coulomb_finalize(ctx);
+        if (rc) return rc;
+    }
+    const int64_t link_elems = 4 * 18;
+    if (is_device) {
+        if (elem_bytes == 4) DISPATCH_RR(ctx, CONVERT_OUT, float, links, (int64_t)0, ctx->V);
+        else DISPATCH_RR(ctx, CONVERT_OUT, double, links, (int64_t)0, ctx->V);
+        CU(cudaGetLastError());
+    } else {
+        const int64_t chunk = ctx->V < STAGE_SITES ? ctx->V : STAGE_SITES;
+        int rc = ensure_staging(ctx, (size_t)(chunk * link_elems * elem_bytes));
+        if (rc) return rc;
+        for (int64_t s0 = 0; s0 < ctx->V; s0 += chunk) {
+            const int64_t ns = (ctx->V - s0 < chunk) ? ctx->V - s0 : chunk;
+            char* dst = (char*)links + s0 * link_elems * elem_bytes;
+            if (elem_bytes == 4) DISPATCH_RR(ctx, CONVERT_OUT, float, ctx->staging, s0, ns);
+            else DISPATCH_RR(ctx, CONVERT_OUT, double, ctx->staging, s0, ns);
+            CU(cudaGetLastError());
+            CU(cudaMemcpyAsync(dst, ctx->staging, (size_t)(ns * link_elems * elem_bytes), cudaMemcpyDeviceToHost,
+                               ctx->stream));
+        }
+    }
+    CU(cudaStreamSynchronize(ctx->stream));
+    return GF_OK;
+}
+
+int gf_get_gauge_transform(gf_ctx* ctx, void* g, int elem_bytes, int is_device) {
+    if (!ctx) return GF_EINVAL;
+    if (!g || (elem_bytes != 4 && elem_bytes != 8)) return fail(ctx, GF_EINVAL, "gf_get_gauge_transform: bad arguments");
+    if (!ctx->gtot) return fail(ctx, GF_ESTATE, "gf_get_gauge_transform: context created without GF_FLAG_TRACK_TRANSFORM");
+    const int64_t chunk = is_device ? ctx->V : (ctx->V < 4 * STAGE_SITES ? ctx->V : 4 * STAGE_SITES);
+    if (!is_device) {
+        int rc = ensure_staging(ctx, (size_t)(chunk * 18 * elem_bytes));
+        if (rc) return rc;
+    }
+    for (int64_t s0 = 0; s0 < ctx->V; s0 += chunk) {
+        const int64_t ns = (ctx->V - s0 < chunk) ? ctx->V - s0 : chunk;
+        void* dst = is_device ? (void*)((char*)g + s0 * 18 * elem_bytes) : ctx->staging;
+        const unsigned grid = (unsigned)((ns + 255) / 256);
+        if (ctx->real_bytes == 4) {
+            if (elem_bytes == 4) field_out_kernel<float, float><<<grid, 256, 0, ctx->stream>>>((float*)dst, ctx->gtot, dims_of(ctx), s0, ns);
+            else field_out_kernel<double, float><<<grid, 256, 0, ctx->stream>>>((double*)dst, ctx->gtot, dims_of(ctx), s0, ns);
+        } else {
+            if (elem_bytes == 4) field_out_kernel<float, double><<<grid, 256, 0, ctx->stream>>>((float*)dst, ctx->gtot, dims_of(ctx), s0, ns);
+            else field_out_kernel<double, double><<<grid, 256, 0, ctx->stream>>>((double*)dst, ctx->gtot, dims_of(ctx), s0, ns);
+        }
+        CU(cudaGetLastError());
+        if (!is_device)
+            CU(cudaMemcpyAsync((char*)g + s0 * 18 * elem_bytes, ctx->staging, (size_t)(ns * 18 * elem_bytes),
+                               cudaMemcpyDeviceToHost, ctx->stream));
+    }
+    CU(cudaStreamSynchronize(ctx->stream));
+    return GF_OK;
+}
+
+// ---- sweeps ----------------------------------------------------------------------------------
+static int check_sweep_args(gf_ctx* ctx, int gauge, int algo, double param) {
+    if (!ctx) return GF_EINVAL;
+    if (!ctx->have_links) return fail(ctx, GF_ESTATE, "no links set (call gf_set_links first)");
+    if (gauge < GF_LANDAU || gauge > GF_MAG) return fail(ctx, GF_EINVAL, "unknown gauge %d", gauge);
+    if (algo < GF_OR || algo > GF_MICRO) return fail(ctx, GF_EINVAL, "unknown algorithm %d", algo);
+    if (algo == GF_OR && !(param >= 1.0 && param < 2.0)) return fail(ctx, GF_EINVAL, "omega = %g not in [1,2)", param);
+    if (algo == GF_SR && !(param >= 0.0 && param <= 1.0)) return fail(ctx, GF_EINVAL, "p = %g not in [0,1]", param);
+    if (algo == GF_SA && !(param > 0.0)) return fail(ctx, GF_EINVAL, "T = %g not positive", param);
+    return GF_OK;
+}
+
+static int launch_half(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t sweep_index,
+                       int parity) {
+    SweepArgs a;
+    a.links = ctx->links; a.gtot = ctx->gtot;
+    a.Nt = ctx->Nt; a.Nx = ctx->Nx; a.Ny = ctx->Ny; a.Nz = ctx->Nz;
+    a.parity = parity; a.algo = algo; a.param = param; a.seed = seed; a.sweep_index = sweep_index;
+    a.red = nullptr;
+    const bool track = ctx->gtot != nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (ctx->timing) {
+        if (ctx->ev_used + 2 > ctx->ev.size()) {
+            cudaEvent_t a0, a1;
+            CU(cudaEventCreate(&a0));
+            CU(cudaEventCreate(&a1));
+            ctx->ev.push_back(a0);
+            ctx->ev.push_back(a1);
+        }
+        e0 = ctx->ev[ctx->ev_used]; e1 = ctx->ev[ctx->ev_used + 1];
+        ctx->ev_used += 2;
+        CU(cudaEventRecord(e0, ctx->stream));
+    }
+    cudaError_t e;
+    const int blk = ctx->block_override;
+    if (ctx->precision == GF_DP) {
+        e = (ctx->recon == 18) ? launch_sweep<double, double, 18>(a, gauge, track, blk, ctx->stream)
+                               : launch_sweep<double, double, 12>(a, gauge, track, blk, ctx->stream);
+    } else if (ctx->precision == GF_MP) {
+        e = (ctx->recon == 18) ? launch_sweep<float, double, 18>(a, gauge, track, blk, ctx->stream)
+                               : launch_sweep<float, double, 12>(a, gauge, track, blk, ctx->stream);
+    } else {
+        e = (ctx->recon == 18) ? launch_sweep<float, float, 18>(a, gauge, track, blk, ctx->stream)
+                               : launch_sweep<float, float, 12>(a, gauge, track, blk, ctx->stream);
+    }
+    CU(e);
+    if (ctx->timing) CU(cudaEventRecord(e1, ctx->stream));
+    return GF_OK;
+}
+
+static int pre_sweep(gf_ctx* ctx, int gauge) {
+    if (gauge == GF_COULOMB) {
+        if (ctx->gtot) ctx->temporal_stale = true;
+    } else if (ctx->temporal_stale) {
+        return gf_coulomb_finalize(ctx);
+    }
+    return GF_OK;
+}
+
+int gf_half_sweep(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t sweep_index,
+                  int parity) {
+    int rc = check_sweep_args(ctx, gauge, algo, param);
+    if (rc) return rc;
+    if (parity != 0 && parity != 1) return fail(ctx, GF_EINVAL, "parity %d", parity);
+    rc = pre_sweep(ctx, gauge);
+    if (rc) return rc;
+    return launch_half(ctx, gauge, algo, param, seed, sweep_index, parity);
+}
+
+int gf_sweep(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t sweep_index) {
+    int rc = check_sweep_args(ctx, gauge, algo, param);
+    if (rc) return rc;
+    rc = pre_sweep(ctx, gauge);
+    if (rc) return rc;
+    rc = launch_half(ctx, gauge, algo, param, seed, sweep_index, 0);   // even first (Alg. 1)
+    if (rc) return rc;
+    return launch_half(ctx, gauge, algo, param, seed, sweep_index, 1);
+}
+
+// ---- reductions --------------------------------------------------------------------------------
+#define MEASURE(R, RECON, gauge_)                                                                          \
+    do {                                                                                                   \
+        dim3 grid((unsigned)ctx->meas_gx, (unsigned)ctx->Nt, 2);                                           \
+        if ((gauge_) == GF_LANDAU)                                                                         \
+            measure_kernel<R, RECON, GAUGE_LANDAU><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial); \
+        else if ((gauge_) == GF_COULOMB)                                                                   \
+            measure_kernel<R, RECON, GAUGE_COULOMB><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial); \
+        else                                                                                               \
+            measure_kernel<R, RECON, GAUGE_MAG><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial); \
+    } while (0)
+
+// enqueue the reduction and the copy of the 2*Nt slice sums to pinned host memory
+static int enqueue_measure(gf_ctx* ctx, int gauge) {
+    DISPATCH_RR(ctx, MEASURE, gauge);
+    CU(cudaGetLastError());
+    slice_reduce_kernel<<<ctx->Nt, 128, 0, ctx->stream>>>(ctx->partial, 2 * ctx->meas_gx, ctx->Nt, ctx->slice_dev);
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(ctx->slice_host, ctx->slice_dev, (size_t)2 * ctx->Nt * sizeof(double), cudaMemcpyDeviceToHost,
+                       ctx->stream));
+    return GF_OK;
+}
+
+// after a stream sync: normalise (Eqs. (4), (7), (11)) in a fixed order
+static void finish_measure(const gf_ctx* ctx, int gauge, double* F, double* theta, double* theta_slice,
+                           double* theta_max) {
+    const int nd = (gauge == GF_COULOMB) ? 3 : 4;
+    const double Vs = (double)ctx->Nx * ctx->Ny * ctx->Nz;
+    double fs = 0.0, ths = 0.0, tmax = 0.0;
+    for (int t = 0; t < ctx->Nt; ++t) {
+        fs += ctx->slice_host[t];
+        ths += ctx->slice_host[ctx->Nt + t];
+        const double th_t = ctx->slice_host[ctx->Nt + t] / (3.0 * Vs);
+        if (theta_slice) theta_slice[t] = th_t;
+        if (th_t > tmax) tmax = th_t;
+    }
+    if (F) *F = fs / (3.0 * nd * (double)ctx->V);
+    if (theta) *theta = ths / (3.0 * (double)ctx->V);
+    if (theta_max) *theta_max = tmax;
+}
+
+int gf_measure(gf_ctx* ctx, int gauge, double* F, double* theta, double* theta_slice) {
+    if (!ctx) return GF_EINVAL;
+    if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_measure: no links set");
+    if (gauge < GF_LANDAU || gauge > GF_MAG) return fail(ctx, GF_EINVAL, "unknown gauge %d", gauge);
+    if (gauge != GF_COULOMB && ctx->temporal_stale) {
+        int rc = gf_coulomb_finalize(ctx);
+        if (rc) return rc;
+    }
+    int rc = enqueue_measure(ctx, gauge);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(ctx->stream));
+    finish_measure(ctx, gauge, F, theta, theta_slice, nullptr);
+    return GF_OK;
+}
+
+// ---- reunitarisation -----------------------------------------------------------------------------
+#define REUNIT_LINKS(R, RECON, dummy)                                                                       \
+    reunit_kernel<R, RECON><<<(unsigned)((8 * ctx->Vh + 255) / 256), 256, 0, ctx->stream>>>(ctx->links, ctx->Vh, 8)
+
+int gf_reunitarize(gf_ctx* ctx) {
+    if (!ctx) return GF_EINVAL;
+    if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_reunitarize: no links set");
+    DISPATCH_RR(ctx, REUNIT_LINKS, 0);
+    CU(cudaGetLastError());
+    if (ctx->gtot) {
+        const unsigned g = (unsigned)((2 * ctx->Vh + 255) / 256);
+        if (ctx->real_bytes == 4) reunit_kernel<float, 18><<<g, 256, 0, ctx->stream>>>(ctx->gtot, ctx->Vh, 2);
+        else reunit_kernel<double, 18><<<g, 256, 0, ctx->stream>>>(ctx->gtot, ctx->Vh, 2);
+        CU(cudaGetLastError());
+    }
+    return GF_OK;
+}
+
+// ---- Coulomb finalisation ------------------------------------------------------------------------
+#define FINALIZE(R, RECON, dummy)                                                                           \
+    coulomb_finalize_kernel<R, RECON><<<(unsigned)((2 * ctx->Vh + 127) / 128), 128, 0, ctx->stream>>>(       \
+        ctx->links, ctx->gtot, ctx->gapplied, dims_of(ctx))
+
+int gf_coulomb_finalize(gf_ctx* ctx) {
+    if (!ctx) return GF_EINVAL;
+    if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_coulomb_finalize: no links set");
+    if (!ctx->gtot) return fail(ctx, GF_ESTATE, "gf_coulomb_finalize: context created without GF_FLAG_TRACK_TRANSFORM");
+    if (!ctx->temporal_stale) return GF_OK;
+    DISPATCH_RR(ctx, FINALIZE, 0);
+    CU(cudaGetLastError());
+    if (!ctx->gapplied) {
+        CU(cudaMalloc((void**)&ctx->gapplied, (size_t)field_store_bytes(ctx)));
+        ctx->device_bytes += field_store_bytes(ctx);
+    }
+    CU(cudaMemcpyAsync(ctx->gapplied, ctx->gtot, (size_t)field_store_bytes(ctx), cudaMemcpyDeviceToDevice, ctx->stream));
+    ctx->temporal_stale = false;
+    return GF_OK;
+}
+
+// ---- run loops -----------------------------------------------------------------------------------
+int gf_run(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t first_sweep_index,
+           int max_sweeps, double eps, int check_every, int reunit_every, gf_result* out, double* hist) {
+    int rc = check_sweep_args(ctx, gauge, algo, param);
+    if (rc) return rc;
+    if (max_sweeps < 0 || check_every < 1 || reunit_every < 0) return fail(ctx, GF_EINVAL, "gf_run: bad loop arguments");
+    rc = pre_sweep(ctx, gauge);
+    if (rc) return rc;
+    double F = 0.0, theta = 0.0, tmax = 0.0, stop = 0.0;
+    bool measured = false, converged = false;
+    int s = 0, nh = 0;
+    while (s < max_sweeps) {
+        rc = launch_half(ctx, gauge, algo, param, seed, first_sweep_index + (uint32_t)s, 0);
+        if (rc) return rc;
+        rc = launch_half(ctx, gauge, algo, param, seed, first_sweep_index + (uint32_t)s, 1);
+        if (rc) return rc;
+        ++s;
+        if (reunit_every && s % reunit_every == 0) {
+            rc = gf_reunitarize(ctx);
+            if (rc) return rc;
+        }
+        if (s % check_every == 0 || s == max_sweeps) {
+            rc = enqueue_measure(ctx, gauge);
+            if (rc) return rc;
+            CU(cudaStreamSynchronize(ctx->stream));
+            finish_measure(ctx, gauge, &F, &theta, nullptr, &tmax);
+            stop = (gauge == GF_COULOMB) ? tmax : theta;
+            measured = true;
+            if (hist) { hist[3 * nh] = (double)s; hist[3 * nh + 1] = F; hist[3 * nh + 2] = stop; }
+            ++nh;
+            if (stop < eps) { converged = true; break; }
+        }
+    }
+    if (!measured) {
+        rc = enqueue_measure(ctx, gauge);
+        if (rc) return rc;
+        CU(cudaStreamSynchronize(ctx->stream));
+        finish_measure(ctx, gauge, &F, &theta, nullptr, &tmax);
+        stop = (gauge == GF_COULOMB) ? tmax : theta;
+        converged = stop < eps;
+    }
+    if (gauge == GF_COULOMB && ctx->gtot) {
+        rc = gf_coulomb_finalize(ctx);
+        if (rc) return rc;
+        CU(cudaStreamSynchronize(ctx->stream));
+    }
+    if (out) { out->sweeps = s; out->F = F; out->theta = stop; }
+    return converged ? GF_OK : GF_NOT_CONVERGED;
+}
+
+int gf_anneal(gf_ctx* ctx, int gauge, double T_hi, double T_lo, int n_steps, int n_micro, uint64_t seed,
+              uint32_t first_sweep_index, uint32_t* next_sweep_index) {
+    int rc = check_sweep_args(ctx, gauge, GF_SA, T_hi);
+    if (rc) return rc;
+    if (!(T_lo > 0.0) || n_steps < 0 || n_micro < 0) return fail(ctx, GF_EINVAL, "gf_anneal: bad schedule");
+    rc = pre_sweep(ctx, gauge);
+    if (rc) return rc;
+    uint32_t idx = first_sweep_index;
+    for (int k = 0; k < n_steps; ++k) {
+        const double T = (n_steps <= 1) ? T_hi : T_hi - k * (T_hi - T_lo) / (n_steps - 1);
+        for (int p = 0; p < 2; ++p) {
+            rc = launch_half(ctx, gauge, GF_SA, T, seed, idx, p);
+            if (rc) return rc;
+        }
+        ++idx;
+        for (int m = 0; m < n_micro; ++m) {
+            for (int p = 0; p < 2; ++p) {
+                rc = launch_half(ctx, gauge, GF_MICRO, 0.0, seed, idx, p);
+                if (rc) return rc;
+            }
+            ++idx;
+        }
+    }
+    if (next_sweep_index) *next_sweep_index = idx;
+    return GF_OK;
+}
+
+// ---- instrumentation -----------------------------------------------------------------------------
+int gf_kernel_timing(gf_ctx* ctx, int enable) {
+    if (!ctx) return GF_EINVAL;
+    ctx->timing = enable != 0;
+    return GF_OK;
+}
+
+int gf_kernel_time_ms(gf_ctx* ctx, double* total_ms, int* launches, int reset) {
+    if (!ctx) return GF_EINVAL;
+    CU(cudaStreamSynchronize(ctx->stream));
+    double tot = 0.0;
+    for (size_t k = 0; k + 1 < ctx->ev_used; k += 2) {
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, ctx->ev[k], ctx->ev[k + 1]));
+        tot += ms;
+    }
+    if (total_ms) *total_ms = tot;
+    if (launches) *launches = (int)(ctx->ev_used / 2);
+    if (reset) ctx->ev_used = 0;
+    return GF_OK;
+}
+
+// tuning hook (not declared in gf.h): CTA size of the half-sweep kernel, 0 = default
+int gf_debug_set_block(gf_ctx* ctx, int block) {
+    if (!ctx || block < 0 || (block & 31)) return GF_EINVAL;
+    ctx->block_override = block;
+    return GF_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,303 @@
+// sweep.cuh — the half-sweep kernel: Alg. 1's "for all x of sublattice" for
+// one parity, one thread per site (BASELINE.json north_star), sm_100a.
+//
+// Design: the 2d links of a site are streamed once from HBM into the thread's
+// private slice of shared memory with 16-byte cp.async (no register staging, 2d*R*s bytes in flight
+// per thread), then
+//   pass 1  builds the neighbourhood summary in registers: K(x) of Eq. (19) for
+//           Landau/Coulomb, the three Hermitian M_k for MAG;
+//   Step 1  runs the three Cabibbo-Marinari subgroup updates on the summary
+//           alone (K -> g K, M_k -> g M_k g^dagger), accumulating G = g3 g2 g1;
+//   pass 2  re-reads each link from shared memory, rotates it once with the SU(3) matrix G
+//           (Step 2: U_mu(x) <- G U_mu(x), U_mu(x-mu) <- U_mu(x-mu) G^dagger)
+//           and writes it back in place with 16-byte stores.
+// Every link is read once and written once per half-sweep; nothing is re-read from HBM.  No
+// __syncthreads: a thread only ever touches its own shared-memory slice.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "layout.cuh"
+#include "step1.cuh"
+#include "su3.cuh"
+
+namespace gf {
+
+enum { GAUGE_LANDAU = 0, GAUGE_COULOMB = 1, GAUGE_MAG = 2 };
+
+struct SweepArgs {
+    char* links;   // device link store (layout.cuh)
+    char* gtot;    // tracked transform store or nullptr
+    int Nt, Nx, Ny, Nz;
+    int parity;          // active parity of this half-sweep
+    int algo;            // ALGO_*
+    double param;        // omega | p | T
+    uint64_t seed;
+    uint32_t sweep_index;
+    double* red;         // nullptr, or per-block partial sums [gridDim.x][2] of (F, theta) terms
+};
+
+// ---- asynchronous global -> shared copies -------------------------------------------------
+GF_DEV void cp_async16(uint32_t saddr, const void* g) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(saddr), "l"(g) : "memory");
+}
+GF_DEV void cp_async8(uint32_t saddr, const void* g) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(saddr), "l"(g) : "memory");
+}
+GF_DEV void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
+
+// ---- 16-byte vector moves between shared/global memory and a register matrix ------------------
+template <class R>
+struct Vec16;
+template <>
+struct Vec16<float> {
+    typedef float4 type;
+    GF_DEV static void unpack(const float4& q, float* v) { v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w; }
+    GF_DEV static float4 pack(const float* v) { return make_float4(v[0], v[1], v[2], v[3]); }
+};
+template <>
+struct Vec16<double> {
+    typedef double2 type;
+    GF_DEV static void unpack(const double2& q, double* v) { v[0] = q.x; v[1] = q.y; }
+    GF_DEV static double2 pack(const double* v) { return make_double2(v[0], v[1]); }
+};
+
+// read link slot l of this thread from shared memory (and rebuild row 2 when RECON = 12)
+template <class R, int RECON>
+GF_DEV void smem_get(const unsigned char* smem, int nlinks, int l, Mat<R>& m) {
+    typedef Layout<R, RECON> L;
+    typedef typename Vec16<R>::type V;
+    const int nthr = blockDim.x, tid = threadIdx.x;
+#pragma unroll
+    for (int c = 0; c < L::NV16; ++c) {
+        const V q = *reinterpret_cast<const V*>(smem + ((size_t)(l * L::NV16 + c) * nthr + tid) * 16);
+        Vec16<R>::unpack(q, &m.v[c * L::PER16]);
+    }
+    if (L::TAIL8) {
+        const float2 q = *reinterpret_cast<const float2*>(smem + (size_t)nlinks * L::NV16 * nthr * 16 +
+                                                          ((size_t)l * nthr + tid) * 8);
+        m.v[L::NV16 * L::PER16] = (R)q.x;
+        m.v[L::NV16 * L::PER16 + 1] = (R)q.y;
+    }
+    if (RECON == 12) reconstruct_row2(m);
+}
+
+// store the first RECON reals of a matrix to its place in HBM
+template <class R, int RECON>
+GF_DEV void global_put(char* plane0, int64_t Vh, int cb, const Mat<R>& m) {
+    typedef Layout<R, RECON> L;
+    typedef typename Vec16<R>::type V;
+#pragma unroll
+    for (int c = 0; c < L::NV16; ++c)
+        *reinterpret_cast<V*>(plane0 + (int64_t)c * 16 * Vh + (int64_t)cb * 16) = Vec16<R>::pack(&m.v[c * L::PER16]);
+    if (L::TAIL8)
+        *reinterpret_cast<float2*>(plane0 + (int64_t)L::NV16 * 16 * Vh + (int64_t)cb * 8) =
+            make_float2((float)m.v[L::NV16 * L::PER16], (float)m.v[L::NV16 * L::PER16 + 1]);
+}
+template <class R, int RECON>
+GF_DEV void global_get(const char* plane0, int64_t Vh, int cb, Mat<R>& m) {
+    typedef Layout<R, RECON> L;
+    typedef typename Vec16<R>::type V;
+#pragma unroll
+    for (int c = 0; c < L::NV16; ++c) {
+        const V q = *reinterpret_cast<const V*>(plane0 + (int64_t)c * 16 * Vh + (int64_t)cb * 16);
+        Vec16<R>::unpack(q, &m.v[c * L::PER16]);
+    }
+    if (L::TAIL8) {
+        const float2 q = *reinterpret_cast<const float2*>(plane0 + (int64_t)L::NV16 * 16 * Vh + (int64_t)cb * 8);
+        m.v[L::NV16 * L::PER16] = (R)q.x;
+        m.v[L::NV16 * L::PER16 + 1] = (R)q.y;
+    }
+    if (RECON == 12) reconstruct_row2(m);
+}
+
+// ---- Step 1 for one subgroup (I,J), index S in the Cabibbo-Marinari order (0,1),(0,2),(1,2) ----
+template <bool STOCH, class A>
+GF_DEV void choose_rule(const A a[4], A g[4], bool mag, A Dm, A Em, A Fm, const SweepArgs& args, uint32_t site,
+                        int sub) {
+    if (!STOCH) {
+        if (args.algo == ALGO_MICRO) rule_micro<A>(a, g);
+        else rule_or<A>(a, (A)args.param, g);
+    } else {
+        if (args.algo == ALGO_SR) {
+            // stochastic relaxation: g^2 with probability p, else g
+            const double u = uniform01(rng_draw(args.seed, site, args.sweep_index, sub, 0, 0).x);
+            if (u < args.param) rule_micro<A>(a, g);
+            else rule_or<A>(a, A(1), g);
+        } else {
+            double gd[4];
+            if (mag) {
+                rule_heatbath_mag((double)Dm, (double)Em, (double)Fm, args.param, args.seed, site, args.sweep_index,
+                                  sub, gd);
+            } else {
+                const double ad[4] = {(double)a[0], (double)a[1], (double)a[2], (double)a[3]};
+                rule_heatbath_landau(ad, args.param, args.seed, site, args.sweep_index, sub, gd);
+            }
+            g[0] = (A)gd[0]; g[1] = (A)gd[1]; g[2] = (A)gd[2]; g[3] = (A)gd[3];
+        }
+    }
+}
+
+template <int I, int J, int S, bool STOCH, class A>
+GF_DEV void subgroup_landau(Mat<A>& K, Mat<A>& G, const SweepArgs& args, uint32_t site) {
+    // Fig. A.10 on K, signs per Eq. (15)
+    A a[4], g[4];
+    a[0] = K.v[RE(I, I)] + K.v[RE(J, J)];
+    a[3] = K.v[IM(I, I)] - K.v[IM(J, J)];
+    a[2] = K.v[RE(I, J)] - K.v[RE(J, I)];
+    a[1] = K.v[IM(I, J)] + K.v[IM(J, I)];
+    choose_rule<STOCH, A>(a, g, false, A(0), A(0), A(0), args, site, S);
+    sub_left<I, J>(K, g);   // applying g at x maps K(x) -> g K(x)
+    sub_left<I, J>(G, g);
+}
+
+template <int I, int J, int S, bool STOCH, class A>
+GF_DEV void subgroup_mag(Herm<A> (&M)[3], Mat<A>& G, const SweepArgs& args, uint32_t site) {
+    // f(g) = const + g^T [[D,E,F],[E,-D,0],[F,0,-D]] g  (Eqs. (25)-(28), SU(3) form)
+    // (I,J) with I < J: off-diagonal element (I,J) of a Herm is o[2*OFF], o[2*OFF+1]
+    constexpr int OFF = (I == 0) ? (J - 1) : 2;
+    const A aa = M[I].d[I] + M[J].d[J];
+    const A bb = M[I].d[J] + M[J].d[I];
+    const A Dm = (aa - bb) / A(2);
+    const A Em = M[I].o[2 * OFF + 1] - M[J].o[2 * OFF + 1];
+    const A Fm = M[I].o[2 * OFF] - M[J].o[2 * OFF];
+    const A lam = sqrt_t(Dm * Dm + Em * Em + Fm * Fm);   // Eq. (29)
+    A a[4] = {Dm + lam, -Em, -Fm, A(0)}, g[4];
+    choose_rule<STOCH, A>(a, g, true, Dm, Em, Fm, args, site, S);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {   // M_k -> g M_k g^dagger
+        Mat<A> F;
+        herm_expand(M[k], F);
+        sub_left<I, J>(F, g);
+        sub_right_dagger<I, J>(F, g);
+        herm_compress(F, M[k]);
+    }
+    sub_left<I, J>(G, g);
+}
+
+// ---- the kernel ----------------------------------------------------------------------------
+template <class R>
+struct SweepLaunch {   // CTA shape per storage type
+    static constexpr int MAX_BLOCK = sizeof(R) == 4 ? 128 : 64;
+    static constexpr int MIN_CTAS = sizeof(R) == 4 ? 3 : 3;
+};
+
+template <class R, class A, int RECON, int GAUGE, bool STOCH, bool TRACK>
+__global__ void __launch_bounds__(SweepLaunch<R>::MAX_BLOCK, SweepLaunch<R>::MIN_CTAS)
+sweep_kernel(const SweepArgs args) {
+    typedef Layout<R, RECON> L;
+    constexpr int MU0 = (GAUGE == GAUGE_COULOMB) ? 1 : 0;
+    constexpr int ND = 4 - MU0;
+    constexpr int NL = 2 * ND;
+    extern __shared__ __align__(16) unsigned char smem[];
+
+    const int64_t Vh = (int64_t)args.Nt * args.Nx * args.Ny * (args.Nz / 2);
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= Vh) return;   // no barriers below, so early exit is safe
+    const int cb = (int)idx;
+
+    // ---- a1: decode the checkerboard index, neighbours with periodic wrap ----
+    const int Nzh = args.Nz >> 1;
+    int rem = cb;
+    const int zh = rem % Nzh; rem /= Nzh;
+    const int y = rem % args.Ny; rem /= args.Ny;
+    const int x = rem % args.Nx;
+    const int t = rem / args.Nx;
+    // own parity in the 4-d colouring; Coulomb's 3-d colouring p3 maps to (p3 + t) & 1
+    const int par = (GAUGE == GAUGE_COULOMB) ? ((args.parity + t) & 1) : args.parity;
+    const int r = (t + x + y + par) & 1;   // z = 2 zh + r
+    const int z = 2 * zh + r;
+    const uint32_t site = (uint32_t)(((t * args.Nx + x) * args.Ny + y) * args.Nz + z);
+
+    // checkerboard index of x - mu (lives in the other parity's arrays)
+    const int sy = Nzh, sx = Nzh * args.Ny, st = Nzh * args.Ny * args.Nx;
+    const int cbn0 = cb + (t ? -st : (args.Nt - 1) * st);
+    const int cbn1 = cb + (x ? -sx : (args.Nx - 1) * sx);
+    const int cbn2 = cb + (y ? -sy : (args.Ny - 1) * sy);
+    const int cbn3 = r ? cb : (zh ? cb - 1 : cb + Nzh - 1);
+
+    // ---- a2: stream the 2d links into this thread's shared-memory slice ----
+    const int nthr = blockDim.x, tid = threadIdx.x;
+    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem);
+#pragma unroll
+    for (int l = 0; l < NL; ++l) {
+        const int mu = MU0 + (l >> 1);
+        const bool down = l & 1;
+        const char* p0 = args.links + L::link_offset(down ? 1 - par : par, mu, Vh);
+        const int c_site = !down ? cb : (mu == 0) ? cbn0 : (mu == 1) ? cbn1 : (mu == 2) ? cbn2 : cbn3;
+#pragma unroll
+        for (int c = 0; c < L::NV16; ++c)
+            cp_async16(sbase + (uint32_t)(((l * L::NV16 + c) * nthr + tid) * 16),
+                       p0 + (int64_t)c * 16 * Vh + (int64_t)c_site * 16);
+        if (L::TAIL8)
+            cp_async8(sbase + (uint32_t)(NL * L::NV16 * nthr * 16 + (l * nthr + tid) * 8),
+                      p0 + (int64_t)L::NV16 * 16 * Vh + (int64_t)c_site * 8);
+    }
+    Mat<R> Gt;
+    if (TRACK) global_get<R, 18>(args.gtot + Layout<R, 18>::site_offset(par, Vh), Vh, cb, Gt);
+    cp_async_wait_all();
+
+    // ---- a3: neighbourhood summary, pass 1 over the links ----
+    // (loops over mu are deliberately not unrolled: one link pair in registers at a time)
+    Mat<A> G;
+    set_identity(G);
+    Mat<A> K;             // Landau/Coulomb: Eq. (19)
+    Herm<A> M[3];         // MAG: Hermitian M_k
+    if (GAUGE == GAUGE_MAG) {
+        set_zero(M[0]); set_zero(M[1]); set_zero(M[2]);
+    } else {
+        set_zero(K);
+    }
+#pragma unroll 1
+    for (int m = 0; m < ND; ++m) {
+        Mat<R> U;
+        smem_get<R, RECON>(smem, NL, 2 * m, U);       // U_mu(x)
+        if (GAUGE == GAUGE_MAG) { mag_acc_up<0>(M[0], U); mag_acc_up<1>(M[1], U); mag_acc_up<2>(M[2], U); }
+        else acc_plain(K, U);
+        smem_get<R, RECON>(smem, NL, 2 * m + 1, U);   // U_mu(x - mu)
+        if (GAUGE == GAUGE_MAG) { mag_acc_down<0>(M[0], U); mag_acc_down<1>(M[1], U); mag_acc_down<2>(M[2], U); }
+        else acc_dagger(K, U);
+    }
+
+    // ---- a4/a5: Step 1 through the three SU(2) subgroups, G = g3 g2 g1 ----
+    if (GAUGE == GAUGE_MAG) {
+        subgroup_mag<0, 1, 0, STOCH, A>(M, G, args, site);
+        subgroup_mag<0, 2, 1, STOCH, A>(M, G, args, site);
+        subgroup_mag<1, 2, 2, STOCH, A>(M, G, args, site);
+    } else {
+        subgroup_landau<0, 1, 0, STOCH, A>(K, G, args, site);
+        subgroup_landau<0, 2, 1, STOCH, A>(K, G, args, site);
+        subgroup_landau<1, 2, 2, STOCH, A>(K, G, args, site);
+    }
+
+    // ---- a6/a7: Step 2, pass 2 over the links: rotate and write back in place ----
+    constexpr int NR = (RECON == 12) ? 2 : 3;
+    Mat<R> Gr;   // G in the storage type (MP: Step 2 in SP)
+#pragma unroll
+    for (int k = 0; k < 18; ++k) Gr.v[k] = (R)G.v[k];
+#pragma unroll 1
+    for (int m = 0; m < ND; ++m) {
+        const int mu = MU0 + m;
+        const int cdn = (mu == 0) ? cbn0 : (mu == 1) ? cbn1 : (mu == 2) ? cbn2 : cbn3;
+        Mat<R> U, O;
+        smem_get<R, RECON>(smem, NL, 2 * m, U);
+        mul_left<NR>(Gr, U, O);
+        global_put<R, RECON>(args.links + L::link_offset(par, mu, Vh), Vh, cb, O);
+        smem_get<R, RECON>(smem, NL, 2 * m + 1, U);
+        mul_right_dagger<NR>(U, Gr, O);
+        global_put<R, RECON>(args.links + L::link_offset(1 - par, mu, Vh), Vh, cdn, O);
+    }
+
+    // ---- a8: accumulate the transform, g_tot(x) <- G g_tot(x) ----
+    if (TRACK) {
+        Mat<R> O;
+        mul_left<3>(G, Gt, O);
+        global_put<R, 18>(args.gtot + Layout<R, 18>::site_offset(par, Vh), Vh, cb, O);
+    }
+}
+
+// host-side launcher of one (R, A, RECON) family; defined in sweep_inst.cuh
+template <class R, class A, int RECON>
+cudaError_t launch_sweep(const SweepArgs& args, int gauge, bool track, int block, cudaStream_t stream);
+
+}  // namespace gf

@@ -1,0 +1,5 @@
+// half-sweep kernels: storage float, Step 1 in double, 18 reals per stored link
+#include "sweep_inst.cuh"
+namespace gf {
+template cudaError_t launch_sweep<float, double, 18>(const SweepArgs&, int, bool, int, cudaStream_t);
+}

@@ -1,0 +1,275 @@
+"""Thin Python binding of libgf.so (include/gf.h): argument marshalling only.
+
+Every function has the name and the argument order of the C entry point it forwards to; all
+arithmetic of the method runs in the CUDA kernels behind the ABI.  Buffers may be NumPy arrays
+(host), CPU torch tensors (host, pinned or not) or CUDA torch tensors (device); PyTorch is used for
+device memory and streams only.  The library is loaded at import and the import fails loudly if
+``libgf.so`` has not been built (``python -m paper_1212_5221_b200.build``): there is no fallback.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgf.so")
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1212_5221_b200.build` "
+                      "(nvcc, sm_100a). There is no CPU fallback.")
+_lib = ctypes.CDLL(LIB_PATH)
+
+# constants of include/gf.h
+GF_OK, GF_NOT_CONVERGED, GF_EINVAL, GF_ENOMEM, GF_ECUDA, GF_ESTATE = 0, 1, -1, -2, -3, -4
+GF_SP, GF_DP, GF_MP = 0, 1, 2
+GF_LANDAU, GF_COULOMB, GF_MAG = 0, 1, 2
+GF_OR, GF_SR, GF_SA, GF_MICRO = 0, 1, 2, 3
+GF_FLAG_TRACK_TRANSFORM = 1
+
+EXPORTS = ["gf_create", "gf_destroy", "gf_set_links", "gf_get_links", "gf_get_gauge_transform", "gf_sweep",
+           "gf_half_sweep", "gf_measure", "gf_run", "gf_anneal", "gf_reunitarize", "gf_coulomb_finalize",
+           "gf_sync", "gf_kernel_timing", "gf_kernel_time_ms", "gf_device_bytes", "gf_last_error", "gf_version"]
+
+
+class gf_result(ctypes.Structure):
+    _fields_ = [("sweeps", ctypes.c_int), ("F", ctypes.c_double), ("theta", ctypes.c_double)]
+
+
+_vp, _ci, _cd, _u64, _u32 = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_uint64, ctypes.c_uint32
+_lib.gf_create.argtypes = [ctypes.POINTER(_vp), _ci, _ci, _ci, _ci, _ci, _ci, ctypes.c_uint, _vp]
+_lib.gf_destroy.argtypes = [_vp]
+_lib.gf_set_links.argtypes = [_vp, _vp, _ci, _ci]
+_lib.gf_get_links.argtypes = [_vp, _vp, _ci, _ci]
+_lib.gf_get_gauge_transform.argtypes = [_vp, _vp, _ci, _ci]
+_lib.gf_sweep.argtypes = [_vp, _ci, _ci, _cd, _u64, _u32]
+_lib.gf_half_sweep.argtypes = [_vp, _ci, _ci, _cd, _u64, _u32, _ci]
+_lib.gf_measure.argtypes = [_vp, _ci, ctypes.POINTER(_cd), ctypes.POINTER(_cd), _vp]
+_lib.gf_run.argtypes = [_vp, _ci, _ci, _cd, _u64, _u32, _ci, _cd, _ci, _ci, ctypes.POINTER(gf_result), _vp]
+_lib.gf_anneal.argtypes = [_vp, _ci, _cd, _cd, _ci, _ci, _u64, _u32, ctypes.POINTER(_u32)]
+_lib.gf_reunitarize.argtypes = [_vp]
+_lib.gf_coulomb_finalize.argtypes = [_vp]
+_lib.gf_sync.argtypes = [_vp]
+_lib.gf_kernel_timing.argtypes = [_vp, _ci]
+_lib.gf_kernel_time_ms.argtypes = [_vp, ctypes.POINTER(_cd), ctypes.POINTER(_ci), _ci]
+_lib.gf_device_bytes.argtypes = [_vp]
+_lib.gf_device_bytes.restype = ctypes.c_int64
+_lib.gf_last_error.argtypes = [_vp]
+_lib.gf_last_error.restype = ctypes.c_char_p
+_lib.gf_version.restype = ctypes.c_char_p
+_lib.gf_debug_set_block.argtypes = [_vp, _ci]
+
+
+class GfError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libgf error {code}: {msg}")
+        self.code = code
+
+
+def _check(ctx, rc, ok=(GF_OK,)):
+    if rc not in ok:
+        msg = _lib.gf_last_error(ctx).decode() if ctx else "invalid arguments or no CUDA device"
+        raise GfError(rc, msg)
+    return rc
+
+
+def _buffer(a):
+    """(pointer, elem_bytes, is_device, n_elements) of a NumPy array or torch tensor."""
+    if isinstance(a, np.ndarray):
+        if not a.flags.c_contiguous:
+            raise ValueError("array must be C-contiguous")
+        if a.dtype not in (np.float32, np.float64):
+            raise TypeError(a.dtype)
+        return a.ctypes.data, a.dtype.itemsize, 0, a.size
+    import torch
+    if isinstance(a, torch.Tensor):
+        if not a.is_contiguous():
+            raise ValueError("tensor must be contiguous")
+        if a.dtype not in (torch.float32, torch.float64):
+            raise TypeError(a.dtype)
+        return a.data_ptr(), a.element_size(), 1 if a.is_cuda else 0, a.numel()
+    raise TypeError(type(a))
+
+
+def gf_version() -> str:
+    return _lib.gf_version().decode()
+
+
+def gf_create(Nx, Ny, Nz, Nt, precision, recon=18, flags=0, cuda_stream=None):
+    """-> opaque context handle.  cuda_stream: None (torch's current stream if torch has CUDA,
+    else the default stream), an int cudaStream_t, or a torch.cuda.Stream."""
+    if cuda_stream is None:
+        try:
+            import torch
+            cuda_stream = torch.cuda.current_stream().cuda_stream if torch.cuda.is_available() else 0
+        except ImportError:
+            cuda_stream = 0
+    elif hasattr(cuda_stream, "cuda_stream"):
+        cuda_stream = cuda_stream.cuda_stream
+    h = _vp()
+    rc = _lib.gf_create(ctypes.byref(h), Nx, Ny, Nz, Nt, precision, recon, flags, _vp(cuda_stream))
+    _check(None, rc)
+    return h
+
+
+def gf_destroy(ctx):
+    return _lib.gf_destroy(ctx)
+
+
+def gf_set_links(ctx, links):
+    p, eb, dev, n = _buffer(links)
+    return _check(ctx, _lib.gf_set_links(ctx, _vp(p), eb, dev))
+
+
+def gf_get_links(ctx, out):
+    p, eb, dev, n = _buffer(out)
+    return _check(ctx, _lib.gf_get_links(ctx, _vp(p), eb, dev))
+
+
+def gf_get_gauge_transform(ctx, out):
+    p, eb, dev, n = _buffer(out)
+    return _check(ctx, _lib.gf_get_gauge_transform(ctx, _vp(p), eb, dev))
+
+
+def gf_sweep(ctx, gauge, algo, param, seed=0, sweep_index=0):
+    return _check(ctx, _lib.gf_sweep(ctx, gauge, algo, float(param), seed, sweep_index))
+
+
+def gf_half_sweep(ctx, gauge, algo, param, seed, sweep_index, parity):
+    return _check(ctx, _lib.gf_half_sweep(ctx, gauge, algo, float(param), seed, sweep_index, parity))
+
+
+def gf_measure(ctx, gauge, Nt=None):
+    """-> (F, theta) or, with Nt given, (F, theta, theta_slice[Nt])."""
+    F, th = _cd(), _cd()
+    ts = np.zeros(Nt) if Nt else None
+    _check(ctx, _lib.gf_measure(ctx, gauge, ctypes.byref(F), ctypes.byref(th), _vp(ts.ctypes.data) if Nt else None))
+    return (F.value, th.value, ts) if Nt else (F.value, th.value)
+
+
+def gf_run(ctx, gauge, algo, param, seed=0, first_sweep_index=0, max_sweeps=1000, eps=1e-12, check_every=1,
+           reunit_every=0, history=False):
+    """-> dict(sweeps, F, theta, converged[, history = array of (sweep, F, theta)])."""
+    res = gf_result()
+    hist = np.zeros((max_sweeps // check_every + 1, 3)) if history else None
+    rc = _lib.gf_run(ctx, gauge, algo, float(param), seed, first_sweep_index, max_sweeps, float(eps), check_every,
+                     reunit_every, ctypes.byref(res), _vp(hist.ctypes.data) if history else None)
+    _check(ctx, rc, ok=(GF_OK, GF_NOT_CONVERGED))
+    out = {"sweeps": res.sweeps, "F": res.F, "theta": res.theta, "converged": rc == GF_OK}
+    if history:
+        n = int(np.count_nonzero(hist[:, 0]))
+        out["history"] = hist[:n]
+    return out
+
+
+def gf_anneal(ctx, gauge, T_hi, T_lo, n_steps, n_micro, seed, first_sweep_index=0):
+    nxt = _u32()
+    _check(ctx, _lib.gf_anneal(ctx, gauge, float(T_hi), float(T_lo), n_steps, n_micro, seed, first_sweep_index,
+                               ctypes.byref(nxt)))
+    return nxt.value
+
+
+def gf_reunitarize(ctx):
+    return _check(ctx, _lib.gf_reunitarize(ctx))
+
+
+def gf_coulomb_finalize(ctx):
+    return _check(ctx, _lib.gf_coulomb_finalize(ctx))
+
+
+def gf_sync(ctx):
+    return _check(ctx, _lib.gf_sync(ctx))
+
+
+def gf_kernel_timing(ctx, enable):
+    return _check(ctx, _lib.gf_kernel_timing(ctx, 1 if enable else 0))
+
+
+def gf_kernel_time_ms(ctx, reset=True):
+    ms, n = _cd(), _ci()
+    _check(ctx, _lib.gf_kernel_time_ms(ctx, ctypes.byref(ms), ctypes.byref(n), 1 if reset else 0))
+    return ms.value, n.value
+
+
+def gf_device_bytes(ctx):
+    return int(_lib.gf_device_bytes(ctx))
+
+
+def gf_last_error(ctx) -> str:
+    return _lib.gf_last_error(ctx).decode()
+
+
+def gf_debug_set_block(ctx, block):
+    return _check(ctx, _lib.gf_debug_set_block(ctx, block))
+
+
+class GaugeFixer:
+    """Context manager around one gf_ctx.  Methods forward to the C entry points of the same name."""
+
+    def __init__(self, Nx, Ny, Nz, Nt, precision=GF_DP, recon=18, track_transform=False, cuda_stream=None):
+        self.dims = (Nx, Ny, Nz, Nt)
+        self.precision, self.recon = precision, recon
+        self.ctx = gf_create(Nx, Ny, Nz, Nt, precision, recon, GF_FLAG_TRACK_TRANSFORM if track_transform else 0,
+                             cuda_stream)
+
+    def close(self):
+        if self.ctx is not None:
+            gf_destroy(self.ctx)
+            self.ctx = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def shape(self):
+        Nx, Ny, Nz, Nt = self.dims
+        return (Nt, Nx, Ny, Nz, 4, 3, 3, 2)
+
+    def set_links(self, links):
+        return gf_set_links(self.ctx, links)
+
+    def get_links(self, out=None, dtype=np.float64):
+        if out is None:
+            out = np.empty(self.shape, dtype=dtype)
+        gf_get_links(self.ctx, out)
+        return out
+
+    def get_gauge_transform(self, out=None, dtype=np.float64):
+        if out is None:
+            out = np.empty(self.shape[:4] + (3, 3, 2), dtype=dtype)
+        gf_get_gauge_transform(self.ctx, out)
+        return out
+
+    def sweep(self, gauge, algo, param, seed=0, sweep_index=0):
+        return gf_sweep(self.ctx, gauge, algo, param, seed, sweep_index)
+
+    def half_sweep(self, gauge, algo, param, seed, sweep_index, parity):
+        return gf_half_sweep(self.ctx, gauge, algo, param, seed, sweep_index, parity)
+
+    def measure(self, gauge, slices=False):
+        return gf_measure(self.ctx, gauge, self.dims[3] if slices else None)
+
+    def run(self, gauge, algo, param, **kw):
+        return gf_run(self.ctx, gauge, algo, param, **kw)
+
+    def anneal(self, gauge, T_hi, T_lo, n_steps, n_micro, seed, first_sweep_index=0):
+        return gf_anneal(self.ctx, gauge, T_hi, T_lo, n_steps, n_micro, seed, first_sweep_index)
+
+    def reunitarize(self):
+        return gf_reunitarize(self.ctx)
+
+    def coulomb_finalize(self):
+        return gf_coulomb_finalize(self.ctx)
+
+    def sync(self):
+        return gf_sync(self.ctx)

@@ -1,0 +1,310 @@
+"""GPU parity: the CUDA path (through the C ABI, via the thin binding) against the CPU oracle,
+element by element on identical seeded inputs.  Tolerances are BASELINE.json's:
+  one sweep, per link:   <= 1e-12 (DP), <= 5e-5 (SP/MP)
+  full runs:             F to 1e-10 (DP) / 1e-5 (SP), final theta within 10 % and below eps
+  annealing (RNG draws match exactly): per link <= 1e-11 (DP) after one sweep
+Sizes span several CTAs and a ragged tail (V/2 not a multiple of the CTA size) and anisotropic
+extents so that any swapped index shows.
+"""
+import numpy as np
+import pytest
+
+from paper_1212_5221_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+LANDAU, COULOMB, MAG = 0, 1, 2
+OR, SR, SA, MICRO = 0, 1, 2, 3
+SP, DP, MP = 0, 1, 2
+
+TOL_SWEEP = {DP: 1e-12, SP: 5e-5, MP: 5e-5}
+
+
+@pytest.fixture(scope="module")
+def gf():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1212_5221_b200 import gf as _gf
+    return _gf
+
+
+def make(dims_xyzt, eps=0.5, seed=101):
+    Nx, Ny, Nz, Nt = dims_xyzt
+    return inputs.make_config(Nx, Ny, Nz, Nt, eps, seed, seed + 1)
+
+
+def oracle_dtype(prec):
+    return np.float64 if prec == DP else np.float32
+
+
+def test_library_identifies_itself(gf):
+    assert "sm_100a" in gf.gf_version()
+
+
+@pytest.mark.parametrize("prec,recon", [(DP, 18), (DP, 12), (SP, 18), (SP, 12)])
+def test_layout_roundtrip(gf, prec, recon):
+    dims = (6, 4, 10, 2)
+    U = make(dims)
+    dt = oracle_dtype(prec)
+    L = inputs.as_real(U, dt)
+    with gf.GaugeFixer(*dims, precision=prec, recon=recon) as fx:
+        fx.set_links(L)
+        out = fx.get_links(dtype=dt)
+        if recon == 18:
+            assert np.array_equal(out, L)          # pure data movement: bit exact
+        else:
+            assert np.array_equal(out[..., :2, :, :], L[..., :2, :, :])
+            assert np.abs(out - L).max() < (4e-15 if prec == DP else 5e-7)   # rebuilt third row
+        # element type of the caller's buffer is independent of the context's precision
+        other = np.float32 if dt == np.float64 else np.float64
+        out2 = fx.get_links(dtype=other)
+        assert np.abs(out2.astype(np.float64) - L.astype(np.float64)).max() < 5e-7
+        # device-pointer path
+        import torch
+        Ld = torch.from_numpy(L).cuda()
+        fx.set_links(Ld)
+        outd = torch.empty_like(Ld)
+        gf.gf_get_links(fx.ctx, outd)
+        assert np.abs(outd.cpu().numpy() - L).max() < (4e-15 if prec == DP else 5e-7)
+
+
+SWEEP_CASES = [
+    # (dims_xyzt, gauge, algo, param)
+    ((6, 6, 6, 6), LANDAU, OR, 1.7),
+    ((4, 6, 10, 2), LANDAU, OR, 1.0),
+    ((6, 6, 6, 6), COULOMB, OR, 1.7),
+    ((2, 4, 6, 6), COULOMB, MICRO, 0.0),
+    ((6, 6, 6, 6), MAG, OR, 1.7),
+    ((4, 2, 6, 10), MAG, MICRO, 0.0),
+    ((6, 6, 6, 6), LANDAU, MICRO, 0.0),
+    ((6, 6, 6, 6), LANDAU, SR, 0.5),
+    ((6, 6, 6, 6), MAG, SR, 0.4),
+    ((6, 6, 6, 6), COULOMB, SR, 0.6),
+]
+
+
+@pytest.mark.parametrize("prec,recon", [(DP, 18), (DP, 12), (SP, 18), (SP, 12), (MP, 18), (MP, 12)])
+@pytest.mark.parametrize("dims,gauge,algo,param", SWEEP_CASES)
+def test_one_sweep_per_link(gf, oracle, prec, recon, dims, gauge, algo, param):
+    U = make(dims, seed=200 + gauge * 10 + algo)
+    dt = oracle_dtype(prec)
+    L = inputs.as_real(U, dt)
+    ref = L.copy()
+    Gref = oracle.identity_transform(ref)
+    for s in range(2):
+        oracle.sweep(ref, gauge, algo, param, seed=77, sweep_index=s, mixed=(prec == MP), gtot=Gref)
+    with gf.GaugeFixer(*dims, precision=prec, recon=recon, track_transform=True) as fx:
+        fx.set_links(L)
+        for s in range(2):
+            fx.sweep(gauge, algo, param, seed=77, sweep_index=s)
+        got_g = fx.get_gauge_transform(dtype=dt)
+        if gauge == COULOMB:
+            # compare before the implicit finalisation of the temporal links: spatial links only
+            got = fx.get_links(dtype=dt)
+            tol = TOL_SWEEP[prec]
+            assert np.abs(got[..., 1:, :, :, :].astype(np.float64) - ref[..., 1:, :, :, :]).max() <= tol
+            oracle.coulomb_finalize(ref, Gref)
+            assert np.abs(got.astype(np.float64) - ref).max() <= 4 * tol
+        else:
+            got = fx.get_links(dtype=dt)
+            assert np.abs(got.astype(np.float64) - ref).max() <= TOL_SWEEP[prec]
+        assert np.abs(got_g.astype(np.float64) - Gref).max() <= TOL_SWEEP[prec]
+
+
+@pytest.mark.parametrize("prec", [DP, SP, MP])
+@pytest.mark.parametrize("gauge", [LANDAU, COULOMB, MAG])
+def test_heatbath_sweep_rng_matches(gf, oracle, prec, gauge):
+    # annealing: RNG draws match exactly -> per link <= 1e-11 (DP) after one sweep
+    dims = (6, 4, 6, 6)
+    U = make(dims, seed=300 + gauge)
+    dt = oracle_dtype(prec)
+    L = inputs.as_real(U, dt)
+    for T in (1.45, 0.2, 0.01):
+        ref = L.copy()
+        oracle.sweep(ref, gauge, SA, T, seed=1234, sweep_index=5, mixed=(prec == MP))
+        with gf.GaugeFixer(*dims, precision=prec) as fx:
+            fx.set_links(L)
+            fx.sweep(gauge, SA, T, seed=1234, sweep_index=5)
+            got = fx.get_links(dtype=dt)
+        sel = slice(1, 4) if gauge == COULOMB else slice(0, 4)
+        diff = np.abs(got[..., sel, :, :, :].astype(np.float64) - ref[..., sel, :, :, :]).max()
+        assert diff <= (1e-11 if prec == DP else 5e-5), (T, diff)
+
+
+def test_half_sweeps_compose(gf, oracle):
+    dims = (4, 4, 6, 6)
+    L = inputs.as_real(make(dims, seed=310))
+    ref = L.copy()
+    oracle.sweep(ref, LANDAU, OR, 1.7, parity_mask=1)
+    with gf.GaugeFixer(*dims, precision=DP) as fx:
+        fx.set_links(L)
+        fx.half_sweep(LANDAU, OR, 1.7, 0, 0, 0)
+        assert np.abs(fx.get_links() - ref).max() <= 1e-12
+        oracle.sweep(ref, LANDAU, OR, 1.7, parity_mask=2)
+        fx.half_sweep(LANDAU, OR, 1.7, 0, 0, 1)
+        assert np.abs(fx.get_links() - ref).max() <= 1e-12
+
+
+@pytest.mark.parametrize("prec,recon", [(DP, 18), (DP, 12), (SP, 18), (SP, 12)])
+@pytest.mark.parametrize("gauge", [LANDAU, COULOMB, MAG])
+def test_measure_matches_oracle(gf, oracle, prec, recon, gauge):
+    dims = (6, 4, 10, 6)
+    dt = oracle_dtype(prec)
+    L = inputs.as_real(make(dims, seed=320), dt)
+    for _ in range(2):
+        oracle.sweep(L, gauge, OR, 1.7)
+    m = oracle.measure(L, gauge)
+    with gf.GaugeFixer(*dims, precision=prec, recon=recon) as fx:
+        fx.set_links(L)
+        F, th, ths = fx.measure(gauge, slices=True)
+        F2, th2, _ = fx.measure(gauge, slices=True)
+    rel = 1e-13 if (prec == DP and recon == 18) else (1e-12 if prec == DP else 2e-6)
+    assert F == pytest.approx(m["F"], rel=rel, abs=rel)
+    assert th == pytest.approx(m["theta"], rel=rel * 10)
+    np.testing.assert_allclose(ths, m["theta_slice"], rtol=rel * 10)
+    assert (F, th) == (F2, th2)          # fixed summation order: bit-reproducible
+
+
+@pytest.mark.parametrize("prec,recon", [(DP, 18), (SP, 18), (SP, 12)])
+def test_reunitarize_matches_oracle(gf, oracle, prec, recon):
+    dims = (4, 4, 4, 6)
+    dt = oracle_dtype(prec)
+    rng = np.random.default_rng(5)
+    L = inputs.as_real(make(dims, seed=330), dt)
+    L = (L + 1e-3 * rng.standard_normal(L.shape)).astype(dt)
+    ref = L.copy()
+    oracle.reunitarize(ref)
+    with gf.GaugeFixer(*dims, precision=prec, recon=recon) as fx:
+        fx.set_links(L)
+        fx.reunitarize()
+        got = fx.get_links(dtype=dt)
+    tol = 1e-15 if prec == DP else 3e-7
+    assert np.abs(got.astype(np.float64) - ref).max() <= tol
+
+
+def test_config0_full_run(gf, oracle):
+    # BASELINE.json config 0: Landau OR 1.7, DP, 4^4, theta < 1e-12 within 2000 sweeps
+    U = inputs.config_k(0)
+    L = inputs.as_real(U)
+    ref = L.copy()
+    s, F, th, hist, conv = oracle.run(ref, LANDAU, OR, 1.7, max_sweeps=2000, eps=1e-12)
+    with gf.GaugeFixer(4, 4, 4, 4, precision=DP) as fx:
+        fx.set_links(L)
+        r = fx.run(LANDAU, OR, 1.7, max_sweeps=2000, eps=1e-12, history=True)
+        got = fx.get_links()
+    assert conv and r["converged"] and r["sweeps"] == s
+    assert abs(r["F"] - F) <= 1e-10
+    assert r["theta"] < 1e-12 and abs(r["theta"] - th) <= 0.1 * th
+    np.testing.assert_allclose(r["history"][:, 1], [h[1] for h in hist], atol=1e-10)
+    assert np.abs(got - ref).max() < 1e-9
+
+
+def test_config1_full_run(gf, oracle):
+    # BASELINE.json config 1: 16^4, eps = 0.5, Landau OR 1.7, DP, theta < 1e-12, <= 5000 sweeps
+    U = inputs.config_k(1)
+    L = inputs.as_real(U)
+    ref = L.copy()
+    s, F, th, hist, conv = oracle.run(ref, LANDAU, OR, 1.7, max_sweeps=5000, eps=1e-12)
+    with gf.GaugeFixer(16, 16, 16, 16, precision=DP) as fx:
+        fx.set_links(L)
+        r = fx.run(LANDAU, OR, 1.7, max_sweeps=5000, eps=1e-12, history=True)
+    assert conv and r["converged"]
+    assert abs(r["F"] - F) <= 1e-10
+    assert r["theta"] < 1e-12 and abs(r["theta"] - th) <= 0.1 * th
+    assert abs(r["sweeps"] - s) <= 2
+    n = min(len(hist), len(r["history"]))
+    np.testing.assert_allclose(r["history"][:n, 1], [h[1] for h in hist][:n], atol=1e-10)
+
+
+@pytest.mark.parametrize("prec,recon", [(SP, 12), (MP, 12), (SP, 18)])
+def test_coulomb_sp_run_with_reunit(gf, oracle, prec, recon):
+    # BASELINE.json config 2 in miniature: Coulomb OR 1.7, SP links / 12 reals, DP reunit every 100,
+    # DP reductions, per-slice theta < 1e-10.  SP full runs: F to 1e-5, theta below eps.
+    dims = (8, 8, 8, 4)
+    U = make(dims, eps=0.6, seed=340)
+    L = inputs.as_real(U, np.float32)
+    ref = L.copy()
+    Gref = oracle.identity_transform(ref)
+    s, F, th, hist, conv = oracle.run(ref, COULOMB, OR, 1.7, max_sweeps=3000, eps=1e-10, check_every=10,
+                                      reunit_every=100, mixed=(prec == MP), gtot=Gref)
+    oracle.coulomb_finalize(ref, Gref)
+    # DP reference of the same run for the functional value
+    refd = inputs.as_real(U)
+    sd, Fd, thd, _, convd = oracle.run(refd, COULOMB, OR, 1.7, max_sweeps=3000, eps=1e-12, check_every=10)
+    with gf.GaugeFixer(*dims, precision=prec, recon=recon, track_transform=True) as fx:
+        fx.set_links(L)
+        r = fx.run(COULOMB, OR, 1.7, max_sweeps=3000, eps=1e-10, check_every=10, reunit_every=100)
+        got = fx.get_links(dtype=np.float32)
+        g = fx.get_gauge_transform(dtype=np.float64)
+        F2, th2, ths = fx.measure(COULOMB, slices=True)
+    assert conv and convd and r["converged"]
+    assert abs(r["F"] - F) <= 1e-5 and abs(r["F"] - Fd) <= 1e-5
+    assert r["theta"] < 1e-10 and ths.max() < 1e-10
+    # the returned links are the gauge transform of the input by the returned g (Eq. 1), all mu
+    gc = g[..., 0] + 1j * g[..., 1]
+    want = inputs.gauge_transform(U, gc)
+    assert np.abs(inputs.as_complex(got) - want).max() < 2e-5
+
+
+def test_mag_anneal_then_or(gf, oracle):
+    # BASELINE.json config 3 in miniature: MAG, SA 1.45 -> 0.01 linear with 3 microcanonical sweeps
+    # per heatbath sweep (Philox seed 1234), then OR 1.7 to theta < 1e-12, DP.
+    dims = (6, 6, 6, 6)
+    U = make(dims, seed=350)
+    L = inputs.as_real(U)
+    ref = L.copy()
+    nxt = oracle.anneal(ref, MAG, 1.45, 0.01, 12, 3, seed=1234)
+    with gf.GaugeFixer(*dims, precision=DP) as fx:
+        fx.set_links(L)
+        nxt_g = fx.anneal(MAG, 1.45, 0.01, 12, 3, seed=1234)
+        got = fx.get_links()
+        assert nxt_g == nxt == 48
+        # 48 stochastic sweeps with identical draws: still the same trajectory
+        assert np.abs(got - ref).max() < 1e-9
+        s, F, th, hist, conv = oracle.run(ref, MAG, OR, 1.7, max_sweeps=5000, eps=1e-12, first_sweep_index=nxt)
+        r = fx.run(MAG, OR, 1.7, first_sweep_index=nxt, max_sweeps=5000, eps=1e-12)
+    assert conv and r["converged"]
+    assert abs(r["F"] - F) <= 1e-10 and r["theta"] < 1e-12
+
+
+def test_edge_cases(gf, oracle):
+    # smallest legal lattice, Nz = 2 (z-neighbour wraps onto the same checkerboard slot)
+    for dims in ((2, 2, 2, 2), (4, 2, 2, 6)):
+        L = inputs.as_real(make(dims, seed=360))
+        ref = L.copy()
+        for gauge in (LANDAU, COULOMB, MAG):
+            oracle.sweep(ref, gauge, OR, 1.7)
+        with gf.GaugeFixer(*dims, precision=DP) as fx:
+            fx.set_links(L)
+            for gauge in (LANDAU, COULOMB, MAG):
+                fx.sweep(gauge, OR, 1.7)
+            # Coulomb without tracking leaves the temporal links alone, like the oracle's sweep
+            assert np.abs(fx.get_links() - ref).max() <= 1e-12
+    # invalid arguments fail loudly
+    with pytest.raises(gf.GfError):
+        gf.gf_create(3, 4, 4, 4, DP)
+    with pytest.raises(gf.GfError):
+        gf.gf_create(4, 4, 4, 4, 7)
+    with gf.GaugeFixer(4, 4, 4, 4, precision=DP) as fx:
+        with pytest.raises(gf.GfError):
+            fx.sweep(LANDAU, OR, 1.7)            # no links yet
+        fx.set_links(inputs.as_real(make((4, 4, 4, 4))))
+        with pytest.raises(gf.GfError):
+            fx.sweep(LANDAU, OR, 2.5)            # omega out of range
+        with pytest.raises(gf.GfError):
+            fx.get_gauge_transform()             # not tracked
+
+
+def test_cta_sizes_agree(gf, oracle):
+    # the result must not depend on the launch shape (ragged tails, several CTA sizes)
+    dims = (6, 6, 6, 10)
+    L = inputs.as_real(make(dims, seed=370))
+    outs = []
+    for blk in (32, 64):
+        with gf.GaugeFixer(*dims, precision=DP) as fx:
+            gf.gf_debug_set_block(fx.ctx, blk)
+            fx.set_links(L)
+            fx.sweep(LANDAU, OR, 1.7)
+            outs.append(fx.get_links())
+    assert np.array_equal(outs[0], outs[1])
