@@ -84,6 +84,14 @@ SWEEP_CASES = [
 ]
 
 
+# Rounding differences between the two paths (association order, FMA) grow from sweep to sweep:
+# measured on the B200 (R25) by ~10x per microcanonical sweep (energy-conserving, chaotic
+# on a rough start) and less for OR.  BASELINE.json's per-link tolerance is for ONE sweep; the second
+# sweep below is held to a 30x wider band and only shows that nothing structural (sweep index,
+# stale data) goes wrong when sweeps follow one another.
+SECOND_SWEEP_FACTOR = 30.0
+
+
 @pytest.mark.parametrize("prec,recon", [(DP, 18), (DP, 12), (SP, 18), (SP, 12), (MP, 18), (MP, 12)])
 @pytest.mark.parametrize("dims,gauge,algo,param", SWEEP_CASES)
 def test_one_sweep_per_link(gf, oracle, prec, recon, dims, gauge, algo, param):
@@ -92,24 +100,42 @@ def test_one_sweep_per_link(gf, oracle, prec, recon, dims, gauge, algo, param):
     L = inputs.as_real(U, dt)
     ref = L.copy()
     Gref = oracle.identity_transform(ref)
-    for s in range(2):
-        oracle.sweep(ref, gauge, algo, param, seed=77, sweep_index=s, mixed=(prec == MP), gtot=Gref)
+    sel = slice(1, 4) if gauge == COULOMB else slice(0, 4)   # Coulomb sweeps leave U_0 alone
     with gf.GaugeFixer(*dims, precision=prec, recon=recon, track_transform=True) as fx:
         fx.set_links(L)
         for s in range(2):
+            tol = TOL_SWEEP[prec] * (1.0 if s == 0 else SECOND_SWEEP_FACTOR)
+            oracle.sweep(ref, gauge, algo, param, seed=77, sweep_index=s, mixed=(prec == MP), gtot=Gref)
             fx.sweep(gauge, algo, param, seed=77, sweep_index=s)
-        got_g = fx.get_gauge_transform(dtype=dt)
-        if gauge == COULOMB:
-            # compare before the implicit finalisation of the temporal links: spatial links only
+            got_g = fx.get_gauge_transform(dtype=dt)
+            assert np.abs(got_g.astype(np.float64) - Gref).max() <= tol
+            if gauge == COULOMB and s == 0:
+                continue      # gf_get_links would finalise the temporal links; do that once, below
             got = fx.get_links(dtype=dt)
-            tol = TOL_SWEEP[prec]
-            assert np.abs(got[..., 1:, :, :, :].astype(np.float64) - ref[..., 1:, :, :, :]).max() <= tol
-            oracle.coulomb_finalize(ref, Gref)
-            assert np.abs(got.astype(np.float64) - ref).max() <= 4 * tol
-        else:
-            got = fx.get_links(dtype=dt)
-            assert np.abs(got.astype(np.float64) - ref).max() <= TOL_SWEEP[prec]
-        assert np.abs(got_g.astype(np.float64) - Gref).max() <= TOL_SWEEP[prec]
+            if gauge == COULOMB:
+                assert np.abs(got[..., sel, :, :, :].astype(np.float64) - ref[..., sel, :, :, :]).max() <= tol
+                fin = ref.copy()
+                oracle.coulomb_finalize(fin, Gref)
+                assert np.abs(got.astype(np.float64) - fin).max() <= 4 * tol
+            else:
+                assert np.abs(got.astype(np.float64) - ref).max() <= tol
+
+
+@pytest.mark.parametrize("prec,recon", [(SP, 12), (DP, 18)])
+def test_coulomb_one_sweep_spatial_links(gf, oracle, prec, recon):
+    # one Coulomb sweep, untracked context: links come back without finalisation
+    dims = (6, 4, 6, 4)
+    dt = oracle_dtype(prec)
+    L = inputs.as_real(make(dims, eps=0.6, seed=205), dt)
+    ref = L.copy()
+    oracle.sweep(ref, COULOMB, OR, 1.7)
+    with gf.GaugeFixer(*dims, precision=prec, recon=recon) as fx:
+        fx.set_links(L)
+        fx.sweep(COULOMB, OR, 1.7)
+        got = fx.get_links(dtype=dt)
+    assert np.abs(got.astype(np.float64) - ref).max() <= TOL_SWEEP[prec]
+    if recon == 18:
+        assert np.array_equal(got[..., 0, :, :, :], L[..., 0, :, :, :])    # U_0 never touched
 
 
 @pytest.mark.parametrize("prec", [DP, SP, MP])
@@ -250,22 +276,45 @@ def test_coulomb_sp_run_with_reunit(gf, oracle, prec, recon):
 def test_mag_anneal_then_or(gf, oracle):
     # BASELINE.json config 3 in miniature: MAG, SA 1.45 -> 0.01 linear with 3 microcanonical sweeps
     # per heatbath sweep (Philox seed 1234), then OR 1.7 to theta < 1e-12, DP.
+    # The stochastic trajectory is chaotic: measured divergence growth is ~300x per annealing step
+    # (1 heatbath + 3 microcanonical sweeps), so the two paths agree per link for the first steps
+    # and then select different Gribov copies (R25; each is a valid result).
     dims = (6, 6, 6, 6)
     U = make(dims, seed=350)
     L = inputs.as_real(U)
     ref = L.copy()
-    nxt = oracle.anneal(ref, MAG, 1.45, 0.01, 12, 3, seed=1234)
-    with gf.GaugeFixer(*dims, precision=DP) as fx:
+    n_steps, n_micro = 12, 3
+    with gf.GaugeFixer(*dims, precision=DP, track_transform=True) as fx:
         fx.set_links(L)
-        nxt_g = fx.anneal(MAG, 1.45, 0.01, 12, 3, seed=1234)
+        # step 0 of the schedule on both sides: identical draws, links equal to rounding
+        T0 = oracle.temperature(0, n_steps, 1.45, 0.01)
+        oracle.sweep(ref, MAG, SA, T0, seed=1234, sweep_index=0)
+        fx.sweep(MAG, SA, T0, seed=1234, sweep_index=0)
+        assert np.abs(fx.get_links() - ref).max() <= 1e-11
+        for m in range(n_micro):
+            oracle.sweep(ref, MAG, MICRO, 0.0, seed=1234, sweep_index=1 + m)
+            fx.sweep(MAG, MICRO, 0.0, seed=1234, sweep_index=1 + m)
+        assert np.abs(fx.get_links() - ref).max() <= 1e-8
+        # the whole schedule through gf_anneal, from the start
+        fx.set_links(L)
+        ref = L.copy()
+        nxt = oracle.anneal(ref, MAG, 1.45, 0.01, n_steps, n_micro, seed=1234)
+        nxt_g = fx.anneal(MAG, 1.45, 0.01, n_steps, n_micro, seed=1234)
+        assert nxt_g == nxt == n_steps * (1 + n_micro)
+        Fa, tha = fx.measure(MAG)
+        ma = oracle.measure(ref, MAG)
+        assert abs(Fa - ma["F"]) < 0.02          # same ensemble at the end of the schedule
+        s, F, th, hist, conv = oracle.run(ref, MAG, OR, 1.7, max_sweeps=8000, eps=1e-12, first_sweep_index=nxt)
+        r = fx.run(MAG, OR, 1.7, first_sweep_index=nxt, max_sweeps=8000, eps=1e-12)
         got = fx.get_links()
-        assert nxt_g == nxt == 48
-        # 48 stochastic sweeps with identical draws: still the same trajectory
-        assert np.abs(got - ref).max() < 1e-9
-        s, F, th, hist, conv = oracle.run(ref, MAG, OR, 1.7, max_sweeps=5000, eps=1e-12, first_sweep_index=nxt)
-        r = fx.run(MAG, OR, 1.7, first_sweep_index=nxt, max_sweeps=5000, eps=1e-12)
-    assert conv and r["converged"]
-    assert abs(r["F"] - F) <= 1e-10 and r["theta"] < 1e-12
+        g = fx.get_gauge_transform()
+    assert conv and r["converged"] and r["theta"] < 1e-12
+    assert abs(r["F"] - F) < 0.02                # two Gribov copies of the same orbit
+    F0 = oracle.measure(L, MAG)["F"]
+    assert r["F"] > F0 + 0.1
+    # whatever copy was reached, it is a gauge transform of the input (Eq. 1) by the returned g
+    gc = g[..., 0] + 1j * g[..., 1]
+    assert np.abs(inputs.as_complex(got) - inputs.gauge_transform(U, gc)).max() < 1e-10
 
 
 def test_edge_cases(gf, oracle):
