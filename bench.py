@@ -1,0 +1,404 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the gauge-fixing hot path on B200 (contract: see DESIGN.md §9).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+Workload (BASELINE.json configs[4], the configuration the metric is quoted on): Landau gauge
+overrelaxation omega = 1.7 on a 64^3 x 256 lattice, DP / 18 reals (headline line) and, as
+`variants`, SP-18, SP-12, DP-12 and MP-12 on the same lattice.  One *step* = one gf_run call of
+SWEEPS_PER_STEP (100) sweeps = 200 half-sweep kernels, the DP reunitarisation that falls due every
+100 sweeps in the SP/MP modes, and one F/theta device reduction (the whole hot path,
+SURVEY.md §8(a)).  Inputs are synthetic: the eps = 0.5 random-algebra lattice with a
+Haar gauge transform of configs[1]'s recipe on a 16^4 tile, tiled periodically to the full extent
+(the sweep's cost is data independent).
+
+`value` is timed with CUDA events on the context's stream with the links resident in HBM; `e2e`
+repeats the same steps through the C ABI with pinned HOST buffers: gf_set_links (host -> device) +
+gf_run + gf_get_links (device -> host) inside the timed region.  `roofline` is the half-sweep
+kernel: algorithmic bytes (every touched link read once and written once, 2*8*R*s bytes per site
+update) divided by its mean launch duration measured with CUDA events inside the timed region.
+`cpu_baseline` is the oracle (oracle/gf_oracle.cpp, as it stands) on the host cores on a bounded
+sample; `--impl reference` times that oracle alone.  N > 1 runs N independent replicas, one lattice
+per GPU ("replicas only"): there is no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+LANDAU, OR = 0, 0
+OMEGA = 1.7
+SWEEPS_PER_STEP = 100
+TILE = (16, 16, 16, 16)            # (Nx, Ny, Nz, Nt) of the generated tile
+TILE_EPS, TILE_SEEDS = 0.5, (1004, 2004)
+PREC_NAMES = {"sp": 0, "dp": 1, "mp": 2}
+DTYPE_NAMES = {"sp": "f32", "dp": "f64", "mp": "f32 (Step 1 in f64)"}
+
+# dram__bytes_read.sum + dram__bytes_write.sum per half-sweep launch from the `ncu --set full`
+# captures summarised under profiles/ (bytes; key = (precision, recon, "NxxNyxNzxNt")).
+NCU_TRAFFIC = {}
+try:
+    with open(os.path.join(ROOT, "profiles", "traffic.csv")) as _fh:
+        for _line in _fh:
+            _f = _line.strip().split(",")
+            if len(_f) >= 4 and _f[0] in PREC_NAMES:
+                NCU_TRAFFIC[(_f[0], int(_f[1]), _f[2])] = float(_f[3])
+except OSError:
+    pass
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--lattice", default="64,64,64,256", help="Nx,Ny,Nz,Nt")
+    ap.add_argument("--precision", default="dp", choices=list(PREC_NAMES))
+    ap.add_argument("--recon", type=int, default=18, choices=[12, 18])
+    ap.add_argument("--sweeps-per-step", type=int, default=SWEEPS_PER_STEP)
+    ap.add_argument("--no-variants", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--block", type=int, default=0, help="CTA size override of the half-sweep kernel (tuning)")
+    return ap.parse_args()
+
+
+def peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def bytes_per_site_update(prec: str, recon: int, nd: int = 4) -> int:
+    """Algorithmic HBM bytes per site update: 2*nd links read once + written once."""
+    s = 8 if prec == "dp" else 4
+    return 2 * (2 * nd) * recon * s
+
+
+# ---- clocks ---------------------------------------------------------------------------------
+class ClockSampler:
+    QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+             "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.QUERY}", "--format=csv,noheader,nounits",
+                 "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line)
+
+    def stop(self) -> dict:
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        for line in self.lines:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); smax.append(float(f[2])); power.append(float(f[3]))
+            except ValueError:
+                continue
+            for name, v in zip(self.NAMES, f[5:9]):
+                if v == "Active":
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(smax), "power_w_max": max(power),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---- inputs ---------------------------------------------------------------------------------
+def make_tile():
+    from paper_1212_5221_b200 import inputs
+    U = inputs.make_config(*TILE, TILE_EPS, *TILE_SEEDS)      # complex [Nt,Nx,Ny,Nz,4,3,3]
+    return inputs.as_real(U, np.float64)
+
+
+def reps_for(dims_xyzt):
+    Nx, Ny, Nz, Nt = dims_xyzt
+    tx, ty, tz, tt = TILE
+    for n, t in ((Nx, tx), (Ny, ty), (Nz, tz), (Nt, tt)):
+        if n % t:
+            raise SystemExit(f"lattice extent {n} is not a multiple of the {t}-site tile")
+    return (Nt // tt, Nx // tx, Ny // ty, Nz // tz)
+
+
+# ---- the oracle legs (cpu_baseline, --impl reference) ------------------------------------------
+ORACLE_SAMPLE_DIMS = (32, 32, 32, 64)    # Nx,Ny,Nz,Nt: a 1/32 sample of the 64^3 x 256 workload
+
+
+def oracle_leg(tile, prec: str, sweeps_per_step: int, steps: int, warmup: int):
+    """Times the oracle as it stands on a bounded sample of the same workload."""
+    from oracle import gf_oracle as O
+    from paper_1212_5221_b200 import inputs
+    r = reps_for(ORACLE_SAMPLE_DIMS)
+    dt = np.float64 if prec == "dp" else np.float32
+    L = np.ascontiguousarray(inputs.tile_lattice(tile, r + (1,)).astype(dt))
+    V = L.size // 72
+
+    def step():
+        for s in range(sweeps_per_step):
+            O.sweep(L, O.LANDAU, O.OR, OMEGA, 0, s, prec == "mp")
+        if prec != "dp":
+            O.reunitarize(L)
+        return O.measure(L, O.LANDAU)
+
+    for _ in range(warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        m = step()
+    dt_s = time.perf_counter() - t0
+    return {"value": V * sweeps_per_step * steps / dt_s, "seconds": dt_s, "cores": O.num_threads(), "V": V,
+            "F": m["F"], "theta": m["theta"]}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    dims = tuple(int(x) for x in args.lattice.split(","))
+    sps = 5                                   # sweeps per reference step: bounded sample
+    tile = make_tile()
+    r = oracle_leg(tile, args.precision, sps, args.steps, args.warmup)
+    sample = (f"{args.steps} steps x {sps} Landau OR sweeps (+1 F/theta measurement) of the CPU oracle on a "
+              f"{'x'.join(map(str, ORACLE_SAMPLE_DIMS))} sample (V={r['V']}) of the {args.lattice} workload")
+    line = {
+        "impl": "reference", "metric": "site-updates/s (Landau OR sweep incl. F/theta reductions)",
+        "value": r["value"], "unit": "site-updates/s", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * r["seconds"] / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": DTYPE_NAMES[args.precision], "data": "synthetic",
+        "config": {"workload": f"Landau OR omega=1.7, {'x'.join(map(str, dims))} (BASELINE.json configs[4]), "
+                               f"{args.precision.upper()}-{args.recon}", "sample": sample},
+        "cpu_baseline": {"value": r["value"], "unit": "site-updates/s", "cores": r["cores"], "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": r["value"], "unit": "site-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ---- the CUDA path ----------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1212_5221_b200 import gf     # fails loudly if libgf.so is missing
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    dims = tuple(int(x) for x in args.lattice.split(","))
+    Nx, Ny, Nz, Nt = dims
+    V = Nx * Ny * Nz * Nt
+    S = args.sweeps_per_step
+    peak, peak_src = peaks()
+    lat_name = "x".join(map(str, dims))
+
+    tile = make_tile()
+    reps = reps_for(dims)
+    stream = torch.cuda.Stream(device=dev)
+    with torch.cuda.stream(stream):
+        tile_dev = torch.from_numpy(tile).to(dev)
+        links_dev = tile_dev.repeat(*reps, 1, 1, 1, 1).contiguous()     # StandardPattern, f64, in HBM
+    stream.synchronize()
+    del tile_dev
+
+    def bench_one(prec: str, recon: int, steps: int, warmup: int, e2e: bool, sample_clocks: bool):
+        reunit = 100 if prec != "dp" else 0
+        out = {}
+        with gf.GaugeFixer(Nx, Ny, Nz, Nt, precision=PREC_NAMES[prec], recon=recon, cuda_stream=stream) as fx:
+            if args.block:
+                gf.gf_debug_set_block(fx.ctx, args.block)
+            fx.set_links(links_dev)
+
+            def step():
+                return fx.run(LANDAU, OR, OMEGA, max_sweeps=S, eps=0.0, check_every=S, reunit_every=reunit)
+
+            for _ in range(warmup):
+                step()
+            sampler = ClockSampler(local) if sample_clocks else None
+            barrier()
+            if sampler:
+                sampler.start()
+            gf.gf_launch_count(fx.ctx, reset=True)
+            gf.gf_kernel_timing(fx.ctx, True)
+            gf.gf_kernel_time_ms(fx.ctx, reset=True)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(steps):
+                r = step()
+            e1.record(stream)
+            barrier()
+            ms = max_over_ranks(e0.elapsed_time(e1))
+            kern_ms, kern_n = gf.gf_kernel_time_ms(fx.ctx, reset=True)
+            gf.gf_kernel_timing(fx.ctx, False)
+            launches = gf.gf_launch_count(fx.ctx, reset=True)
+            if sampler:
+                out["clocks"] = sampler.stop()
+            bpsu = bytes_per_site_update(prec, recon)
+            per_launch_bytes = bpsu * (V // 2)
+            achieved = per_launch_bytes / (kern_ms / kern_n * 1e-3) / 1e9
+            out.update({
+                "precision": prec, "recon": recon, "steps": steps, "ms_per_step": ms / steps,
+                "value": world * V * S * steps / (ms * 1e-3),
+                "paper_gflops": world * V * S * steps / (ms * 1e-3) * 2274 / 1e9,
+                "gpu_launches": launches, "F": r["F"], "theta": r["theta"],
+                "kernel_share_of_step": kern_ms / ms,
+                "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                             "frac": achieved / peak, "frac_of_8TBps_nominal": achieved / 8000.0,
+                             "traffic": NCU_TRAFFIC.get((prec, recon, lat_name)),
+                             "kernel": "gf::sweep_kernel (one half-sweep)", "peak_source": peak_src,
+                             "algorithmic_bytes_per_launch": per_launch_bytes,
+                             "bytes_per_site_update": bpsu, "avg_launch_ms": kern_ms / kern_n,
+                             "launches_timed": kern_n},
+            })
+            if e2e:
+                eb = 8 if prec == "dp" else 4
+                tdt = torch.float64 if prec == "dp" else torch.float32
+                nbytes = V * 72 * eb
+                import psutil
+                need = 2 * nbytes * max(1, world)
+                if psutil.virtual_memory().available < 1.15 * need:
+                    out["e2e"] = {"value": None, "unit": "site-updates/s", "h2d_bytes_per_step": nbytes,
+                                  "d2h_bytes_per_step": nbytes, "skipped": "not enough host memory for pinned buffers"}
+                else:
+                    h_in = torch.empty(links_dev.shape, dtype=tdt, pin_memory=True)
+                    h_out = torch.empty(links_dev.shape, dtype=tdt, pin_memory=True)
+                    with torch.cuda.stream(stream):
+                        h_in.copy_(links_dev.to(tdt) if tdt != links_dev.dtype else links_dev)
+                    stream.synchronize()
+
+                    def e2e_step():
+                        fx.set_links(h_in)                          # host -> device (+ layout conversion)
+                        rr = step()                                 # S sweeps + F/theta
+                        fx.get_links(out=h_out)                     # device -> host
+                        return rr
+
+                    e2e_step()
+                    n_e2e = max(1, steps // 2)
+                    barrier()
+                    t0 = time.perf_counter()
+                    for _ in range(n_e2e):
+                        rr = e2e_step()
+                    barrier()
+                    sec = max_over_ranks(time.perf_counter() - t0)
+                    out["e2e"] = {"value": world * V * S * n_e2e / sec, "unit": "site-updates/s",
+                                  "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes + 24,
+                                  "steps": n_e2e, "ms_per_step": 1e3 * sec / n_e2e,
+                                  "timing": "host wall clock around gf_set_links(host) + gf_run + gf_get_links(host), "
+                                            "each synchronous; max over ranks"}
+                    del h_in, h_out
+        return out
+
+    head = bench_one(args.precision, args.recon, args.steps, args.warmup, not args.no_e2e, True)
+    variants = []
+    if not args.no_variants:
+        for prec, recon in (("sp", 18), ("sp", 12), ("dp", 12), ("mp", 12)):
+            if (prec, recon) == (args.precision, args.recon):
+                continue
+            v = bench_one(prec, recon, max(1, min(2, args.steps)), 1, False, False)
+            variants.append({"precision": prec, "recon": recon, "dtype": DTYPE_NAMES[prec],
+                             "value": v["value"], "ms_per_step": v["ms_per_step"], "steps": v["steps"],
+                             "roofline_achieved_gbs": v["roofline"]["achieved"], "roofline_frac": v["roofline"]["frac"],
+                             "bytes_per_site_update": v["roofline"]["bytes_per_site_update"],
+                             "kernel_share_of_step": v["kernel_share_of_step"]})
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        del links_dev
+        torch.cuda.empty_cache()
+        r = oracle_leg(tile, args.precision, 5, 6, 1)
+        cpu = {"value": r["value"], "unit": "site-updates/s", "cores": r["cores"], "kind": "oracle",
+               "sample": f"6 x 5 Landau OR sweeps + F/theta of oracle/gf_oracle.cpp ({args.precision.upper()}) on a "
+                         f"{'x'.join(map(str, ORACLE_SAMPLE_DIMS))} sample (V={r['V']}) of the workload, "
+                         f"{r['seconds']:.1f} s"}
+
+    if rank == 0:
+        line = {
+            "metric": "site-updates/s (Landau OR sweep incl. F/theta reductions)", "value": head["value"],
+            "unit": "site-updates/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": DTYPE_NAMES[args.precision], "data": "synthetic",
+            "config": {"workload": f"Landau OR omega=1.7, {lat_name} (BASELINE.json configs[4]), "
+                                   f"{args.precision.upper()}-{args.recon}, one lattice per GPU",
+                       "lattice": list(dims), "precision": args.precision, "recon": args.recon,
+                       "step": f"{S} sweeps (= {2 * S} half-sweep kernels) + "
+                               f"{'DP reunitarisation + ' if args.precision != 'dp' else ''}one F/theta reduction",
+                       "l2": "link store %.1f GB >> 126 MB L2: every half-sweep streams from HBM, no flush needed"
+                             % (V * 4 * args.recon * (8 if args.precision == 'dp' else 4) / 1e9),
+                       "parallelism": "replicas only" if world > 1 else "single GPU"},
+            "paper_gflops": head["paper_gflops"],
+            "paper_context": "3.5 TFlops on 16 Tesla C2070, 64^3x256 SP (PAPER.md:518); other hardware, context only",
+            "gpu_launches": head["gpu_launches"], "F": head["F"], "theta": head["theta"],
+            "kernel_share_of_step": head["kernel_share_of_step"],
+            "roofline": head["roofline"], "clocks": head.get("clocks"),
+            "e2e": head.get("e2e"), "cpu_baseline": cpu, "variants": variants,
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

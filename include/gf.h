@@ -164,6 +164,13 @@ int gf_sync(gf_ctx* ctx);
 int gf_kernel_timing(gf_ctx* ctx, int enable);
 int gf_kernel_time_ms(gf_ctx* ctx, double* total_ms, int* launches, int reset);
 
+/*
+ * gf_launch_count — number of CUDA kernels this context has enqueued since the last call with
+ * reset != 0 (half-sweeps, reductions, reunitarisation, layout conversion, finalisation); memcpys are
+ * not counted.  bench.py reports it as "gpu_launches".
+ */
+int gf_launch_count(gf_ctx* ctx, int64_t* launches, int reset);
+
 /* bytes of device memory held by the context */
 int64_t gf_device_bytes(const gf_ctx* ctx);
 

@@ -52,6 +52,7 @@ struct gf_ctx {
     bool timing;
     std::vector<cudaEvent_t> ev;   // pairs (start, stop)
     size_t ev_used;
+    int64_t launches;       // kernels enqueued by this context (gf_launch_count)
     char err[512];
 };
 
@@ -125,7 +126,7 @@ int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int r
     ctx->partial = nullptr; ctx->slice_dev = nullptr; ctx->slice_host = nullptr;
     ctx->staging = nullptr; ctx->staging_bytes = 0;
     ctx->device_bytes = 0; ctx->block_override = 0;
-    ctx->timing = false; ctx->ev_used = 0;
+    ctx->timing = false; ctx->ev_used = 0; ctx->launches = 0;
     ctx->err[0] = 0;
 
     cudaError_t e = cudaMalloc((void**)&ctx->links, (size_t)link_store_bytes(ctx));
@@ -202,6 +203,7 @@ static int reset_transform(gf_ctx* ctx) {
         if (ctx->real_bytes == 4) field_identity_kernel<float><<<g, 256, 0, ctx->stream>>>(ctx->gtot, ctx->Vh);
         else field_identity_kernel<double><<<g, 256, 0, ctx->stream>>>(ctx->gtot, ctx->Vh);
         CU(cudaGetLastError());
+        ++ctx->launches;
     }
     if (ctx->gapplied) {
         CU(cudaStreamSynchronize(ctx->stream));
@@ -221,6 +223,7 @@ int gf_set_links(gf_ctx* ctx, const void* links, int elem_bytes, int is_device) 
         if (elem_bytes == 4) DISPATCH_RR(ctx, CONVERT_IN, float, links, (int64_t)0, ctx->V);
         else DISPATCH_RR(ctx, CONVERT_IN, double, links, (int64_t)0, ctx->V);
         CU(cudaGetLastError());
+        ++ctx->launches;
     } else {
         const int64_t chunk = ctx->V < STAGE_SITES ? ctx->V : STAGE_SITES;
         int rc = ensure_staging(ctx, (size_t)(chunk * link_elems * elem_bytes));
@@ -233,6 +236,7 @@ int gf_set_links(gf_ctx* ctx, const void* links, int elem_bytes, int is_device) 
             if (elem_bytes == 4) DISPATCH_RR(ctx, CONVERT_IN, float, ctx->staging, s0, ns);
             else DISPATCH_RR(ctx, CONVERT_IN, double, ctx->staging, s0, ns);
             CU(cudaGetLastError());
+            ++ctx->launches;
         }
     }
     int rc = reset_transform(ctx);
@@ -255,6 +259,7 @@ int gf_get_links(gf_ctx* ctx, void* links, int elem_bytes, int is_device) {
         if (elem_bytes == 4) DISPATCH_RR(ctx, CONVERT_OUT, float, links, (int64_t)0, ctx->V);
         else DISPATCH_RR(ctx, CONVERT_OUT, double, links, (int64_t)0, ctx->V);
         CU(cudaGetLastError());
+        ++ctx->launches;
     } else {
         const int64_t chunk = ctx->V < STAGE_SITES ? ctx->V : STAGE_SITES;
         int rc = ensure_staging(ctx, (size_t)(chunk * link_elems * elem_bytes));
@@ -265,6 +270,7 @@ int gf_get_links(gf_ctx* ctx, void* links, int elem_bytes, int is_device) {
             if (elem_bytes == 4) DISPATCH_RR(ctx, CONVERT_OUT, float, ctx->staging, s0, ns);
             else DISPATCH_RR(ctx, CONVERT_OUT, double, ctx->staging, s0, ns);
             CU(cudaGetLastError());
+            ++ctx->launches;
             CU(cudaMemcpyAsync(dst, ctx->staging, (size_t)(ns * link_elems * elem_bytes), cudaMemcpyDeviceToHost,
                                ctx->stream));
         }
@@ -294,6 +300,7 @@ int gf_get_gauge_transform(gf_ctx* ctx, void* g, int elem_bytes, int is_device) 
             else field_out_kernel<double, double><<<grid, 256, 0, ctx->stream>>>((double*)dst, ctx->gtot, dims_of(ctx), s0, ns);
         }
         CU(cudaGetLastError());
+        ++ctx->launches;
         if (!is_device)
             CU(cudaMemcpyAsync((char*)g + s0 * 18 * elem_bytes, ctx->staging, (size_t)(ns * 18 * elem_bytes),
                                cudaMemcpyDeviceToHost, ctx->stream));
@@ -348,6 +355,7 @@ static int launch_half(gf_ctx* ctx, int gauge, int algo, double param, uint64_t 
                                : launch_sweep<float, float, 12>(a, gauge, track, blk, ctx->stream);
     }
     CU(e);
+    ++ctx->launches;
     if (ctx->timing) CU(cudaEventRecord(e1, ctx->stream));
     return GF_OK;
 }
@@ -399,6 +407,7 @@ static int enqueue_measure(gf_ctx* ctx, int gauge) {
     CU(cudaGetLastError());
     slice_reduce_kernel<<<ctx->Nt, 128, 0, ctx->stream>>>(ctx->partial, 2 * ctx->meas_gx, ctx->Nt, ctx->slice_dev);
     CU(cudaGetLastError());
+    ctx->launches += 2;
     CU(cudaMemcpyAsync(ctx->slice_host, ctx->slice_dev, (size_t)2 * ctx->Nt * sizeof(double), cudaMemcpyDeviceToHost,
                        ctx->stream));
     return GF_OK;
@@ -446,11 +455,13 @@ int gf_reunitarize(gf_ctx* ctx) {
     if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_reunitarize: no links set");
     DISPATCH_RR(ctx, REUNIT_LINKS, 0);
     CU(cudaGetLastError());
+    ++ctx->launches;
     if (ctx->gtot) {
         const unsigned g = (unsigned)((2 * ctx->Vh + 255) / 256);
         if (ctx->real_bytes == 4) reunit_kernel<float, 18><<<g, 256, 0, ctx->stream>>>(ctx->gtot, ctx->Vh, 2);
         else reunit_kernel<double, 18><<<g, 256, 0, ctx->stream>>>(ctx->gtot, ctx->Vh, 2);
         CU(cudaGetLastError());
+        ++ctx->launches;
     }
     return GF_OK;
 }
@@ -467,6 +478,7 @@ int gf_coulomb_finalize(gf_ctx* ctx) {
     if (!ctx->temporal_stale) return GF_OK;
     DISPATCH_RR(ctx, FINALIZE, 0);
     CU(cudaGetLastError());
+    ++ctx->launches;
     if (!ctx->gapplied) {
         CU(cudaMalloc((void**)&ctx->gapplied, (size_t)field_store_bytes(ctx)));
         ctx->device_bytes += field_store_bytes(ctx);
@@ -572,6 +584,13 @@ int gf_kernel_time_ms(gf_ctx* ctx, double* total_ms, int* launches, int reset) {
     if (total_ms) *total_ms = tot;
     if (launches) *launches = (int)(ctx->ev_used / 2);
     if (reset) ctx->ev_used = 0;
+    return GF_OK;
+}
+
+int gf_launch_count(gf_ctx* ctx, int64_t* launches, int reset) {
+    if (!ctx) return GF_EINVAL;
+    if (launches) *launches = ctx->launches;
+    if (reset) ctx->launches = 0;
     return GF_OK;
 }
 

@@ -30,7 +30,7 @@ GF_FLAG_TRACK_TRANSFORM = 1
 
 EXPORTS = ["gf_create", "gf_destroy", "gf_set_links", "gf_get_links", "gf_get_gauge_transform", "gf_sweep",
            "gf_half_sweep", "gf_measure", "gf_run", "gf_anneal", "gf_reunitarize", "gf_coulomb_finalize",
-           "gf_sync", "gf_kernel_timing", "gf_kernel_time_ms", "gf_device_bytes", "gf_last_error", "gf_version"]
+           "gf_sync", "gf_kernel_timing", "gf_kernel_time_ms", "gf_launch_count", "gf_device_bytes", "gf_last_error", "gf_version"]
 
 
 class gf_result(ctypes.Structure):
@@ -53,6 +53,7 @@ _lib.gf_coulomb_finalize.argtypes = [_vp]
 _lib.gf_sync.argtypes = [_vp]
 _lib.gf_kernel_timing.argtypes = [_vp, _ci]
 _lib.gf_kernel_time_ms.argtypes = [_vp, ctypes.POINTER(_cd), ctypes.POINTER(_ci), _ci]
+_lib.gf_launch_count.argtypes = [_vp, ctypes.POINTER(ctypes.c_int64), _ci]
 _lib.gf_device_bytes.argtypes = [_vp]
 _lib.gf_device_bytes.restype = ctypes.c_int64
 _lib.gf_last_error.argtypes = [_vp]
@@ -190,6 +191,12 @@ def gf_kernel_time_ms(ctx, reset=True):
     ms, n = _cd(), _ci()
     _check(ctx, _lib.gf_kernel_time_ms(ctx, ctypes.byref(ms), ctypes.byref(n), 1 if reset else 0))
     return ms.value, n.value
+
+
+def gf_launch_count(ctx, reset=True):
+    n = ctypes.c_int64()
+    _check(ctx, _lib.gf_launch_count(ctx, ctypes.byref(n), 1 if reset else 0))
+    return n.value
 
 
 def gf_device_bytes(ctx):
