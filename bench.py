@@ -211,34 +211,61 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+# ---- one process per GPU: the only cross-rank traffic is the barrier and a max of the timings ----
+class Ranks:
+    """Replicas only: N independent lattices, no data-path collective."""
+
+    def __init__(self, backend: str = "nccl", device=None):
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        self.device = device
+        self.dist = None
+        if self.world > 1:
+            import torch.distributed as dist
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            kw = {"device_id": device} if (backend == "nccl" and device is not None) else {}
+            dist.init_process_group(backend, rank=self.rank, world_size=self.world, **kw)
+            self.dist = dist
+
+    def barrier(self):
+        if self.dist:
+            self.dist.barrier()
+
+    def max_over_ranks(self, x: float) -> float:
+        if not self.dist:
+            return float(x)
+        import torch
+        t = torch.tensor([x], dtype=torch.float64, device=self.device if self.device is not None else "cpu")
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def whole_job_value(self, units_per_rank: float, seconds_local: float) -> float:
+        """units all ranks processed / slowest rank's time (every rank does the same amount of work)."""
+        return self.world * units_per_rank / self.max_over_ranks(seconds_local)
+
+    def close(self):
+        if self.dist:
+            self.dist.destroy_process_group()
+
+
 # ---- the CUDA path ----------------------------------------------------------------------------
 def run_ours(args):
     import torch
-    import torch.distributed as dist
     from paper_1212_5221_b200 import gf     # fails loudly if libgf.so is missing
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    if world > 1:
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=dev)
+    ranks = Ranks("nccl", dev)
+    world, rank = ranks.world, ranks.rank
+    max_over_ranks = ranks.max_over_ranks
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        ranks.barrier()
         torch.cuda.synchronize()
-
-    def max_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
 
     dims = tuple(int(x) for x in args.lattice.split(","))
     Nx, Ny, Nz, Nt = dims
@@ -388,8 +415,7 @@ def run_ours(args):
             "e2e": head.get("e2e"), "cpu_baseline": cpu, "variants": variants,
         }
         print(json.dumps(line), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
+    ranks.close()
 
 
 def main():
