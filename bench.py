@@ -292,7 +292,7 @@ def run_ours(args):
             fx.set_links(links_dev)
 
             def step():
-                return fx.run(LANDAU, OR, OMEGA, max_sweeps=S, eps=0.0, check_every=S, reunit_every=reunit)
+                return fx.run(LANDAU, OR, OMEGA, max_sweeps=S, eps=-1.0, check_every=S, reunit_every=reunit)
 
             for _ in range(warmup):
                 step()

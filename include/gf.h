@@ -174,6 +174,9 @@ int gf_launch_count(gf_ctx* ctx, int64_t* launches, int reset);
 /* bytes of device memory held by the context */
 int64_t gf_device_bytes(const gf_ctx* ctx);
 
+/* number of lattice sites V = Nx*Ny*Nz*Nt of the context (a links buffer holds V*4*18 reals, a transform V*18) */
+int64_t gf_volume(const gf_ctx* ctx);
+
 const char* gf_last_error(const gf_ctx* ctx);
 const char* gf_version(void);
 

@@ -245,6 +245,22 @@ __global__ void slice_reduce_kernel(const double* partial, int blocks_per_slice,
     if (threadIdx.x == 0) { out[t] = a; out[Nt + t] = b; }
 }
 
+// fused-reduction partials of the half-sweep kernels: partial[t][gx][3] -> out[t][3], one block per
+// time-slice, fixed summation order (bit-reproducible)
+__global__ void red_reduce_kernel(const double* partial, int gx, double* out) {
+    const int t = blockIdx.x;
+    double a = 0.0, b = 0.0, c = 0.0;
+    for (int k = threadIdx.x; k < gx; k += blockDim.x) {
+        const double* p = partial + ((size_t)t * gx + k) * 3;
+        a += p[0]; b += p[1]; c += p[2];
+    }
+    block_sum2(a, b);
+    __syncthreads();
+    double dummy = 0.0;
+    block_sum2(c, dummy);
+    if (threadIdx.x == 0) { out[3 * t] = a; out[3 * t + 1] = b; out[3 * t + 2] = c; }
+}
+
 // ---- Coulomb finalisation: U_0(x) <- R(x) U_0(x) R(x+t)^dag, R = g_tot g_applied^dag -----------
 template <class R, int RECON>
 __global__ void coulomb_finalize_kernel(char* links, const char* gtot, const char* gapp, Dims d) {

@@ -43,6 +43,11 @@ struct gf_ctx {
     int meas_block, meas_gx;
     double* slice_dev;      // [2*Nt]
     double* slice_host;     // pinned [2*Nt]
+    // fused reductions of the half-sweep kernels
+    double* red_part[2];    // per-block partials of the even / odd half-sweep, [Nt][gx_max][3]
+    double* red_dev;        // [2][Nt][3] slice sums
+    double* red_host;       // pinned copy
+    int fused;              // gf_run uses the fused reductions (default 1)
     // host<->device staging for gf_set_links / gf_get_*
     void* staging;
     size_t staging_bytes;
@@ -100,6 +105,8 @@ const char* gf_last_error(const gf_ctx* ctx) { return ctx ? ctx->err : "null con
 
 int64_t gf_device_bytes(const gf_ctx* ctx) { return ctx ? ctx->device_bytes : 0; }
 
+int64_t gf_volume(const gf_ctx* ctx) { return ctx ? ctx->V : 0; }
+
 int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int recon, unsigned flags,
               void* cuda_stream) {
     if (!out) return GF_EINVAL;
@@ -124,6 +131,8 @@ int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int r
     ctx->links = ctx->gtot = ctx->gapplied = nullptr;
     ctx->have_links = false; ctx->temporal_stale = false;
     ctx->partial = nullptr; ctx->slice_dev = nullptr; ctx->slice_host = nullptr;
+    ctx->red_part[0] = ctx->red_part[1] = nullptr; ctx->red_dev = nullptr; ctx->red_host = nullptr;
+    ctx->fused = 1;
     ctx->staging = nullptr; ctx->staging_bytes = 0;
     ctx->device_bytes = 0; ctx->block_override = 0;
     ctx->timing = false; ctx->ev_used = 0; ctx->launches = 0;
@@ -142,13 +151,18 @@ int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int r
     if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->partial, npart * 2 * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->slice_dev, (size_t)2 * Nt * sizeof(double));
     if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->slice_host, (size_t)2 * Nt * sizeof(double));
+    const size_t nred = (size_t)((Vsh + 31) / 32) * Nt * 3;   // smallest CTA = 32 sites
+    for (int k = 0; k < 2; ++k)
+        if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->red_part[k], nred * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->red_dev, (size_t)6 * Nt * sizeof(double));
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->red_host, (size_t)6 * Nt * sizeof(double));
     if (e != cudaSuccess) {
         const int code = (e == cudaErrorMemoryAllocation) ? GF_ENOMEM : GF_ECUDA;
         gf_destroy(ctx);
         cudaGetLastError();
         return code;
     }
-    ctx->device_bytes += (int64_t)(npart * 2 + 2 * Nt) * sizeof(double);
+    ctx->device_bytes += (int64_t)(npart * 2 + 2 * Nt + 2 * nred + 6 * Nt) * sizeof(double);
     *out = ctx;
     return GF_OK;
 }
@@ -162,6 +176,10 @@ int gf_destroy(gf_ctx* ctx) {
     cudaFree(ctx->partial);
     cudaFree(ctx->slice_dev);
     cudaFree(ctx->staging);
+    cudaFree(ctx->red_part[0]);
+    cudaFree(ctx->red_part[1]);
+    cudaFree(ctx->red_dev);
+    if (ctx->red_host) cudaFreeHost(ctx->red_host);
     if (ctx->slice_host) cudaFreeHost(ctx->slice_host);
     for (cudaEvent_t ev : ctx->ev) cudaEventDestroy(ev);
     delete ctx;
@@ -322,12 +340,13 @@ static int check_sweep_args(gf_ctx* ctx, int gauge, int algo, double param) {
 }
 
 static int launch_half(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t sweep_index,
-                       int parity) {
+                       int parity, double* red = nullptr) {
     SweepArgs a;
     a.links = ctx->links; a.gtot = ctx->gtot;
     a.Nt = ctx->Nt; a.Nx = ctx->Nx; a.Ny = ctx->Ny; a.Nz = ctx->Nz;
     a.parity = parity; a.algo = algo; a.param = param; a.seed = seed; a.sweep_index = sweep_index;
-    a.red = nullptr;
+    a.red = red;
+    a.slice_skip = nullptr;
     const bool track = ctx->gtot != nullptr;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (ctx->timing) {
@@ -489,6 +508,46 @@ int gf_coulomb_finalize(gf_ctx* ctx) {
 }
 
 // ---- run loops -----------------------------------------------------------------------------------
+static int sweep_gx(const gf_ctx* ctx) {
+    const int Vsh = ctx->Nx * ctx->Ny * (ctx->Nz / 2);
+    const int block = (ctx->real_bytes == 4) ? sweep_block<float>(Vsh, ctx->block_override)
+                                             : sweep_block<double>(Vsh, ctx->block_override);
+    return (Vsh + block - 1) / block;
+}
+
+// exact F / theta of the current links (measure kernels: double, both parities) -> host scalars
+static int exact_measure(gf_ctx* ctx, int gauge, double* F, double* stop) {
+    int rc = enqueue_measure(ctx, gauge);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(ctx->stream));
+    double theta = 0.0, tmax = 0.0;
+    finish_measure(ctx, gauge, F, &theta, nullptr, &tmax);
+    *stop = (gauge == GF_COULOMB) ? tmax : theta;
+    return GF_OK;
+}
+
+// stopping quantity from per-slice sums of theta terms: theta (Eq. (7)), or max_t theta_t for Coulomb
+static double stop_from_slices(const gf_ctx* ctx, int gauge, const double* a, int sa, const double* b, int sb) {
+    const double Vs = (double)ctx->Nx * ctx->Ny * ctx->Nz;
+    double tot = 0.0, tmax = 0.0;
+    for (int t = 0; t < ctx->Nt; ++t) {
+        const double v = a[(size_t)t * sa] + (b ? b[(size_t)t * sb] : 0.0);
+        tot += v;
+        if (v / (3.0 * Vs) > tmax) tmax = v / (3.0 * Vs);
+    }
+    return (gauge == GF_COULOMB) ? tmax : tot / (3.0 * (double)ctx->V);
+}
+
+/*
+ * gf_run.  With the fused reductions (default) the odd half-sweep of a check sweep s
+ * leaves, at no extra traffic, F(s) (every link touches exactly one odd site) and theta_odd(s), the odd
+ * sites' share of theta(s); the even sites' share is what the even half-sweep of sweep s+1 sees before
+ * it updates.  theta(s) >= theta_odd(s), so a check with theta_odd(s) >= eps cannot have converged and
+ * costs nothing; only when theta_odd(s) < eps is the exact reduction (measure kernels) run, so the
+ * stopping decision is the one a reduction after every check would take.  History entries carry
+ * theta(s) = theta_odd(s) + theta_even(s), completed at the following check (or by the exact
+ * reduction); the values returned in *out always come from the exact reduction of the final links.
+ */
 int gf_run(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t first_sweep_index,
            int max_sweeps, double eps, int check_every, int reunit_every, gf_result* out, double* hist) {
     int rc = check_sweep_args(ctx, gauge, algo, param);
@@ -496,38 +555,91 @@ int gf_run(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32
     if (max_sweeps < 0 || check_every < 1 || reunit_every < 0) return fail(ctx, GF_EINVAL, "gf_run: bad loop arguments");
     rc = pre_sweep(ctx, gauge);
     if (rc) return rc;
-    double F = 0.0, theta = 0.0, tmax = 0.0, stop = 0.0;
-    bool measured = false, converged = false;
-    int s = 0, nh = 0;
+    const bool fused = ctx->fused != 0;
+    const int nd = (gauge == GF_COULOMB) ? 3 : 4;
+    const int Nt = ctx->Nt;
+    const int gx = sweep_gx(ctx);
+    double F = 0.0, stop = 0.0;
+    bool have_exact = false, converged = false;
+    // history entry still waiting for the even sites' share of theta:
+    //   stage 1 = the next even half-sweep must produce it, stage 2 = produced, reduced at the next check
+    int pend_stage = 0, pend_entry = -1;
+    std::vector<double> pend_odd((size_t)Nt, 0.0);
+    int s = 0, nh = 0, last_entry_sweep = -1;
     while (s < max_sweeps) {
-        rc = launch_half(ctx, gauge, algo, param, seed, first_sweep_index + (uint32_t)s, 0);
+        const bool check_now = ((s + 1) % check_every == 0) || (s + 1 == max_sweeps);
+        const bool red_even = fused && pend_stage == 1;
+        const uint32_t idx = first_sweep_index + (uint32_t)s;
+        rc = launch_half(ctx, gauge, algo, param, seed, idx, 0, red_even ? ctx->red_part[0] : nullptr);
         if (rc) return rc;
-        rc = launch_half(ctx, gauge, algo, param, seed, first_sweep_index + (uint32_t)s, 1);
+        if (red_even) pend_stage = 2;
+        const bool reunit_now = reunit_every && (s + 1) % reunit_every == 0;
+        rc = launch_half(ctx, gauge, algo, param, seed, idx, 1,
+                         (fused && check_now && !reunit_now) ? ctx->red_part[1] : nullptr);
         if (rc) return rc;
         ++s;
-        if (reunit_every && s % reunit_every == 0) {
+        if (reunit_now) {
             rc = gf_reunitarize(ctx);
             if (rc) return rc;
         }
-        if (s % check_every == 0 || s == max_sweeps) {
-            rc = enqueue_measure(ctx, gauge);
+        have_exact = false;
+        if (!check_now) continue;
+        if (!fused || reunit_now) {   // links were just reprojected: reduce what is stored now
+            if (pend_stage == 2) {
+                red_reduce_kernel<<<Nt, 128, 0, ctx->stream>>>(ctx->red_part[0], gx, ctx->red_dev);
+                CU(cudaGetLastError());
+                ++ctx->launches;
+                CU(cudaMemcpyAsync(ctx->red_host, ctx->red_dev, (size_t)3 * Nt * sizeof(double),
+                                   cudaMemcpyDeviceToHost, ctx->stream));
+            }
+            rc = exact_measure(ctx, gauge, &F, &stop);
             if (rc) return rc;
+            if (pend_stage == 2 && hist)
+                hist[3 * pend_entry + 2] = stop_from_slices(ctx, gauge, pend_odd.data(), 1, ctx->red_host + 2, 3);
+            pend_stage = 0;
+            have_exact = true;
+        } else {
+            red_reduce_kernel<<<Nt, 128, 0, ctx->stream>>>(ctx->red_part[1], gx, ctx->red_dev + 3 * Nt);
+            CU(cudaGetLastError());
+            ++ctx->launches;
+            if (pend_stage == 2) {
+                red_reduce_kernel<<<Nt, 128, 0, ctx->stream>>>(ctx->red_part[0], gx, ctx->red_dev);
+                CU(cudaGetLastError());
+                ++ctx->launches;
+            }
+            CU(cudaMemcpyAsync(ctx->red_host, ctx->red_dev, (size_t)6 * Nt * sizeof(double), cudaMemcpyDeviceToHost,
+                               ctx->stream));
             CU(cudaStreamSynchronize(ctx->stream));
-            finish_measure(ctx, gauge, &F, &theta, nullptr, &tmax);
-            stop = (gauge == GF_COULOMB) ? tmax : theta;
-            measured = true;
-            if (hist) { hist[3 * nh] = (double)s; hist[3 * nh + 1] = F; hist[3 * nh + 2] = stop; }
-            ++nh;
-            if (stop < eps) { converged = true; break; }
+            const double* ev = ctx->red_host;            // [t][3]: even half-sweep of this or an earlier sweep
+            const double* od = ctx->red_host + 3 * Nt;   // [t][3]: odd half-sweep of sweep s
+            if (pend_stage == 2) {
+                if (hist) hist[3 * pend_entry + 2] = stop_from_slices(ctx, gauge, pend_odd.data(), 1, ev + 2, 3);
+                pend_stage = 0;
+            }
+            double fs = 0.0;
+            for (int t = 0; t < Nt; ++t) fs += od[3 * t];
+            F = fs / (3.0 * nd * (double)ctx->V);
+            stop = stop_from_slices(ctx, gauge, od + 1, 3, nullptr, 0);   // lower bound of theta(s)
+            if (stop < eps) {
+                rc = exact_measure(ctx, gauge, &F, &stop);
+                if (rc) return rc;
+                have_exact = true;
+            } else {
+                for (int t = 0; t < Nt; ++t) pend_odd[(size_t)t] = od[3 * t + 1];
+                pend_stage = 1;
+                pend_entry = nh;
+            }
         }
+        if (hist) { hist[3 * nh] = (double)s; hist[3 * nh + 1] = F; hist[3 * nh + 2] = stop; }
+        last_entry_sweep = s;
+        ++nh;
+        if (have_exact && stop < eps) { converged = true; break; }
     }
-    if (!measured) {
-        rc = enqueue_measure(ctx, gauge);
+    if (!have_exact) {
+        rc = exact_measure(ctx, gauge, &F, &stop);
         if (rc) return rc;
-        CU(cudaStreamSynchronize(ctx->stream));
-        finish_measure(ctx, gauge, &F, &theta, nullptr, &tmax);
-        stop = (gauge == GF_COULOMB) ? tmax : theta;
         converged = stop < eps;
+        if (hist && nh > 0 && last_entry_sweep == s) { hist[3 * (nh - 1) + 1] = F; hist[3 * (nh - 1) + 2] = stop; }
     }
     if (gauge == GF_COULOMB && ctx->gtot) {
         rc = gf_coulomb_finalize(ctx);
@@ -591,6 +703,13 @@ int gf_launch_count(gf_ctx* ctx, int64_t* launches, int reset) {
     if (!ctx) return GF_EINVAL;
     if (launches) *launches = ctx->launches;
     if (reset) ctx->launches = 0;
+    return GF_OK;
+}
+
+// tuning hook (not declared in gf.h): 0 = gf_run measures after every check with the measure kernels
+int gf_debug_set_fused(gf_ctx* ctx, int fused) {
+    if (!ctx) return GF_EINVAL;
+    ctx->fused = fused != 0;
     return GF_OK;
 }
 

@@ -34,7 +34,11 @@ struct SweepArgs {
     double param;        // omega | p | T
     uint64_t seed;
     uint32_t sweep_index;
-    double* red;         // nullptr, or per-block partial sums [gridDim.x][2] of (F, theta) terms
+    // nullptr, or per-block partial sums [gridDim.y = Nt][gridDim.x][3] of
+    //   (F term after the update, theta term after the update, theta term before the update)
+    // of the sites this launch updates (fused reductions)
+    double* red;
+    const unsigned char* slice_skip;   // nullptr, or [Nt]: 1 = leave this time-slice alone (frozen)
 };
 
 // ---- asynchronous global -> shared copies -------------------------------------------------
@@ -84,27 +88,27 @@ GF_DEV void smem_get(const unsigned char* smem, int nlinks, int l, Mat<R>& m) {
 
 // store the first RECON reals of a matrix to its place in HBM
 template <class R, int RECON>
-GF_DEV void global_put(char* plane0, int64_t Vh, int cb, const Mat<R>& m) {
+GF_DEV void global_put(char* plane0, int64_t Vh, int64_t cb, const Mat<R>& m) {
     typedef Layout<R, RECON> L;
     typedef typename Vec16<R>::type V;
 #pragma unroll
     for (int c = 0; c < L::NV16; ++c)
-        *reinterpret_cast<V*>(plane0 + (int64_t)c * 16 * Vh + (int64_t)cb * 16) = Vec16<R>::pack(&m.v[c * L::PER16]);
+        *reinterpret_cast<V*>(plane0 + (int64_t)c * 16 * Vh + cb * 16) = Vec16<R>::pack(&m.v[c * L::PER16]);
     if (L::TAIL8)
-        *reinterpret_cast<float2*>(plane0 + (int64_t)L::NV16 * 16 * Vh + (int64_t)cb * 8) =
+        *reinterpret_cast<float2*>(plane0 + (int64_t)L::NV16 * 16 * Vh + cb * 8) =
             make_float2((float)m.v[L::NV16 * L::PER16], (float)m.v[L::NV16 * L::PER16 + 1]);
 }
 template <class R, int RECON>
-GF_DEV void global_get(const char* plane0, int64_t Vh, int cb, Mat<R>& m) {
+GF_DEV void global_get(const char* plane0, int64_t Vh, int64_t cb, Mat<R>& m) {
     typedef Layout<R, RECON> L;
     typedef typename Vec16<R>::type V;
 #pragma unroll
     for (int c = 0; c < L::NV16; ++c) {
-        const V q = *reinterpret_cast<const V*>(plane0 + (int64_t)c * 16 * Vh + (int64_t)cb * 16);
+        const V q = *reinterpret_cast<const V*>(plane0 + (int64_t)c * 16 * Vh + cb * 16);
         Vec16<R>::unpack(q, &m.v[c * L::PER16]);
     }
     if (L::TAIL8) {
-        const float2 q = *reinterpret_cast<const float2*>(plane0 + (int64_t)L::NV16 * 16 * Vh + (int64_t)cb * 8);
+        const float2 q = *reinterpret_cast<const float2*>(plane0 + (int64_t)L::NV16 * 16 * Vh + cb * 8);
         m.v[L::NV16 * L::PER16] = (R)q.x;
         m.v[L::NV16 * L::PER16 + 1] = (R)q.y;
     }
@@ -175,6 +179,43 @@ GF_DEV void subgroup_mag(Herm<A> (&M)[3], Mat<A>& G, const SweepArgs& args, uint
     sub_left<I, J>(G, g);
 }
 
+// ---- per-site terms of the fused reductions (a9 inside the sweep) -------------
+// Landau/Coulomb: Delta(x) = traceless[(K - K^dag)/2i] (Eq. (6)), term = tr[Delta Delta^dag]
+// (Eq. (7)); Re tr K(x) is the sum of Re tr over the 2d links that touch x (Eq. (17)).
+template <class A>
+GF_DEV A theta_term_landau(const Mat<A>& K) {
+    A sum = A(0), tr = A(0);
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            const A xr = K.v[RE(a, b)] - K.v[RE(b, a)];
+            const A xi = K.v[IM(a, b)] + K.v[IM(b, a)];
+            sum += A(0.25) * (xr * xr + xi * xi);
+            if (a == b) tr += A(0.5) * xi;
+        }
+    return sum - tr * tr / A(3);
+}
+template <class A>
+GF_DEV A f_term_landau(const Mat<A>& K) { return K.v[RE(0, 0)] + K.v[RE(1, 1)] + K.v[RE(2, 2)]; }
+// MAG: sum over the subgroups of |X^s_12|^2 = E_s^2 + F_s^2 (R11); local value of Eq. (11)
+template <class A>
+GF_DEV A theta_term_mag(const Herm<A> (&M)[3]) {
+    A th = A(0);
+    {   const A E = M[0].o[1] - M[1].o[1], F = M[0].o[0] - M[1].o[0]; th += E * E + F * F; }
+    {   const A E = M[0].o[3] - M[2].o[3], F = M[0].o[2] - M[2].o[2]; th += E * E + F * F; }
+    {   const A E = M[1].o[5] - M[2].o[5], F = M[1].o[4] - M[2].o[4]; th += E * E + F * F; }
+    return th;
+}
+template <class A>
+GF_DEV A f_term_mag(const Herm<A> (&M)[3]) { return M[0].d[0] + M[1].d[1] + M[2].d[2]; }
+
+GF_DEV double warp_sum_d(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+
 // ---- the kernel ----------------------------------------------------------------------------
 template <class R>
 struct SweepLaunch {   // CTA shape per storage type
@@ -182,7 +223,7 @@ struct SweepLaunch {   // CTA shape per storage type
     static constexpr int MIN_CTAS = sizeof(R) == 4 ? 3 : 3;
 };
 
-template <class R, class A, int RECON, int GAUGE, bool STOCH, bool TRACK>
+template <class R, class A, int RECON, int GAUGE, bool STOCH, bool TRACK, bool RED>
 __global__ void __launch_bounds__(SweepLaunch<R>::MAX_BLOCK, SweepLaunch<R>::MIN_CTAS)
 sweep_kernel(const SweepArgs args) {
     typedef Layout<R, RECON> L;
@@ -191,18 +232,24 @@ sweep_kernel(const SweepArgs args) {
     constexpr int NL = 2 * ND;
     extern __shared__ __align__(16) unsigned char smem[];
 
-    const int64_t Vh = (int64_t)args.Nt * args.Nx * args.Ny * (args.Nz / 2);
-    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= Vh) return;   // no barriers below, so early exit is safe
-    const int cb = (int)idx;
+    // grid = (ceil(Vsh / block), Nt): blockIdx.y is the time-slice, so a CTA never straddles slices
+    // (per-slice reductions, frozen slices).  Threads past the end of the slice redo the last site
+    // without storing, so that every thread reaches the block reduction.
+    const int Nzh = args.Nz >> 1;
+    const int Vsh = args.Nx * args.Ny * Nzh;
+    const int64_t Vh = (int64_t)args.Nt * Vsh;
+    const int t = blockIdx.y;
+    if (args.slice_skip && args.slice_skip[t]) return;   // block-uniform
+    const int i_raw = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool active = i_raw < Vsh;
+    const int i_s = active ? i_raw : Vsh - 1;
+    const int64_t cb = (int64_t)t * Vsh + i_s;
 
     // ---- a1: decode the checkerboard index, neighbours with periodic wrap ----
-    const int Nzh = args.Nz >> 1;
-    int rem = cb;
+    int rem = i_s;
     const int zh = rem % Nzh; rem /= Nzh;
-    const int y = rem % args.Ny; rem /= args.Ny;
-    const int x = rem % args.Nx;
-    const int t = rem / args.Nx;
+    const int y = rem % args.Ny;
+    const int x = rem / args.Ny;
     // own parity in the 4-d colouring; Coulomb's 3-d colouring p3 maps to (p3 + t) & 1
     const int par = (GAUGE == GAUGE_COULOMB) ? ((args.parity + t) & 1) : args.parity;
     const int r = (t + x + y + par) & 1;   // z = 2 zh + r
@@ -210,11 +257,12 @@ sweep_kernel(const SweepArgs args) {
     const uint32_t site = (uint32_t)(((t * args.Nx + x) * args.Ny + y) * args.Nz + z);
 
     // checkerboard index of x - mu (lives in the other parity's arrays)
-    const int sy = Nzh, sx = Nzh * args.Ny, st = Nzh * args.Ny * args.Nx;
-    const int cbn0 = cb + (t ? -st : (args.Nt - 1) * st);
-    const int cbn1 = cb + (x ? -sx : (args.Nx - 1) * sx);
-    const int cbn2 = cb + (y ? -sy : (args.Ny - 1) * sy);
-    const int cbn3 = r ? cb : (zh ? cb - 1 : cb + Nzh - 1);
+    const int sy = Nzh, sx = Nzh * args.Ny;
+    const int64_t st = Vsh;
+    const int64_t cbn0 = cb + (t ? -st : (int64_t)(args.Nt - 1) * st);
+    const int64_t cbn1 = cb + (x ? -sx : (args.Nx - 1) * sx);
+    const int64_t cbn2 = cb + (y ? -sy : (args.Ny - 1) * sy);
+    const int64_t cbn3 = r ? cb : (zh ? cb - 1 : cb + Nzh - 1);
 
     // ---- a2: stream the 2d links into this thread's shared-memory slice ----
     const int nthr = blockDim.x, tid = threadIdx.x;
@@ -224,14 +272,14 @@ sweep_kernel(const SweepArgs args) {
         const int mu = MU0 + (l >> 1);
         const bool down = l & 1;
         const char* p0 = args.links + L::link_offset(down ? 1 - par : par, mu, Vh);
-        const int c_site = !down ? cb : (mu == 0) ? cbn0 : (mu == 1) ? cbn1 : (mu == 2) ? cbn2 : cbn3;
+        const int64_t c_site = !down ? cb : (mu == 0) ? cbn0 : (mu == 1) ? cbn1 : (mu == 2) ? cbn2 : cbn3;
 #pragma unroll
         for (int c = 0; c < L::NV16; ++c)
             cp_async16(sbase + (uint32_t)(((l * L::NV16 + c) * nthr + tid) * 16),
-                       p0 + (int64_t)c * 16 * Vh + (int64_t)c_site * 16);
+                       p0 + (int64_t)c * 16 * Vh + c_site * 16);
         if (L::TAIL8)
             cp_async8(sbase + (uint32_t)(NL * L::NV16 * nthr * 16 + (l * nthr + tid) * 8),
-                      p0 + (int64_t)L::NV16 * 16 * Vh + (int64_t)c_site * 8);
+                      p0 + (int64_t)L::NV16 * 16 * Vh + c_site * 8);
     }
     Mat<R> Gt;
     if (TRACK) global_get<R, 18>(args.gtot + Layout<R, 18>::site_offset(par, Vh), Vh, cb, Gt);
@@ -259,6 +307,11 @@ sweep_kernel(const SweepArgs args) {
         else acc_dagger(K, U);
     }
 
+    // fused reductions: theta term of this site before its update (completes theta of the previous sweep)
+    constexpr bool red = RED;   // args.red is non-null exactly when RED
+    A th_pre = A(0);
+    if (red) th_pre = (GAUGE == GAUGE_MAG) ? theta_term_mag<A>(M) : theta_term_landau<A>(K);
+
     // ---- a4/a5: Step 1 through the three SU(2) subgroups, G = g3 g2 g1 ----
     if (GAUGE == GAUGE_MAG) {
         subgroup_mag<0, 1, 0, STOCH, A>(M, G, args, site);
@@ -270,6 +323,14 @@ sweep_kernel(const SweepArgs args) {
         subgroup_landau<1, 2, 2, STOCH, A>(K, G, args, site);
     }
 
+    // the summary now is that of the updated site (K -> G K, M_k -> G M_k G^dag): its F and theta terms
+    double red_f = 0.0, red_th = 0.0, red_pre = 0.0;
+    if (red && active) {
+        red_f = (double)((GAUGE == GAUGE_MAG) ? f_term_mag<A>(M) : f_term_landau<A>(K));
+        red_th = (double)((GAUGE == GAUGE_MAG) ? theta_term_mag<A>(M) : theta_term_landau<A>(K));
+        red_pre = (double)th_pre;
+    }
+
     // ---- a6/a7: Step 2, pass 2 over the links: rotate and write back in place ----
     constexpr int NR = (RECON == 12) ? 2 : 3;
     Mat<R> Gr;   // G in the storage type (MP: Step 2 in SP)
@@ -278,22 +339,49 @@ sweep_kernel(const SweepArgs args) {
 #pragma unroll 1
     for (int m = 0; m < ND; ++m) {
         const int mu = MU0 + m;
-        const int cdn = (mu == 0) ? cbn0 : (mu == 1) ? cbn1 : (mu == 2) ? cbn2 : cbn3;
+        const int64_t cdn = (mu == 0) ? cbn0 : (mu == 1) ? cbn1 : (mu == 2) ? cbn2 : cbn3;
         Mat<R> U, O;
         smem_get<R, RECON>(smem, NL, 2 * m, U);
         mul_left<NR>(Gr, U, O);
-        global_put<R, RECON>(args.links + L::link_offset(par, mu, Vh), Vh, cb, O);
+        if (active) global_put<R, RECON>(args.links + L::link_offset(par, mu, Vh), Vh, cb, O);
         smem_get<R, RECON>(smem, NL, 2 * m + 1, U);
         mul_right_dagger<NR>(U, Gr, O);
-        global_put<R, RECON>(args.links + L::link_offset(1 - par, mu, Vh), Vh, cdn, O);
+        if (active) global_put<R, RECON>(args.links + L::link_offset(1 - par, mu, Vh), Vh, cdn, O);
     }
 
     // ---- a8: accumulate the transform, g_tot(x) <- G g_tot(x) ----
     if (TRACK) {
         Mat<R> O;
         mul_left<3>(G, Gt, O);
-        global_put<R, 18>(args.gtot + Layout<R, 18>::site_offset(par, Vh), Vh, cb, O);
+        if (active) global_put<R, 18>(args.gtot + Layout<R, 18>::site_offset(par, Vh), Vh, cb, O);
     }
+
+    // ---- a9 fused: block partials of (F, theta after, theta before), double, fixed order ----
+    if (red) {   // block-uniform
+        __shared__ double red_s[3][4];
+        const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+        red_f = warp_sum_d(red_f);
+        red_th = warp_sum_d(red_th);
+        red_pre = warp_sum_d(red_pre);
+        if (lane == 0) { red_s[0][w] = red_f; red_s[1][w] = red_th; red_s[2][w] = red_pre; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const int nw = (blockDim.x + 31) >> 5;
+            double a = 0.0, b = 0.0, c = 0.0;
+            for (int k = 0; k < nw; ++k) { a += red_s[0][k]; b += red_s[1][k]; c += red_s[2][k]; }
+            double* p = args.red + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * 3;
+            p[0] = a; p[1] = b; p[2] = c;
+        }
+    }
+}
+
+// CTA size actually used for a slice of Vsh sites per parity (block_override = 0: default)
+template <class R>
+inline int sweep_block(int Vsh, int block_override) {
+    int block = block_override;
+    if (block <= 0 || block > SweepLaunch<R>::MAX_BLOCK) block = SweepLaunch<R>::MAX_BLOCK;
+    const int need = ((Vsh + 31) / 32) * 32;
+    return block < need ? block : need;
 }
 
 // host-side launcher of one (R, A, RECON) family; defined in sweep_inst.cuh

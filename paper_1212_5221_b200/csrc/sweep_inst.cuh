@@ -6,12 +6,12 @@
 
 namespace gf {
 
-template <class R, class A, int RECON, int GAUGE, bool STOCH, bool TRACK>
+template <class R, class A, int RECON, int GAUGE, bool STOCH, bool TRACK, bool RED>
 static cudaError_t launch_one(const SweepArgs& args, int block, cudaStream_t stream) {
     constexpr int ND = (GAUGE == GAUGE_COULOMB) ? 3 : 4;
-    auto kern = sweep_kernel<R, A, RECON, GAUGE, STOCH, TRACK>;
-    const int64_t Vh = (int64_t)args.Nt * args.Nx * args.Ny * (args.Nz / 2);
-    if (block <= 0 || block > SweepLaunch<R>::MAX_BLOCK) block = SweepLaunch<R>::MAX_BLOCK;
+    auto kern = sweep_kernel<R, A, RECON, GAUGE, STOCH, TRACK, RED>;
+    const int Vsh = args.Nx * args.Ny * (args.Nz / 2);
+    block = sweep_block<R>(Vsh, block);
     const size_t smem = (size_t)block * 2 * ND * Layout<R, RECON>::LINK_BYTES;
     static size_t smem_set = 0;   // per instantiation
     if (smem > smem_set) {
@@ -21,7 +21,7 @@ static cudaError_t launch_one(const SweepArgs& args, int block, cudaStream_t str
         if (e != cudaSuccess) return e;
         smem_set = smem;
     }
-    const unsigned grid = (unsigned)((Vh + block - 1) / block);
+    const dim3 grid((unsigned)((Vsh + block - 1) / block), (unsigned)args.Nt);
     kern<<<grid, block, smem, stream>>>(args);
     return cudaGetLastError();
 }
@@ -29,12 +29,17 @@ static cudaError_t launch_one(const SweepArgs& args, int block, cudaStream_t str
 template <class R, class A, int RECON, int GAUGE>
 static cudaError_t launch_gauge(const SweepArgs& args, bool track, int block, cudaStream_t stream) {
     const bool stoch = (args.algo == ALGO_SR || args.algo == ALGO_SA);
-    if (stoch) {
-        if (track) return launch_one<R, A, RECON, GAUGE, true, true>(args, block, stream);
-        return launch_one<R, A, RECON, GAUGE, true, false>(args, block, stream);
+    const int which = (stoch ? 4 : 0) | (track ? 2 : 0) | (args.red ? 1 : 0);
+    switch (which) {
+        case 0: return launch_one<R, A, RECON, GAUGE, false, false, false>(args, block, stream);
+        case 1: return launch_one<R, A, RECON, GAUGE, false, false, true>(args, block, stream);
+        case 2: return launch_one<R, A, RECON, GAUGE, false, true, false>(args, block, stream);
+        case 3: return launch_one<R, A, RECON, GAUGE, false, true, true>(args, block, stream);
+        case 4: return launch_one<R, A, RECON, GAUGE, true, false, false>(args, block, stream);
+        case 5: return launch_one<R, A, RECON, GAUGE, true, false, true>(args, block, stream);
+        case 6: return launch_one<R, A, RECON, GAUGE, true, true, false>(args, block, stream);
+        default: return launch_one<R, A, RECON, GAUGE, true, true, true>(args, block, stream);
     }
-    if (track) return launch_one<R, A, RECON, GAUGE, false, true>(args, block, stream);
-    return launch_one<R, A, RECON, GAUGE, false, false>(args, block, stream);
 }
 
 template <class R, class A, int RECON>

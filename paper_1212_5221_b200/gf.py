@@ -30,7 +30,7 @@ GF_FLAG_TRACK_TRANSFORM = 1
 
 EXPORTS = ["gf_create", "gf_destroy", "gf_set_links", "gf_get_links", "gf_get_gauge_transform", "gf_sweep",
            "gf_half_sweep", "gf_measure", "gf_run", "gf_anneal", "gf_reunitarize", "gf_coulomb_finalize",
-           "gf_sync", "gf_kernel_timing", "gf_kernel_time_ms", "gf_launch_count", "gf_device_bytes", "gf_last_error", "gf_version"]
+           "gf_sync", "gf_kernel_timing", "gf_kernel_time_ms", "gf_launch_count", "gf_device_bytes", "gf_volume", "gf_last_error", "gf_version"]
 
 
 class gf_result(ctypes.Structure):
@@ -56,10 +56,13 @@ _lib.gf_kernel_time_ms.argtypes = [_vp, ctypes.POINTER(_cd), ctypes.POINTER(_ci)
 _lib.gf_launch_count.argtypes = [_vp, ctypes.POINTER(ctypes.c_int64), _ci]
 _lib.gf_device_bytes.argtypes = [_vp]
 _lib.gf_device_bytes.restype = ctypes.c_int64
+_lib.gf_volume.argtypes = [_vp]
+_lib.gf_volume.restype = ctypes.c_int64
 _lib.gf_last_error.argtypes = [_vp]
 _lib.gf_last_error.restype = ctypes.c_char_p
 _lib.gf_version.restype = ctypes.c_char_p
 _lib.gf_debug_set_block.argtypes = [_vp, _ci]
+_lib.gf_debug_set_fused.argtypes = [_vp, _ci]
 
 
 class GfError(RuntimeError):
@@ -118,18 +121,27 @@ def gf_destroy(ctx):
     return _lib.gf_destroy(ctx)
 
 
+def _sized(ctx, n, per_site, what):
+    want = gf_volume(ctx) * per_site
+    if n != want:
+        raise ValueError(f"{what}: buffer holds {n} reals, the context's lattice needs {want}")
+
+
 def gf_set_links(ctx, links):
     p, eb, dev, n = _buffer(links)
+    _sized(ctx, n, 72, "gf_set_links")
     return _check(ctx, _lib.gf_set_links(ctx, _vp(p), eb, dev))
 
 
 def gf_get_links(ctx, out):
     p, eb, dev, n = _buffer(out)
+    _sized(ctx, n, 72, "gf_get_links")
     return _check(ctx, _lib.gf_get_links(ctx, _vp(p), eb, dev))
 
 
 def gf_get_gauge_transform(ctx, out):
     p, eb, dev, n = _buffer(out)
+    _sized(ctx, n, 18, "gf_get_gauge_transform")
     return _check(ctx, _lib.gf_get_gauge_transform(ctx, _vp(p), eb, dev))
 
 
@@ -199,12 +211,20 @@ def gf_launch_count(ctx, reset=True):
     return n.value
 
 
+def gf_volume(ctx):
+    return int(_lib.gf_volume(ctx))
+
+
 def gf_device_bytes(ctx):
     return int(_lib.gf_device_bytes(ctx))
 
 
 def gf_last_error(ctx) -> str:
     return _lib.gf_last_error(ctx).decode()
+
+
+def gf_debug_set_fused(ctx, fused):
+    return _check(ctx, _lib.gf_debug_set_fused(ctx, 1 if fused else 0))
 
 
 def gf_debug_set_block(ctx, block):

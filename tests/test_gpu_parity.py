@@ -223,6 +223,8 @@ def test_config0_full_run(gf, oracle):
     assert abs(r["F"] - F) <= 1e-10
     assert r["theta"] < 1e-12 and abs(r["theta"] - th) <= 0.1 * th
     np.testing.assert_allclose(r["history"][:, 1], [h[1] for h in hist], atol=1e-10)
+    # theta per sweep (fused: odd sites' share from sweep s + even sites' share seen by sweep s+1)
+    np.testing.assert_allclose(r["history"][:, 2], [h[2] for h in hist], rtol=1e-6)
     assert np.abs(got - ref).max() < 1e-9
 
 
@@ -241,6 +243,7 @@ def test_config1_full_run(gf, oracle):
     assert abs(r["sweeps"] - s) <= 2
     n = min(len(hist), len(r["history"]))
     np.testing.assert_allclose(r["history"][:n, 1], [h[1] for h in hist][:n], atol=1e-10)
+    np.testing.assert_allclose(r["history"][:n - 5, 2], [h[2] for h in hist][:n - 5], rtol=1e-4)
 
 
 @pytest.mark.parametrize("prec,recon", [(SP, 12), (MP, 12), (SP, 18)])
@@ -315,6 +318,49 @@ def test_mag_anneal_then_or(gf, oracle):
     # whatever copy was reached, it is a gauge transform of the input (Eq. 1) by the returned g
     gc = g[..., 0] + 1j * g[..., 1]
     assert np.abs(inputs.as_complex(got) - inputs.gauge_transform(U, gc)).max() < 1e-10
+
+
+@pytest.mark.parametrize("gauge,prec,recon", [(LANDAU, DP, 18), (COULOMB, DP, 12), (MAG, DP, 18), (LANDAU, SP, 12),
+                                              (COULOMB, MP, 12), (MAG, SP, 18)])
+@pytest.mark.parametrize("check_every", [1, 3])
+def test_fused_run_equals_measured_run(gf, oracle, gauge, prec, recon, check_every):
+    # gf_run's fused reductions (F and theta from inside the half-sweeps) against (a) the same run with a
+    # measure-kernel reduction after every check and (b) the oracle's run loop: same number of sweeps,
+    # same history.  Ragged slice (Vsh = 5*6*3 = 90 sites: one full 64-CTA + a tail / a 96-thread CTA).
+    dims = (5 * 2, 6, 6, 4)
+    dt = oracle_dtype(prec)
+    U = make(dims, eps=0.4, seed=380 + gauge)
+    L = inputs.as_real(U, dt)
+    eps = 1e-9 if prec == DP else 3e-8
+    kw = dict(max_sweeps=400, eps=eps, check_every=check_every, reunit_every=(0 if prec == DP else 50))
+    ref = L.copy()
+    s, F, th, hist, conv = oracle.run(ref, gauge, OR, 1.7, mixed=(prec == MP), **kw)
+    res = []
+    for fused in (True, False):
+        with gf.GaugeFixer(*dims, precision=prec, recon=recon) as fx:
+            gf.gf_debug_set_fused(fx.ctx, fused)
+            fx.set_links(L)
+            res.append(fx.run(gauge, OR, 1.7, history=True, **kw))
+    a, b = res
+    assert a["converged"] == b["converged"] == conv
+    if prec == DP:
+        assert a["sweeps"] == b["sweeps"] == s
+        # both from the exact reduction; the links differ in the last bits only (the kernel with fused
+        # reductions is another instantiation: other FMA contractions)
+        assert abs(a["F"] - b["F"]) <= 1e-13 and abs(a["theta"] - b["theta"]) <= 1e-3 * b["theta"]
+        assert abs(a["F"] - F) <= 1e-10 and abs(a["theta"] - th) <= 0.1 * th
+        n = len(hist)
+        assert len(a["history"]) == len(b["history"]) == n
+        np.testing.assert_allclose(a["history"][:, 1], b["history"][:, 1], atol=1e-12)
+        np.testing.assert_allclose(a["history"][:, 2], b["history"][:, 2], rtol=1e-6)
+        np.testing.assert_allclose(a["history"][:, 1], [h[1] for h in hist], atol=1e-10)
+        np.testing.assert_allclose(a["history"][:, 2], [h[2] for h in hist], rtol=1e-5)
+    else:
+        assert abs(a["sweeps"] - b["sweeps"]) <= 3 * check_every and abs(a["sweeps"] - s) <= 3 * check_every
+        assert abs(a["F"] - F) <= 1e-5 and abs(b["F"] - F) <= 1e-5
+        n = min(len(a["history"]), len(b["history"]), len(hist)) - 2
+        np.testing.assert_allclose(a["history"][:n, 1], b["history"][:n, 1], atol=2e-6)
+        np.testing.assert_allclose(a["history"][:n, 1], [h[1] for h in hist][:n], atol=1e-5)
 
 
 def test_edge_cases(gf, oracle):
