@@ -60,6 +60,7 @@ typedef struct gf_ctx gf_ctx; /* opaque */
 
 /* gf_create flags */
 #define GF_FLAG_TRACK_TRANSFORM 1u /* accumulate g(x) so that gf_get_gauge_transform / Coulomb finalisation work */
+#define GF_FLAG_FREEZE_SLICES 2u   /* gf_run(Coulomb): stop sweeping a time-slice once its own theta_t < eps */
 
 /*
  * gf_create — allocate a context for an Nx*Ny*Nz*Nt periodic lattice (BASELINE.json north_star:
@@ -129,6 +130,20 @@ typedef struct {
  */
 int gf_run(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t first_sweep_index,
            int max_sweeps, double eps, int check_every, int reunit_every, gf_result* out, double* hist);
+
+/*
+ * Per-slice Coulomb fixing (contexts created with GF_FLAG_FREEZE_SLICES).  In Coulomb gauge every
+ * time-slice is an independent optimisation problem and the paper fixes them one at a
+ * time.  Here all slices are swept in the same launches, and gf_run(GF_COULOMB) stops
+ * sweeping slice t at the first check at which theta_t < eps (the CTAs of a stopped slice exit at
+ * once), so the result of slice t is that of a stand-alone run on that slice.  gf_run then returns
+ * GF_OK when every slice has stopped; out->theta = max_t theta_t of the final links.  Reprojection
+ * (reunit_every) still covers all links.  Landau/MAG runs ignore the flag.
+ * gf_get_slice_sweeps: sweeps[Nt] (host) receives the number of sweeps applied to every slice by the
+ * last gf_run (without the flag or for other gauges: that run's sweep count in every entry).
+ * GF_ESTATE before the first gf_run.
+ */
+int gf_get_slice_sweeps(gf_ctx* ctx, int* sweeps);
 
 /*
  * gf_anneal — simulated annealing schedule: n_steps heatbath sweeps at

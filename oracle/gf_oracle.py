@@ -195,6 +195,49 @@ def run(links: np.ndarray, gauge: int, algo: int, param: float, seed: int = 0, m
     return s, m["F"], stop_value(m, gauge), hist, conv
 
 
+def run_coulomb_freeze(links: np.ndarray, algo: int, param: float, seed: int = 0, max_sweeps: int = 1000,
+                       eps: float = 1e-12, check_every: int = 1, reunit_every: int = 0, mixed: bool = False,
+                       gtot: np.ndarray | None = None, first_sweep_index: int = 0):
+    """Coulomb gauge with every time-slice treated as the independent problem it is (PAPER.md:76,
+    376 "one slice at a time"): slice t stops being swept at the first check at which its own
+    theta_t < eps (R21b).  Written the slow, obvious way: sweep everything, then put the
+    spatial links (and the tracked transform) of the already-stopped slices back.  Reprojection, when
+    asked for, is applied to every link of every slice.  Returns
+    (sweeps, F, max_t theta_t, history[(sweep, F, max_t theta_t)], converged, slice_sweeps[Nt])."""
+    Nt = links.shape[0]
+    frozen = np.zeros(Nt, dtype=bool)
+    slice_sweeps = np.zeros(Nt, dtype=np.int64)
+    hist = []
+    m = None
+    s = 0
+    conv = False
+    while s < max_sweeps:
+        keep = links[frozen].copy()
+        keep_g = gtot[frozen].copy() if gtot is not None else None
+        sweep(links, COULOMB, algo, param, seed, first_sweep_index + s, mixed, gtot)
+        links[frozen] = keep
+        if gtot is not None:
+            gtot[frozen] = keep_g
+        s += 1
+        if reunit_every and s % reunit_every == 0:
+            reunitarize(links)
+            if gtot is not None:
+                reunitarize(gtot)
+        if s % check_every == 0 or s == max_sweeps:
+            m = measure(links, COULOMB)
+            newly = (~frozen) & (m["theta_slice"] < eps)
+            slice_sweeps[newly] = s
+            frozen |= newly
+            hist.append((s, m["F"], float(m["theta_slice"].max())))
+            if frozen.all():
+                conv = True
+                break
+    if m is None:
+        m = measure(links, COULOMB)
+    slice_sweeps[~frozen] = s
+    return s, m["F"], float(m["theta_slice"].max()), hist, conv, slice_sweeps
+
+
 def temperature(k: int, n_steps: int, T_hi: float, T_lo: float) -> float:
     """Linear schedule (BASELINE.json config 3; R17)."""
     if n_steps <= 1:

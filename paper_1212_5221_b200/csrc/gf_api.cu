@@ -48,6 +48,11 @@ struct gf_ctx {
     double* red_dev;        // [2][Nt][3] slice sums
     double* red_host;       // pinned copy
     int fused;              // gf_run uses the fused reductions (default 1)
+    // per-slice Coulomb fixing (GF_FLAG_FREEZE_SLICES)
+    unsigned char* skip_dev;    // [Nt] 1 = slice stopped, its CTAs exit at once
+    unsigned char* skip_host;   // pinned copy
+    std::vector<int> slice_sweeps;   // sweeps applied to every slice by the last gf_run
+    bool have_slice_sweeps;
     // host<->device staging for gf_set_links / gf_get_*
     void* staging;
     size_t staging_bytes;
@@ -133,6 +138,7 @@ int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int r
     ctx->partial = nullptr; ctx->slice_dev = nullptr; ctx->slice_host = nullptr;
     ctx->red_part[0] = ctx->red_part[1] = nullptr; ctx->red_dev = nullptr; ctx->red_host = nullptr;
     ctx->fused = 1;
+    ctx->skip_dev = nullptr; ctx->skip_host = nullptr; ctx->have_slice_sweeps = false;
     ctx->staging = nullptr; ctx->staging_bytes = 0;
     ctx->device_bytes = 0; ctx->block_override = 0;
     ctx->timing = false; ctx->ev_used = 0; ctx->launches = 0;
@@ -156,6 +162,8 @@ int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int r
         if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->red_part[k], nred * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->red_dev, (size_t)6 * Nt * sizeof(double));
     if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->red_host, (size_t)6 * Nt * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->skip_dev, (size_t)Nt);
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->skip_host, (size_t)Nt);
     if (e != cudaSuccess) {
         const int code = (e == cudaErrorMemoryAllocation) ? GF_ENOMEM : GF_ECUDA;
         gf_destroy(ctx);
@@ -179,6 +187,8 @@ int gf_destroy(gf_ctx* ctx) {
     cudaFree(ctx->red_part[0]);
     cudaFree(ctx->red_part[1]);
     cudaFree(ctx->red_dev);
+    cudaFree(ctx->skip_dev);
+    if (ctx->skip_host) cudaFreeHost(ctx->skip_host);
     if (ctx->red_host) cudaFreeHost(ctx->red_host);
     if (ctx->slice_host) cudaFreeHost(ctx->slice_host);
     for (cudaEvent_t ev : ctx->ev) cudaEventDestroy(ev);
@@ -340,13 +350,13 @@ static int check_sweep_args(gf_ctx* ctx, int gauge, int algo, double param) {
 }
 
 static int launch_half(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t sweep_index,
-                       int parity, double* red = nullptr) {
+                       int parity, double* red = nullptr, const unsigned char* skip = nullptr) {
     SweepArgs a;
     a.links = ctx->links; a.gtot = ctx->gtot;
     a.Nt = ctx->Nt; a.Nx = ctx->Nx; a.Ny = ctx->Ny; a.Nz = ctx->Nz;
     a.parity = parity; a.algo = algo; a.param = param; a.seed = seed; a.sweep_index = sweep_index;
     a.red = red;
-    a.slice_skip = nullptr;
+    a.slice_skip = skip;
     const bool track = ctx->gtot != nullptr;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (ctx->timing) {
@@ -526,18 +536,6 @@ static int exact_measure(gf_ctx* ctx, int gauge, double* F, double* stop) {
     return GF_OK;
 }
 
-// stopping quantity from per-slice sums of theta terms: theta (Eq. (7)), or max_t theta_t for Coulomb
-static double stop_from_slices(const gf_ctx* ctx, int gauge, const double* a, int sa, const double* b, int sb) {
-    const double Vs = (double)ctx->Nx * ctx->Ny * ctx->Nz;
-    double tot = 0.0, tmax = 0.0;
-    for (int t = 0; t < ctx->Nt; ++t) {
-        const double v = a[(size_t)t * sa] + (b ? b[(size_t)t * sb] : 0.0);
-        tot += v;
-        if (v / (3.0 * Vs) > tmax) tmax = v / (3.0 * Vs);
-    }
-    return (gauge == GF_COULOMB) ? tmax : tot / (3.0 * (double)ctx->V);
-}
-
 /*
  * gf_run.  With the fused reductions (default) the odd half-sweep of a check sweep s
  * leaves, at no extra traffic, F(s) (every link touches exactly one odd site) and theta_odd(s), the odd
@@ -547,6 +545,11 @@ static double stop_from_slices(const gf_ctx* ctx, int gauge, const double* a, in
  * stopping decision is the one a reduction after every check would take.  History entries carry
  * theta(s) = theta_odd(s) + theta_even(s), completed at the following check (or by the exact
  * reduction); the values returned in *out always come from the exact reduction of the final links.
+ *
+ * Per-slice Coulomb fixing (GF_FLAG_FREEZE_SLICES): the same bound is used slice by
+ * slice.  A slice whose theta_odd,t(s) < eps triggers the exact reduction; every not yet stopped slice
+ * with exact theta_t(s) < eps is stopped at sweep s: its flag in skip_dev makes its CTAs exit at once
+ * in all later half-sweeps, and its exact slice sums stand in for the (no longer written) partials.
  */
 int gf_run(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t first_sweep_index,
            int max_sweeps, double eps, int check_every, int reunit_every, gf_result* out, double* hist) {
@@ -556,11 +559,58 @@ int gf_run(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32
     rc = pre_sweep(ctx, gauge);
     if (rc) return rc;
     const bool fused = ctx->fused != 0;
-    const int nd = (gauge == GF_COULOMB) ? 3 : 4;
+    const bool coulomb = gauge == GF_COULOMB;
+    const bool freeze = coulomb && (ctx->flags & GF_FLAG_FREEZE_SLICES);
+    const int nd = coulomb ? 3 : 4;
     const int Nt = ctx->Nt;
     const int gx = sweep_gx(ctx);
+    const double Vs = (double)ctx->Nx * ctx->Ny * ctx->Nz;
     double F = 0.0, stop = 0.0;
     bool have_exact = false, converged = false;
+
+    // slices already stopped, with the exact slice sums (F terms, theta terms) they were stopped at
+    std::vector<unsigned char> frozen((size_t)Nt, 0);
+    std::vector<double> fz_F((size_t)Nt, 0.0), fz_th((size_t)Nt, 0.0);
+    int n_frozen = 0;
+    ctx->slice_sweeps.assign((size_t)Nt, 0);
+    ctx->have_slice_sweeps = true;
+    const unsigned char* skip = nullptr;
+    if (freeze) {
+        memset(ctx->skip_host, 0, (size_t)Nt);
+        CU(cudaMemcpyAsync(ctx->skip_dev, ctx->skip_host, (size_t)Nt, cudaMemcpyHostToDevice, ctx->stream));
+        skip = ctx->skip_dev;
+    }
+    // stopping quantity from per-slice sums of theta terms a[t] (+ b[t]): theta (Eq. (7)), or max_t theta_t
+    auto stop_of = [&](const double* a, int sa, const double* b, int sb) {
+        double tot = 0.0, tmax = 0.0;
+        for (int t = 0; t < Nt; ++t) {
+            const double v = frozen[(size_t)t] ? fz_th[(size_t)t]
+                                               : a[(size_t)t * sa] + (b ? b[(size_t)t * sb] : 0.0);
+            tot += v;
+            if (v / (3.0 * Vs) > tmax) tmax = v / (3.0 * Vs);
+        }
+        return coulomb ? tmax : tot / (3.0 * (double)ctx->V);
+    };
+    // stop every running slice whose exact theta_t (slice_host, just reduced) is below eps
+    auto apply_freeze = [&](int s_now) -> int {
+        bool changed = false;
+        for (int t = 0; t < Nt; ++t) {
+            if (frozen[(size_t)t]) continue;
+            if (ctx->slice_host[Nt + t] / (3.0 * Vs) < eps) {
+                frozen[(size_t)t] = 1;
+                fz_F[(size_t)t] = ctx->slice_host[t];
+                fz_th[(size_t)t] = ctx->slice_host[Nt + t];
+                ctx->slice_sweeps[(size_t)t] = s_now;
+                ctx->skip_host[t] = 1;
+                ++n_frozen;
+                changed = true;
+            }
+        }
+        if (changed)
+            CU(cudaMemcpyAsync(ctx->skip_dev, ctx->skip_host, (size_t)Nt, cudaMemcpyHostToDevice, ctx->stream));
+        return GF_OK;
+    };
+
     // history entry still waiting for the even sites' share of theta:
     //   stage 1 = the next even half-sweep must produce it, stage 2 = produced, reduced at the next check
     int pend_stage = 0, pend_entry = -1;
@@ -570,12 +620,12 @@ int gf_run(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32
         const bool check_now = ((s + 1) % check_every == 0) || (s + 1 == max_sweeps);
         const bool red_even = fused && pend_stage == 1;
         const uint32_t idx = first_sweep_index + (uint32_t)s;
-        rc = launch_half(ctx, gauge, algo, param, seed, idx, 0, red_even ? ctx->red_part[0] : nullptr);
+        rc = launch_half(ctx, gauge, algo, param, seed, idx, 0, red_even ? ctx->red_part[0] : nullptr, skip);
         if (rc) return rc;
         if (red_even) pend_stage = 2;
         const bool reunit_now = reunit_every && (s + 1) % reunit_every == 0;
         rc = launch_half(ctx, gauge, algo, param, seed, idx, 1,
-                         (fused && check_now && !reunit_now) ? ctx->red_part[1] : nullptr);
+                         (fused && check_now && !reunit_now) ? ctx->red_part[1] : nullptr, skip);
         if (rc) return rc;
         ++s;
         if (reunit_now) {
@@ -595,9 +645,13 @@ int gf_run(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32
             rc = exact_measure(ctx, gauge, &F, &stop);
             if (rc) return rc;
             if (pend_stage == 2 && hist)
-                hist[3 * pend_entry + 2] = stop_from_slices(ctx, gauge, pend_odd.data(), 1, ctx->red_host + 2, 3);
+                hist[3 * pend_entry + 2] = stop_of(pend_odd.data(), 1, ctx->red_host + 2, 3);
             pend_stage = 0;
             have_exact = true;
+            if (freeze) {
+                rc = apply_freeze(s);
+                if (rc) return rc;
+            }
         } else {
             red_reduce_kernel<<<Nt, 128, 0, ctx->stream>>>(ctx->red_part[1], gx, ctx->red_dev + 3 * Nt);
             CU(cudaGetLastError());
@@ -613,17 +667,25 @@ int gf_run(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32
             const double* ev = ctx->red_host;            // [t][3]: even half-sweep of this or an earlier sweep
             const double* od = ctx->red_host + 3 * Nt;   // [t][3]: odd half-sweep of sweep s
             if (pend_stage == 2) {
-                if (hist) hist[3 * pend_entry + 2] = stop_from_slices(ctx, gauge, pend_odd.data(), 1, ev + 2, 3);
+                if (hist) hist[3 * pend_entry + 2] = stop_of(pend_odd.data(), 1, ev + 2, 3);
                 pend_stage = 0;
             }
             double fs = 0.0;
-            for (int t = 0; t < Nt; ++t) fs += od[3 * t];
+            for (int t = 0; t < Nt; ++t) fs += frozen[(size_t)t] ? fz_F[(size_t)t] : od[3 * t];
             F = fs / (3.0 * nd * (double)ctx->V);
-            stop = stop_from_slices(ctx, gauge, od + 1, 3, nullptr, 0);   // lower bound of theta(s)
-            if (stop < eps) {
+            stop = stop_of(od + 1, 3, nullptr, 0);   // lower bound of theta(s)
+            bool need_exact = stop < eps;
+            if (freeze)   // a running slice may have converged on its own
+                for (int t = 0; t < Nt && !need_exact; ++t)
+                    need_exact = !frozen[(size_t)t] && od[3 * t + 1] / (3.0 * Vs) < eps;
+            if (need_exact) {
                 rc = exact_measure(ctx, gauge, &F, &stop);
                 if (rc) return rc;
                 have_exact = true;
+                if (freeze) {
+                    rc = apply_freeze(s);
+                    if (rc) return rc;
+                }
             } else {
                 for (int t = 0; t < Nt; ++t) pend_odd[(size_t)t] = od[3 * t + 1];
                 pend_stage = 1;
@@ -633,21 +695,31 @@ int gf_run(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32
         if (hist) { hist[3 * nh] = (double)s; hist[3 * nh + 1] = F; hist[3 * nh + 2] = stop; }
         last_entry_sweep = s;
         ++nh;
-        if (have_exact && stop < eps) { converged = true; break; }
+        if (freeze ? (n_frozen == Nt) : (have_exact && stop < eps)) { converged = true; break; }
     }
     if (!have_exact) {
         rc = exact_measure(ctx, gauge, &F, &stop);
         if (rc) return rc;
-        converged = stop < eps;
+        converged = freeze ? (n_frozen == Nt) : (stop < eps);
         if (hist && nh > 0 && last_entry_sweep == s) { hist[3 * (nh - 1) + 1] = F; hist[3 * (nh - 1) + 2] = stop; }
     }
-    if (gauge == GF_COULOMB && ctx->gtot) {
+    for (int t = 0; t < Nt; ++t)
+        if (!frozen[(size_t)t]) ctx->slice_sweeps[(size_t)t] = s;
+    if (coulomb && ctx->gtot) {
         rc = gf_coulomb_finalize(ctx);
         if (rc) return rc;
         CU(cudaStreamSynchronize(ctx->stream));
     }
     if (out) { out->sweeps = s; out->F = F; out->theta = stop; }
     return converged ? GF_OK : GF_NOT_CONVERGED;
+}
+
+int gf_get_slice_sweeps(gf_ctx* ctx, int* sweeps) {
+    if (!ctx) return GF_EINVAL;
+    if (!sweeps) return fail(ctx, GF_EINVAL, "gf_get_slice_sweeps: NULL pointer");
+    if (!ctx->have_slice_sweeps) return fail(ctx, GF_ESTATE, "gf_get_slice_sweeps: no gf_run yet");
+    for (int t = 0; t < ctx->Nt; ++t) sweeps[t] = ctx->slice_sweeps[(size_t)t];
+    return GF_OK;
 }
 
 int gf_anneal(gf_ctx* ctx, int gauge, double T_hi, double T_lo, int n_steps, int n_micro, uint64_t seed,

@@ -27,9 +27,10 @@ GF_SP, GF_DP, GF_MP = 0, 1, 2
 GF_LANDAU, GF_COULOMB, GF_MAG = 0, 1, 2
 GF_OR, GF_SR, GF_SA, GF_MICRO = 0, 1, 2, 3
 GF_FLAG_TRACK_TRANSFORM = 1
+GF_FLAG_FREEZE_SLICES = 2
 
 EXPORTS = ["gf_create", "gf_destroy", "gf_set_links", "gf_get_links", "gf_get_gauge_transform", "gf_sweep",
-           "gf_half_sweep", "gf_measure", "gf_run", "gf_anneal", "gf_reunitarize", "gf_coulomb_finalize",
+           "gf_half_sweep", "gf_measure", "gf_run", "gf_get_slice_sweeps", "gf_anneal", "gf_reunitarize", "gf_coulomb_finalize",
            "gf_sync", "gf_kernel_timing", "gf_kernel_time_ms", "gf_launch_count", "gf_device_bytes", "gf_volume", "gf_last_error", "gf_version"]
 
 
@@ -47,6 +48,7 @@ _lib.gf_sweep.argtypes = [_vp, _ci, _ci, _cd, _u64, _u32]
 _lib.gf_half_sweep.argtypes = [_vp, _ci, _ci, _cd, _u64, _u32, _ci]
 _lib.gf_measure.argtypes = [_vp, _ci, ctypes.POINTER(_cd), ctypes.POINTER(_cd), _vp]
 _lib.gf_run.argtypes = [_vp, _ci, _ci, _cd, _u64, _u32, _ci, _cd, _ci, _ci, ctypes.POINTER(gf_result), _vp]
+_lib.gf_get_slice_sweeps.argtypes = [_vp, _vp]
 _lib.gf_anneal.argtypes = [_vp, _ci, _cd, _cd, _ci, _ci, _u64, _u32, ctypes.POINTER(_u32)]
 _lib.gf_reunitarize.argtypes = [_vp]
 _lib.gf_coulomb_finalize.argtypes = [_vp]
@@ -176,6 +178,12 @@ def gf_run(ctx, gauge, algo, param, seed=0, first_sweep_index=0, max_sweeps=1000
     return out
 
 
+def gf_get_slice_sweeps(ctx, Nt):
+    out = np.zeros(Nt, dtype=np.int32)
+    _check(ctx, _lib.gf_get_slice_sweeps(ctx, _vp(out.ctypes.data)))
+    return out
+
+
 def gf_anneal(ctx, gauge, T_hi, T_lo, n_steps, n_micro, seed, first_sweep_index=0):
     nxt = _u32()
     _check(ctx, _lib.gf_anneal(ctx, gauge, float(T_hi), float(T_lo), n_steps, n_micro, seed, first_sweep_index,
@@ -234,11 +242,12 @@ def gf_debug_set_block(ctx, block):
 class GaugeFixer:
     """Context manager around one gf_ctx.  Methods forward to the C entry points of the same name."""
 
-    def __init__(self, Nx, Ny, Nz, Nt, precision=GF_DP, recon=18, track_transform=False, cuda_stream=None):
+    def __init__(self, Nx, Ny, Nz, Nt, precision=GF_DP, recon=18, track_transform=False, cuda_stream=None,
+                 freeze_slices=False):
         self.dims = (Nx, Ny, Nz, Nt)
         self.precision, self.recon = precision, recon
-        self.ctx = gf_create(Nx, Ny, Nz, Nt, precision, recon, GF_FLAG_TRACK_TRANSFORM if track_transform else 0,
-                             cuda_stream)
+        flags = (GF_FLAG_TRACK_TRANSFORM if track_transform else 0) | (GF_FLAG_FREEZE_SLICES if freeze_slices else 0)
+        self.ctx = gf_create(Nx, Ny, Nz, Nt, precision, recon, flags, cuda_stream)
 
     def close(self):
         if self.ctx is not None:
@@ -288,6 +297,9 @@ class GaugeFixer:
 
     def run(self, gauge, algo, param, **kw):
         return gf_run(self.ctx, gauge, algo, param, **kw)
+
+    def slice_sweeps(self):
+        return gf_get_slice_sweeps(self.ctx, self.dims[3])
 
     def anneal(self, gauge, T_hi, T_lo, n_steps, n_micro, seed, first_sweep_index=0):
         return gf_anneal(self.ctx, gauge, T_hi, T_lo, n_steps, n_micro, seed, first_sweep_index)

@@ -276,6 +276,62 @@ def test_coulomb_sp_run_with_reunit(gf, oracle, prec, recon):
     assert np.abs(inputs.as_complex(got) - want).max() < 2e-5
 
 
+@pytest.mark.parametrize("prec,recon,check_every,reunit", [(DP, 18, 1, 0), (DP, 12, 5, 0), (SP, 12, 10, 100),
+                                                          (MP, 18, 10, 100)])
+def test_coulomb_freeze_slices(gf, oracle, prec, recon, check_every, reunit):
+    # Per-slice Coulomb fixing (GF_FLAG_FREEZE_SLICES): every slice stops at the first
+    # check at which its own theta_t < eps.  Oracle: run_coulomb_freeze (pinned to stand-alone runs of the
+    # single slices).  The number of sweeps each slice received is an integer decision taken from
+    # theta_t: DP must agree exactly, SP/MP within one check (theta at the 1e-10 SP noise floor).
+    dims = (6, 8, 6, 6)
+    eps = 1e-12 if prec == DP else 1e-10
+    U = make(dims, eps=0.6, seed=345)
+    L = inputs.as_real(U, oracle_dtype(prec))
+    ref = L.copy()
+    Gref = oracle.identity_transform(ref)
+    s, F, th, hist, conv, ss = oracle.run_coulomb_freeze(ref, OR, 1.7, max_sweeps=4000, eps=eps,
+                                                         check_every=check_every, reunit_every=reunit,
+                                                         mixed=(prec == MP), gtot=Gref)
+    oracle.coulomb_finalize(ref, Gref)
+    with gf.GaugeFixer(*dims, precision=prec, recon=recon, track_transform=True, freeze_slices=True) as fx:
+        fx.set_links(L)
+        r = fx.run(COULOMB, OR, 1.7, max_sweeps=4000, eps=eps, check_every=check_every, reunit_every=reunit,
+                   history=True)
+        ss_g = fx.slice_sweeps()
+        got = fx.get_links(dtype=np.float64)
+        g = fx.get_gauge_transform(dtype=np.float64)
+        F2, th2, ths = fx.measure(COULOMB, slices=True)
+    assert conv and r["converged"]
+    assert len(set(ss.tolist())) > 1            # the slices really stop at different sweeps
+    if prec == DP:
+        assert np.array_equal(ss_g, ss) and r["sweeps"] == s
+        assert abs(r["F"] - F) <= 1e-10 and ths.max() < eps
+        assert np.abs(got - ref).max() < 1e-8
+        n = len(hist)
+        assert len(r["history"]) == n
+        np.testing.assert_allclose(r["history"][:, 1], [h[1] for h in hist], atol=1e-10)
+    else:
+        assert np.abs(ss_g - ss).max() <= check_every
+        assert abs(r["F"] - F) <= 1e-5
+        assert ths.max() < 3 * eps               # a stopped SP slice is reprojected afterwards
+    gc = g[..., 0] + 1j * g[..., 1]
+    want = inputs.gauge_transform(U, gc)
+    assert np.abs(inputs.as_complex(got) - want).max() < (1e-10 if prec == DP else 2e-5)
+
+
+def test_freeze_flag_ignored_outside_coulomb(gf, oracle):
+    dims = (4, 4, 4, 4)
+    L = inputs.as_real(make(dims, eps=0.3, seed=346))
+    out = []
+    for fz in (False, True):
+        with gf.GaugeFixer(*dims, precision=DP, freeze_slices=fz) as fx:
+            fx.set_links(L)
+            r = fx.run(LANDAU, OR, 1.7, max_sweeps=2000, eps=1e-12)
+            out.append((r["sweeps"], r["F"], fx.get_links(), fx.slice_sweeps()))
+    assert out[0][0] == out[1][0] and out[0][1] == out[1][1] and np.array_equal(out[0][2], out[1][2])
+    assert np.all(out[1][3] == out[1][0])
+
+
 def test_mag_anneal_then_or(gf, oracle):
     # BASELINE.json config 3 in miniature: MAG, SA 1.45 -> 0.01 linear with 3 microcanonical sweeps
     # per heatbath sweep (Philox seed 1234), then OR 1.7 to theta < 1e-12, DP.

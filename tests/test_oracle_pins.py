@@ -327,6 +327,29 @@ def test_coulomb_slices_independent(oracle):
     assert mA["theta_slice"][2] == mB["theta_slice"][2]
 
 
+def test_coulomb_freeze_is_one_standalone_run_per_slice(oracle):
+    # the paper fixes one slice at a time.  The frozen run of the whole lattice must give,
+    # in slice t, bit for bit what the plain run loop gives on a lattice made of slice t alone (all its
+    # slices then converge at the same check), with the same sweep count; slices stop at different sweeps.
+    U = small_config(44, dims=(4, 4, 4, 4), eps=0.6)
+    L = inputs.as_real(U)
+    G = oracle.identity_transform(L)
+    s, F, th, hist, conv, ss = oracle.run_coulomb_freeze(L, OR, 1.7, max_sweeps=2000, eps=1e-12, check_every=3,
+                                                         gtot=G)
+    assert conv and th < 1e-12 and s == ss.max() and len(set(ss.tolist())) > 1
+    for t in range(4):
+        one = inputs.as_real(np.stack([U[t], U[t]]))
+        g1 = oracle.identity_transform(one)
+        s1, F1, th1, h1, c1 = oracle.run(one, COULOMB, OR, 1.7, max_sweeps=2000, eps=1e-12, check_every=3, gtot=g1)
+        assert c1 and s1 == ss[t]
+        assert np.array_equal(one[0][..., 1:, :, :, :], L[t][..., 1:, :, :, :])
+        assert np.array_equal(g1[0], G[t])
+    # temporal links untouched until finalisation; afterwards the whole field is a gauge transform of U
+    assert np.array_equal(L[..., 0, :, :, :], inputs.as_real(U)[..., 0, :, :, :])
+    oracle.coulomb_finalize(L, G)
+    np.testing.assert_allclose(H.plaquettes(H.cplx(L)), H.plaquettes(U), atol=1e-12)
+
+
 def test_coulomb_finalize_keeps_all_plaquettes(oracle):
     U0 = small_config(43)
     L = inputs.as_real(U0)
