@@ -32,6 +32,11 @@ GF_DEV void set_zero(Mat<T>& m) {
     for (int k = 0; k < 18; ++k) m.v[k] = T(0);
 }
 
+// fused multiply-add in the matrix type (explicit: the compiler may contract a*b+c but not
+// re-associate a*b - c*d + e, which would otherwise cost an extra rounding and instruction per term)
+GF_DEV float fma_t(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+GF_DEV double fma_t(double a, double b, double c) { return __fma_rn(a, b, c); }
+
 // third row from the first two: w = (u x v)^*
 template <class T>
 GF_DEV void reconstruct_row2(Mat<T>& m) {
@@ -39,12 +44,16 @@ GF_DEV void reconstruct_row2(Mat<T>& m) {
     for (int j = 0; j < 3; ++j) {
         const int a = (j + 1) % 3, b = (j + 2) % 3;
         // (u_a v_b - u_b v_a), then conjugate
-        T re = m.v[RE(0, a)] * m.v[RE(1, b)] - m.v[IM(0, a)] * m.v[IM(1, b)] -
-               (m.v[RE(0, b)] * m.v[RE(1, a)] - m.v[IM(0, b)] * m.v[IM(1, a)]);
-        T im = m.v[RE(0, a)] * m.v[IM(1, b)] + m.v[IM(0, a)] * m.v[RE(1, b)] -
-               (m.v[RE(0, b)] * m.v[IM(1, a)] + m.v[IM(0, b)] * m.v[RE(1, a)]);
+        T re = m.v[RE(0, a)] * m.v[RE(1, b)];
+        re = fma_t(-m.v[IM(0, a)], m.v[IM(1, b)], re);
+        re = fma_t(-m.v[RE(0, b)], m.v[RE(1, a)], re);
+        re = fma_t(m.v[IM(0, b)], m.v[IM(1, a)], re);
+        T im = m.v[RE(0, b)] * m.v[IM(1, a)];   // -Im(u_a v_b - u_b v_a)
+        im = fma_t(m.v[IM(0, b)], m.v[RE(1, a)], im);
+        im = fma_t(-m.v[RE(0, a)], m.v[IM(1, b)], im);
+        im = fma_t(-m.v[IM(0, a)], m.v[RE(1, b)], im);
         m.v[RE(2, j)] = re;
-        m.v[IM(2, j)] = -im;
+        m.v[IM(2, j)] = im;
     }
 }
 
@@ -55,12 +64,17 @@ GF_DEV void mul_left(const Mat<TG>& G, const Mat<T>& M, Mat<T>& out) {
     for (int i = 0; i < NR; ++i)
 #pragma unroll
         for (int j = 0; j < 3; ++j) {
-            T re = T(0), im = T(0);
+            T re = (T)G.v[RE(i, 0)] * M.v[RE(0, j)];
+            T im = (T)G.v[RE(i, 0)] * M.v[IM(0, j)];
+            re = fma_t(-(T)G.v[IM(i, 0)], M.v[IM(0, j)], re);
+            im = fma_t((T)G.v[IM(i, 0)], M.v[RE(0, j)], im);
 #pragma unroll
-            for (int k = 0; k < 3; ++k) {
+            for (int k = 1; k < 3; ++k) {
                 const T gr = (T)G.v[RE(i, k)], gi = (T)G.v[IM(i, k)];
-                re += gr * M.v[RE(k, j)] - gi * M.v[IM(k, j)];
-                im += gr * M.v[IM(k, j)] + gi * M.v[RE(k, j)];
+                re = fma_t(gr, M.v[RE(k, j)], re);
+                re = fma_t(-gi, M.v[IM(k, j)], re);
+                im = fma_t(gr, M.v[IM(k, j)], im);
+                im = fma_t(gi, M.v[RE(k, j)], im);
             }
             out.v[RE(i, j)] = re;
             out.v[IM(i, j)] = im;
@@ -74,12 +88,18 @@ GF_DEV void mul_right_dagger(const Mat<T>& M, const Mat<TG>& G, Mat<T>& out) {
     for (int i = 0; i < NR; ++i)
 #pragma unroll
         for (int j = 0; j < 3; ++j) {
-            T re = T(0), im = T(0);
+            // sum_k M_ik conj(G_jk)
+            T re = M.v[RE(i, 0)] * (T)G.v[RE(j, 0)];
+            T im = M.v[IM(i, 0)] * (T)G.v[RE(j, 0)];
+            re = fma_t(M.v[IM(i, 0)], (T)G.v[IM(j, 0)], re);
+            im = fma_t(-M.v[RE(i, 0)], (T)G.v[IM(j, 0)], im);
 #pragma unroll
-            for (int k = 0; k < 3; ++k) {
-                const T gr = (T)G.v[RE(j, k)], gi = -(T)G.v[IM(j, k)];   // conj(G_jk)
-                re += M.v[RE(i, k)] * gr - M.v[IM(i, k)] * gi;
-                im += M.v[RE(i, k)] * gi + M.v[IM(i, k)] * gr;
+            for (int k = 1; k < 3; ++k) {
+                const T gr = (T)G.v[RE(j, k)], gi = (T)G.v[IM(j, k)];
+                re = fma_t(M.v[RE(i, k)], gr, re);
+                re = fma_t(M.v[IM(i, k)], gi, re);
+                im = fma_t(M.v[IM(i, k)], gr, im);
+                im = fma_t(-M.v[RE(i, k)], gi, im);
             }
             out.v[RE(i, j)] = re;
             out.v[IM(i, j)] = im;

@@ -66,20 +66,23 @@ struct Vec16<double> {
     GF_DEV static double2 pack(const double* v) { return make_double2(v[0], v[1]); }
 };
 
-// read link slot l of this thread from shared memory (and rebuild row 2 when RECON = 12)
-template <class R, int RECON>
+// read link slot l of this thread from shared memory (and rebuild row 2 when RECON = 12).
+// The slice stride NTHR is the compile-time maximal CTA size, whatever blockDim.x is, so that every
+// shared-memory address is tid*16 + an immediate (+ one multiply-add for a run-time l).
+template <class R, int RECON, int NTHR>
 GF_DEV void smem_get(const unsigned char* smem, int nlinks, int l, Mat<R>& m) {
     typedef Layout<R, RECON> L;
     typedef typename Vec16<R>::type V;
-    const int nthr = blockDim.x, tid = threadIdx.x;
+    const int tid = threadIdx.x;
+    const unsigned char* base = smem + tid * 16 + l * (L::NV16 * NTHR * 16);
 #pragma unroll
     for (int c = 0; c < L::NV16; ++c) {
-        const V q = *reinterpret_cast<const V*>(smem + ((size_t)(l * L::NV16 + c) * nthr + tid) * 16);
+        const V q = *reinterpret_cast<const V*>(base + c * NTHR * 16);
         Vec16<R>::unpack(q, &m.v[c * L::PER16]);
     }
     if (L::TAIL8) {
-        const float2 q = *reinterpret_cast<const float2*>(smem + (size_t)nlinks * L::NV16 * nthr * 16 +
-                                                          ((size_t)l * nthr + tid) * 8);
+        const float2 q = *reinterpret_cast<const float2*>(smem + nlinks * L::NV16 * NTHR * 16 +
+                                                          (l * NTHR + tid) * 8);
         m.v[L::NV16 * L::PER16] = (R)q.x;
         m.v[L::NV16 * L::PER16 + 1] = (R)q.y;
     }
@@ -91,11 +94,13 @@ template <class R, int RECON>
 GF_DEV void global_put(char* plane0, int64_t Vh, int64_t cb, const Mat<R>& m) {
     typedef Layout<R, RECON> L;
     typedef typename Vec16<R>::type V;
+    const int64_t plane = 16 * Vh;
+    char* q = plane0 + cb * 16;
 #pragma unroll
-    for (int c = 0; c < L::NV16; ++c)
-        *reinterpret_cast<V*>(plane0 + (int64_t)c * 16 * Vh + cb * 16) = Vec16<R>::pack(&m.v[c * L::PER16]);
+    for (int c = 0; c < L::NV16; ++c, q += plane)
+        *reinterpret_cast<V*>(q) = Vec16<R>::pack(&m.v[c * L::PER16]);
     if (L::TAIL8)
-        *reinterpret_cast<float2*>(plane0 + (int64_t)L::NV16 * 16 * Vh + cb * 8) =
+        *reinterpret_cast<float2*>(q - cb * 8) =
             make_float2((float)m.v[L::NV16 * L::PER16], (float)m.v[L::NV16 * L::PER16 + 1]);
 }
 template <class R, int RECON>
@@ -217,14 +222,17 @@ GF_DEV double warp_sum_d(double v) {
 }
 
 // ---- the kernel ----------------------------------------------------------------------------
-template <class R>
-struct SweepLaunch {   // CTA shape per storage type (DESIGN.md §6.5)
+#ifndef GF_MIN_CTAS_MP
+#define GF_MIN_CTAS_MP 4
+#endif
+template <class R, class A = R>
+struct SweepLaunch {   // CTA shape per storage type (DESIGN.md §6.1)
     static constexpr int MAX_BLOCK = sizeof(R) == 4 ? 128 : 64;
-    static constexpr int MIN_CTAS = sizeof(R) == 4 ? 3 : 3;
+    static constexpr int MIN_CTAS = (sizeof(R) == 4 && sizeof(A) == 8) ? GF_MIN_CTAS_MP : 3;
 };
 
 template <class R, class A, int RECON, int GAUGE, bool STOCH, bool TRACK, bool RED>
-__global__ void __launch_bounds__(SweepLaunch<R>::MAX_BLOCK, SweepLaunch<R>::MIN_CTAS)
+__global__ void __launch_bounds__(SweepLaunch<R, A>::MAX_BLOCK, SweepLaunch<R, A>::MIN_CTAS)
 sweep_kernel(const SweepArgs args) {
     typedef Layout<R, RECON> L;
     constexpr int MU0 = (GAUGE == GAUGE_COULOMB) ? 1 : 0;
@@ -265,21 +273,36 @@ sweep_kernel(const SweepArgs args) {
     const int64_t cbn3 = r ? cb : (zh ? cb - 1 : cb + Nzh - 1);
 
     // ---- a2: stream the 2d links into this thread's shared-memory slice ----
-    const int nthr = blockDim.x, tid = threadIdx.x;
-    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem);
+    // slice layout [link][chunk][NTHR] x 16 bytes (+ [link][NTHR] x 8 bytes of SP-18 tails); pointers step
+    // by one chunk plane (16 Vh bytes) and one link array (LINK_BYTES Vh bytes)
+    constexpr int NTHR = SweepLaunch<R, A>::MAX_BLOCK;
+    const int tid = threadIdx.x;
+    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem) + (uint32_t)tid * 16;
+    const int64_t plane = 16 * Vh;
+    const int64_t lstride = (int64_t)L::LINK_BYTES * Vh;
+    char* const up0 = args.links + L::link_offset(par, MU0, Vh);        // U_mu(x): own parity
+    char* const dn0 = args.links + L::link_offset(1 - par, MU0, Vh);    // U_mu(x - mu): other parity
+    {
+        const char* pu = up0;
+        const char* pd = dn0;
 #pragma unroll
-    for (int l = 0; l < NL; ++l) {
-        const int mu = MU0 + (l >> 1);
-        const bool down = l & 1;
-        const char* p0 = args.links + L::link_offset(down ? 1 - par : par, mu, Vh);
-        const int64_t c_site = !down ? cb : (mu == 0) ? cbn0 : (mu == 1) ? cbn1 : (mu == 2) ? cbn2 : cbn3;
+        for (int m = 0; m < ND; ++m, pu += lstride, pd += lstride) {
+            const int mu = MU0 + m;
+            const int64_t cdn = (mu == 0) ? cbn0 : (mu == 1) ? cbn1 : (mu == 2) ? cbn2 : cbn3;
+            const char* qu = pu + cb * 16;
+            const char* qd = pd + cdn * 16;
 #pragma unroll
-        for (int c = 0; c < L::NV16; ++c)
-            cp_async16(sbase + (uint32_t)(((l * L::NV16 + c) * nthr + tid) * 16),
-                       p0 + (int64_t)c * 16 * Vh + c_site * 16);
-        if (L::TAIL8)
-            cp_async8(sbase + (uint32_t)(NL * L::NV16 * nthr * 16 + (l * nthr + tid) * 8),
-                      p0 + (int64_t)L::NV16 * 16 * Vh + c_site * 8);
+            for (int c = 0; c < L::NV16; ++c, qu += plane, qd += plane) {
+                cp_async16(sbase + (uint32_t)(((2 * m) * L::NV16 + c) * NTHR * 16), qu);
+                cp_async16(sbase + (uint32_t)(((2 * m + 1) * L::NV16 + c) * NTHR * 16), qd);
+            }
+            if (L::TAIL8) {
+                cp_async8(sbase - (uint32_t)tid * 8 + (uint32_t)(NL * L::NV16 * NTHR * 16 + (2 * m) * NTHR * 8),
+                          qu - cb * 8);
+                cp_async8(sbase - (uint32_t)tid * 8 + (uint32_t)(NL * L::NV16 * NTHR * 16 + (2 * m + 1) * NTHR * 8),
+                          qd - cdn * 8);
+            }
+        }
     }
     Mat<R> Gt;
     if (TRACK) global_get<R, 18>(args.gtot + Layout<R, 18>::site_offset(par, Vh), Vh, cb, Gt);
@@ -299,10 +322,10 @@ sweep_kernel(const SweepArgs args) {
 #pragma unroll 1
     for (int m = 0; m < ND; ++m) {
         Mat<R> U;
-        smem_get<R, RECON>(smem, NL, 2 * m, U);       // U_mu(x)
+        smem_get<R, RECON, NTHR>(smem, NL, 2 * m, U);       // U_mu(x)
         if (GAUGE == GAUGE_MAG) { mag_acc_up<0>(M[0], U); mag_acc_up<1>(M[1], U); mag_acc_up<2>(M[2], U); }
         else acc_plain(K, U);
-        smem_get<R, RECON>(smem, NL, 2 * m + 1, U);   // U_mu(x - mu)
+        smem_get<R, RECON, NTHR>(smem, NL, 2 * m + 1, U);   // U_mu(x - mu)
         if (GAUGE == GAUGE_MAG) { mag_acc_down<0>(M[0], U); mag_acc_down<1>(M[1], U); mag_acc_down<2>(M[2], U); }
         else acc_dagger(K, U);
     }
@@ -336,17 +359,21 @@ sweep_kernel(const SweepArgs args) {
     Mat<R> Gr;   // G in the storage type (MP: Step 2 in SP)
 #pragma unroll
     for (int k = 0; k < 18; ++k) Gr.v[k] = (R)G.v[k];
+    {
+        char* pu = up0;
+        char* pd = dn0;
 #pragma unroll 1
-    for (int m = 0; m < ND; ++m) {
-        const int mu = MU0 + m;
-        const int64_t cdn = (mu == 0) ? cbn0 : (mu == 1) ? cbn1 : (mu == 2) ? cbn2 : cbn3;
-        Mat<R> U, O;
-        smem_get<R, RECON>(smem, NL, 2 * m, U);
-        mul_left<NR>(Gr, U, O);
-        if (active) global_put<R, RECON>(args.links + L::link_offset(par, mu, Vh), Vh, cb, O);
-        smem_get<R, RECON>(smem, NL, 2 * m + 1, U);
-        mul_right_dagger<NR>(U, Gr, O);
-        if (active) global_put<R, RECON>(args.links + L::link_offset(1 - par, mu, Vh), Vh, cdn, O);
+        for (int m = 0; m < ND; ++m, pu += lstride, pd += lstride) {
+            const int mu = MU0 + m;
+            const int64_t cdn = (mu == 0) ? cbn0 : (mu == 1) ? cbn1 : (mu == 2) ? cbn2 : cbn3;
+            Mat<R> U, O;
+            smem_get<R, RECON, NTHR>(smem, NL, 2 * m, U);
+            mul_left<NR>(Gr, U, O);
+            if (active) global_put<R, RECON>(pu, Vh, cb, O);
+            smem_get<R, RECON, NTHR>(smem, NL, 2 * m + 1, U);
+            mul_right_dagger<NR>(U, Gr, O);
+            if (active) global_put<R, RECON>(pd, Vh, cdn, O);
+        }
     }
 
     // ---- a8: accumulate the transform, g_tot(x) <- G g_tot(x) ----

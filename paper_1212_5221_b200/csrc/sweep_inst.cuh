@@ -12,7 +12,8 @@ static cudaError_t launch_one(const SweepArgs& args, int block, cudaStream_t str
     auto kern = sweep_kernel<R, A, RECON, GAUGE, STOCH, TRACK, RED>;
     const int Vsh = args.Nx * args.Ny * (args.Nz / 2);
     block = sweep_block<R>(Vsh, block);
-    const size_t smem = (size_t)block * 2 * ND * Layout<R, RECON>::LINK_BYTES;
+    // the slice stride is the maximal CTA size whatever the block (sweep.cuh, smem_get)
+    const size_t smem = (size_t)SweepLaunch<R, A>::MAX_BLOCK * 2 * ND * Layout<R, RECON>::LINK_BYTES;
     static size_t smem_set = 0;   // per instantiation
     if (smem > smem_set) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
