@@ -74,6 +74,28 @@ int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int r
 int gf_destroy(gf_ctx* ctx);
 
 /*
+ * Batched gauge copies.  The paper's production use fixes many gauge copies
+ * of one configuration — "100 randomly chosen points on the gauge orbit" — and
+ * a 32^4 or smaller lattice does not fill a B200.  gf_create_batch makes a context that holds
+ * n_copies independent lattices of the same extents (contiguous in HBM, each in the layout of
+ * gf_create); every sweep / reduction / reunitarisation launch then covers all copies
+ * (grid.y = n_copies * Nt, so n_copies * Nt <= 65535).  Copy c draws its random numbers with the
+ * Philox key seed + c, so its trajectory is that of a single-lattice context run with seed + c.
+ * gf_create(...) == gf_create_batch(..., n_copies = 1, ...).
+ *
+ * On a batch context gf_set_links stores the same configuration into every copy; gf_sweep,
+ * gf_half_sweep, gf_anneal, gf_reunitarize, gf_coulomb_finalize and gf_random_gauge act on all copies;
+ * gf_get_links, gf_get_gauge_transform, gf_measure and gf_run need n_copies == 1 (else GF_ESTATE) —
+ * use the _copy / _batch forms below, which are valid for any n_copies.
+ */
+int gf_create_batch(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int n_copies, int precision, int recon,
+                    unsigned flags, void* cuda_stream);
+int gf_num_copies(const gf_ctx* ctx);
+int gf_set_links_copy(gf_ctx* ctx, int copy, const void* links, int elem_bytes, int is_device);
+int gf_get_links_copy(gf_ctx* ctx, int copy, void* links, int elem_bytes, int is_device);
+int gf_get_gauge_transform_copy(gf_ctx* ctx, int copy, void* g, int elem_bytes, int is_device);
+
+/*
  * gf_set_links / gf_get_links — copy a whole configuration in / out in StandardPattern.
  * links: host pointer (is_device = 0) or device pointer (is_device = 1) to Nt*Nx*Ny*Nz*4*18 reals of
  * elem_bytes = 4 (float) or 8 (double), independent of the context's precision (converted on the
@@ -112,6 +134,8 @@ int gf_half_sweep(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed,
  * (V -> Nx*Ny*Nz), the Coulomb stopping quantity.  Synchronous.
  */
 int gf_measure(gf_ctx* ctx, int gauge, double* F, double* theta, double* theta_slice);
+/* the same for every copy: F[n_copies], theta[n_copies], theta_slice NULL or [n_copies][Nt] */
+int gf_measure_batch(gf_ctx* ctx, int gauge, double* F, double* theta, double* theta_slice);
 
 typedef struct {
     int sweeps;   /* sweeps performed */
@@ -130,6 +154,16 @@ typedef struct {
  */
 int gf_run(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t first_sweep_index,
            int max_sweeps, double eps, int check_every, int reunit_every, gf_result* out, double* hist);
+/*
+ * gf_run_batch — gf_run for every copy of a batch context in the same launches.  Every copy is its own
+ * optimisation problem: copy c is no longer swept after the first check at which its stopping quantity
+ * is < eps (its CTAs exit at once), so out[c] (n_copies entries) is what gf_run returns for a
+ * single-lattice context holding copy c (seed + c).  hist: NULL or 3 * n_copies * (max_sweeps /
+ * check_every + 1) doubles, entry (check k, copy c) at hist[3 * (k * n_copies + c)]; a stopped copy
+ * repeats its final values.  GF_OK if every copy converged, else GF_NOT_CONVERGED.
+ */
+int gf_run_batch(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t first_sweep_index,
+                 int max_sweeps, double eps, int check_every, int reunit_every, gf_result* out, double* hist);
 
 /*
  * Per-slice Coulomb fixing (contexts created with GF_FLAG_FREEZE_SLICES).  In Coulomb gauge every
@@ -139,8 +173,9 @@ int gf_run(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32
  * once), so the result of slice t is that of a stand-alone run on that slice.  gf_run then returns
  * GF_OK when every slice has stopped; out->theta = max_t theta_t of the final links.  Reprojection
  * (reunit_every) still covers all links.  Landau/MAG runs ignore the flag.
- * gf_get_slice_sweeps: sweeps[Nt] (host) receives the number of sweeps applied to every slice by the
- * last gf_run (without the flag or for other gauges: that run's sweep count in every entry).
+ * gf_get_slice_sweeps: sweeps[n_copies * Nt] (host) receives the number of sweeps applied to every slice
+ * of every copy by the last gf_run / gf_run_batch (without the flag or for other gauges: the sweep count
+ * of the slice's copy in every entry).
  * GF_ESTATE before the first gf_run.
  */
 int gf_get_slice_sweeps(gf_ctx* ctx, int* sweeps);
@@ -153,6 +188,43 @@ int gf_get_slice_sweeps(gf_ctx* ctx, int* sweeps);
  */
 int gf_anneal(gf_ctx* ctx, int gauge, double T_hi, double T_lo, int n_steps, int n_micro, uint64_t seed,
               uint32_t first_sweep_index, uint32_t* next_sweep_index);
+
+/*
+ * gf_fix — the paper's production recipe as one call: (1) sa_steps steps of
+ * simulated annealing from sa_T_hi down to sa_T_lo (gf_anneal's schedule, sa_micro microcanonical sweeps
+ * after every heatbath sweep), (2) at most sr_max_sweeps sweeps of stochastic relaxation with probability
+ * sr_p, (3) overrelaxation with or_omega until theta < eps or or_max_sweeps.  A stage of length 0 is left
+ * out.  Stages (2) and (3) are gf_run_batch loops (checks every check_every sweeps; a copy that reaches
+ * theta < eps is stopped and takes no part in later stages); reunit_every > 0 reprojects after every
+ * reunit_every-th sweep of each stage.  Sweep indices run on from stage to stage starting at 0; copy c
+ * uses the Philox key seed + c.  out[n_copies]: total sweeps of all stages, F and the stopping quantity
+ * of the final links.  GF_OK if every copy converged, else GF_NOT_CONVERGED.  Synchronous.
+ */
+typedef struct {
+    int gauge;
+    uint64_t seed;
+    int sa_steps;
+    double sa_T_hi, sa_T_lo;
+    int sa_micro;
+    int sr_max_sweeps;
+    double sr_p;
+    double or_omega;
+    int or_max_sweeps;
+    double eps;
+    int check_every, reunit_every;
+} gf_fix_params;
+int gf_fix(gf_ctx* ctx, const gf_fix_params* params, gf_result* out);
+
+/*
+ * gf_random_gauge — a random start on the gauge orbit ("100 randomly chosen points on the
+ * gauge orbit", 580): every copy c is gauge transformed, U_mu(x) <- h(x) U_mu(x) h(x+mu)^dagger (Eq. (1),
+ * PAPER.md:25), with h(x) Haar distributed on SU(3): two rows of complex standard normals — Box-Muller on
+ * the Philox uniforms of counter (site, 0, k | 3 << 8, 0), k = 0,1,2, key seed + c: normals 4k..4k+3 =
+ * sqrt(-2 ln u0) (cos, sin)(2 pi u1), sqrt(-2 ln u2) (cos, sin)(2 pi u3) — orthonormalised by
+ * Gram-Schmidt, third row (u x v)^* (R27), all in double.  A tracked transform is updated,
+ * g(x) <- h(x) g(x).  Synchronous.
+ */
+int gf_random_gauge(gf_ctx* ctx, uint64_t seed);
 
 /*
  * gf_reunitarize — reproject every link (and the tracked transform) onto SU(3): Gram-Schmidt on rows

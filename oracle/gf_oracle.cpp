@@ -716,6 +716,28 @@ void gfo_apply_subgroup_d(double* mat18, const double* g4, int i, int j, int whi
     store<double>(mat18, U);
 }
 
+// Random start on the gauge orbit (reading R27): h(x) Haar on SU(3) from two rows of
+// complex standard normals, Box-Muller on the Philox uniforms of counter (site, 0, k | 3<<8, 0), k=0..2:
+// normals 4k..4k+3 = sqrt(-2 ln u0)(cos, sin)(2 pi u1), sqrt(-2 ln u2)(cos, sin)(2 pi u3); then the
+// Gram-Schmidt reprojection above.  h: [V][3][3][2] doubles in site order.
+void gfo_haar_field_d(double* h, const int* dims, uint64_t seed) {
+    const int64_t V = (int64_t)dims[0] * dims[1] * dims[2] * dims[3];
+    const double two_pi = 6.283185307179586477;
+    for (int64_t s = 0; s < V; ++s) {
+        double* p = h + s * 18;
+        for (int k = 0; k < 3; ++k) {
+            Philox4 w = draw(seed, (uint32_t)s, 0u, k, 3, 0u);
+            const double r0 = std::sqrt(-2.0 * std::log(u01(w.v[0]))), r1 = std::sqrt(-2.0 * std::log(u01(w.v[2])));
+            p[4 * k] = r0 * std::cos(two_pi * u01(w.v[1]));
+            p[4 * k + 1] = r0 * std::sin(two_pi * u01(w.v[1]));
+            p[4 * k + 2] = r1 * std::cos(two_pi * u01(w.v[3]));
+            p[4 * k + 3] = r1 * std::sin(two_pi * u01(w.v[3]));
+        }
+        for (int k = 12; k < 18; ++k) p[k] = 0.0;
+    }
+    reunitarize<double>(h, V);
+}
+
 int gfo_num_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

@@ -77,6 +77,8 @@ def lib():
         L.gfo_apply_subgroup_d.argtypes = [vp, vp, ci, ci, ci]
         L.gfo_apply_subgroup_d.restype = None
         L.gfo_num_threads.restype = ci
+        L.gfo_haar_field_d.argtypes = [vp, vp, u64]
+        L.gfo_haar_field_d.restype = None
         _lib = L
     return _lib
 
@@ -258,6 +260,80 @@ def anneal(links: np.ndarray, gauge: int, T_hi: float, T_lo: float, n_steps: int
             sweep(links, gauge, MICRO, 0.0, seed, idx, mixed, gtot)
             idx += 1
     return idx
+
+
+def haar_field(dims_txyz, seed: int) -> np.ndarray:
+    """h[t,x,y,z,3,3,2] (float64), Haar on SU(3) from Philox normals (R27)."""
+    d = np.array(dims_txyz, dtype=np.int32)
+    h = np.zeros(tuple(int(v) for v in d) + (3, 3, 2))
+    lib().gfo_haar_field_d(_p(h), _p(d), seed)
+    return h
+
+
+def gauge_transform(links: np.ndarray, h: np.ndarray) -> None:
+    """Eq. (1), PAPER.md:25, in place: U_mu(x) <- h(x) U_mu(x) h(x+mu)^dagger (computed in double)."""
+    U = links[..., 0].astype(np.float64) + 1j * links[..., 1].astype(np.float64)
+    H = h[..., 0].astype(np.float64) + 1j * h[..., 1].astype(np.float64)
+    for mu in range(4):
+        Hf = np.roll(H, -1, axis=mu)                      # h(x + mu)
+        U[..., mu, :, :] = np.einsum("...ab,...bc,...dc->...ad", H, U[..., mu, :, :], Hf.conj())
+    links[..., 0] = U.real
+    links[..., 1] = U.imag
+
+
+def random_gauge(links: np.ndarray, seed: int, gtot: np.ndarray | None = None) -> None:
+    """A random start on the gauge orbit: Haar h(x), Eq. (1); g(x) <- h(x) g(x)."""
+    h = haar_field(links.shape[:4], seed).astype(links.dtype)
+    gauge_transform(links, h)
+    if gtot is not None:
+        H = h[..., 0].astype(np.float64) + 1j * h[..., 1].astype(np.float64)
+        G = gtot[..., 0].astype(np.float64) + 1j * gtot[..., 1].astype(np.float64)
+        G = np.einsum("...ab,...bc->...ac", H, G)
+        gtot[..., 0] = G.real
+        gtot[..., 1] = G.imag
+
+
+def fix(links: np.ndarray, gauge: int, seed: int = 0, sa_steps: int = 0, sa_T_hi: float = 1.0, sa_T_lo: float = 0.01,
+        sa_micro: int = 3, sr_max_sweeps: int = 0, sr_p: float = 0.5, or_omega: float = 1.7, or_max_sweeps: int = 1000,
+        eps: float = 1e-12, check_every: int = 1, reunit_every: int = 0, mixed: bool = False,
+        gtot: np.ndarray | None = None):
+    """The production recipe of PAPER.md:556 / 580-582: simulated annealing (with microcanonical sweeps),
+    then at most sr_max_sweeps stochastic-relaxation sweeps, then overrelaxation until theta < eps.  A stage
+    of length 0 is left out; a stage is not entered once theta < eps was reached.  Sweep indices run on from
+    stage to stage; reprojection every reunit_every sweeps of each stage.
+    Returns (total sweeps, F, theta, converged)."""
+    idx = 0
+    total = 0
+    conv = False
+    m = None
+    if sa_steps > 0:
+        done = 0
+        for k in range(sa_steps):
+            T = temperature(k, sa_steps, sa_T_hi, sa_T_lo)
+            for algo, par in [(SA, T)] + [(MICRO, 0.0)] * sa_micro:
+                sweep(links, gauge, algo, par, seed, idx, mixed, gtot)
+                idx += 1
+                done += 1
+                if reunit_every and done % reunit_every == 0:
+                    reunitarize(links)
+                    if gtot is not None:
+                        reunitarize(gtot)
+        total += idx
+    if sr_max_sweeps > 0:
+        s, F, th, _, conv = run(links, gauge, SR, sr_p, seed, sr_max_sweeps, eps, check_every, reunit_every, mixed,
+                                gtot, idx)
+        total += s
+        m = (F, th)
+    if or_max_sweeps > 0 and not conv:
+        s, F, th, _, conv = run(links, gauge, OR, or_omega, seed, or_max_sweeps, eps, check_every, reunit_every,
+                                mixed, gtot, idx)
+        total += s
+        m = (F, th)
+    if m is None:
+        mm = measure(links, gauge)
+        m = (mm["F"], stop_value(mm, gauge))
+        conv = m[1] < eps
+    return total, m[0], m[1], conv
 
 
 def site_update(up: np.ndarray, dn: np.ndarray, gauge: int, algo: int, param: float, seed: int = 0,

@@ -15,6 +15,7 @@ namespace gf {
 struct Dims {
     int Nt, Nx, Ny, Nz;
 };
+GF_DEV int64_t Vh_of(const Dims& d) { return (int64_t)d.Nt * d.Nx * d.Ny * d.Nz / 2; }
 
 // lexicographic site index s = ((t*Nx + x)*Ny + y)*Nz + z  ->  parity, checkerboard index
 GF_DEV void site_to_cb(const Dims& d, int64_t s, int& par, int& cb) {
@@ -115,10 +116,12 @@ GF_DEV void gram_schmidt(Mat<double>& m) {
 }
 
 // nmats matrices stored as planes [slot][chunk][cb] with `slot_bytes` = RECON*sizeof(R)*Vh between slots
+// blockIdx.y = gauge copy, copy_bytes apart
 template <class R, int RECON>
-__global__ void reunit_kernel(char* base, int64_t Vh, int nslots) {
+__global__ void reunit_kernel(char* base, int64_t Vh, int nslots, int64_t copy_bytes) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= (int64_t)nslots * Vh) return;
+    base += blockIdx.y * copy_bytes;
     const int slot = (int)(i / Vh);
     const int cb = (int)(i % Vh);
     char* p0 = base + (int64_t)slot * Layout<R, RECON>::LINK_BYTES * Vh;
@@ -134,8 +137,8 @@ __global__ void reunit_kernel(char* base, int64_t Vh, int nslots) {
 }
 
 // ---- F and theta ---------------------------------------------------------------------------
-// grid = (ceil(Vsh / block), Nt, 2): one thread per site of parity blockIdx.z in time-slice
-// blockIdx.y.  Each block writes one (F-term, theta-term) pair; slice_reduce_kernel sums them in a
+// grid = (ceil(Vsh / block), ncopies*Nt, 2): one thread per site of parity blockIdx.z in (gauge copy,
+// time-slice) blockIdx.y.  Each block writes one (F-term, theta-term) pair; slice_reduce_kernel sums them in a
 // fixed order, so results are bit-reproducible.  All arithmetic in double (BASELINE.json).
 GF_DEV double warp_sum(double v) {
 #pragma unroll
@@ -158,13 +161,15 @@ GF_DEV void block_sum2(double& a, double& b) {
 }
 
 template <class R, int RECON, int GAUGE>
-__global__ void measure_kernel(const char* links, Dims d, double* partial) {
+__global__ void measure_kernel(const char* links, Dims d, double* partial, int64_t copy_bytes) {
     typedef Layout<R, RECON> L;
     constexpr int MU0 = (GAUGE == GAUGE_COULOMB) ? 1 : 0;
     const int Nzh = d.Nz >> 1;
     const int Vsh = d.Nx * d.Ny * Nzh;
     const int64_t Vh = (int64_t)d.Nt * Vsh;
-    const int t = blockIdx.y, par = blockIdx.z;
+    const int copy = blockIdx.y / d.Nt;
+    const int t = blockIdx.y - copy * d.Nt, par = blockIdx.z;
+    links += copy * copy_bytes;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     double f_term = 0.0, th_term = 0.0;
     if (i < Vsh) {
@@ -227,13 +232,13 @@ __global__ void measure_kernel(const char* links, Dims d, double* partial) {
     }
     block_sum2(f_term, th_term);
     if (threadIdx.x == 0) {
-        const int64_t b = ((int64_t)(t * 2 + par)) * gridDim.x + blockIdx.x;
+        const int64_t b = ((int64_t)(blockIdx.y * 2 + par)) * gridDim.x + blockIdx.x;
         partial[2 * b] = f_term;
         partial[2 * b + 1] = th_term;
     }
 }
 
-// one block per time-slice: out[t] = sum of F terms, out[Nt + t] = sum of theta terms
+// one block per (copy, time-slice) (Nt here = ncopies*Nt): out[t] = sum of F terms, out[Nt + t] = sum of theta terms
 __global__ void slice_reduce_kernel(const double* partial, int blocks_per_slice, int Nt, double* out) {
     const int t = blockIdx.x;
     double a = 0.0, b = 0.0;
@@ -263,7 +268,11 @@ __global__ void red_reduce_kernel(const double* partial, int gx, double* out) {
 
 // ---- Coulomb finalisation: U_0(x) <- R(x) U_0(x) R(x+t)^dag, R = g_tot g_applied^dag -----------
 template <class R, int RECON>
-__global__ void coulomb_finalize_kernel(char* links, const char* gtot, const char* gapp, Dims d) {
+__global__ void coulomb_finalize_kernel(char* links, const char* gtot, const char* gapp, Dims d,
+                                        int64_t copy_links_bytes, int64_t copy_field_bytes) {
+    links += blockIdx.y * copy_links_bytes;   // blockIdx.y = gauge copy
+    gtot += blockIdx.y * copy_field_bytes;
+    if (gapp) gapp += blockIdx.y * copy_field_bytes;
     const int Nzh = d.Nz >> 1;
     const int Vsh = d.Nx * d.Ny * Nzh;
     const int64_t Vh = (int64_t)d.Nt * Vsh;
@@ -288,6 +297,82 @@ __global__ void coulomb_finalize_kernel(char* links, const char* gtot, const cha
     mul_left<3>(Ga, U, T);
     mul_right_dagger<3>(T, Gb, O);
     global_put<R, RECON>(p0, Vh, cb, O);
+}
+
+// ---- random start on the gauge orbit (R27) ------------------------
+// h(x) Haar-distributed on SU(3): two rows of independent complex standard normals (Box-Muller on
+// Philox uniforms, counter = (site, 0, k | 3 << 8, 0), k = 0..2, key = seed + copy), Gram-Schmidt,
+// third row (u x v)^*.  All in double.  One thread per site; field layout [copy][p][chunk][cb].
+template <class R>
+__global__ void haar_field_kernel(char* field, Dims d, uint64_t seed, int64_t copy_bytes) {
+    const int64_t V = (int64_t)d.Nt * d.Nx * d.Ny * d.Nz;
+    const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= V) return;
+    const int copy = blockIdx.y;
+    int par, cb;
+    site_to_cb(d, s, par, cb);
+    Mat<double> h;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const u32x4 w = rng_draw(seed + (uint64_t)copy, (uint32_t)s, 0u, k, 3, 0u);
+        const double r0 = sqrt(-2.0 * log(uniform01(w.x))), r1 = sqrt(-2.0 * log(uniform01(w.z)));
+        double s0, c0, s1, c1;
+        sincos(6.283185307179586477 * uniform01(w.y), &s0, &c0);
+        sincos(6.283185307179586477 * uniform01(w.w), &s1, &c1);
+        h.v[4 * k] = r0 * c0; h.v[4 * k + 1] = r0 * s0; h.v[4 * k + 2] = r1 * c1; h.v[4 * k + 3] = r1 * s1;
+    }
+#pragma unroll
+    for (int k = 12; k < 18; ++k) h.v[k] = 0.0;
+    gram_schmidt(h);
+    Mat<R> o;
+#pragma unroll
+    for (int k = 0; k < 18; ++k) o.v[k] = (R)h.v[k];
+    global_put<R, 18>(field + copy * copy_bytes + Layout<R, 18>::site_offset(par, Vh_of(d)), Vh_of(d), cb, o);
+}
+
+// U_mu(x) <- h(x) U_mu(x) h(x+mu)^dagger (Eq. (1)) and, when tracked, g(x) <- h(x) g(x).
+// One thread per site (parity blockIdx.z, copy blockIdx.y).
+template <class R, int RECON>
+__global__ void gauge_apply_kernel(char* links, char* gtot, const char* hfield, Dims d, int64_t copy_links_bytes,
+                                   int64_t copy_field_bytes) {
+    typedef Layout<R, RECON> L;
+    const int Nzh = d.Nz >> 1;
+    const int Vsh = d.Nx * d.Ny * Nzh;
+    const int64_t Vh = (int64_t)d.Nt * Vsh;
+    const int64_t cb = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (cb >= Vh) return;
+    const int par = blockIdx.z;
+    links += blockIdx.y * copy_links_bytes;
+    hfield += blockIdx.y * copy_field_bytes;
+    int64_t rem = cb;
+    const int zh = (int)(rem % Nzh); rem /= Nzh;
+    const int y = (int)(rem % d.Ny); rem /= d.Ny;
+    const int x = (int)(rem % d.Nx);
+    const int t = (int)(rem / d.Nx);
+    const int r = (t + x + y + par) & 1;   // z = 2 zh + r
+    // checkerboard index of x + mu (other parity)
+    int64_t cbf[4];
+    cbf[0] = cb + ((t == d.Nt - 1) ? -(int64_t)(d.Nt - 1) * Vsh : (int64_t)Vsh);
+    cbf[1] = cb + ((x == d.Nx - 1) ? -(d.Nx - 1) * Nzh * d.Ny : Nzh * d.Ny);
+    cbf[2] = cb + ((y == d.Ny - 1) ? -(d.Ny - 1) * Nzh : Nzh);
+    cbf[3] = r ? ((zh == Nzh - 1) ? cb - (Nzh - 1) : cb + 1) : cb;
+    Mat<R> h, hf, U, T, O;
+    global_get<R, 18>(hfield + Layout<R, 18>::site_offset(par, Vh), Vh, cb, h);
+#pragma unroll 1
+    for (int mu = 0; mu < 4; ++mu) {
+        global_get<R, 18>(hfield + Layout<R, 18>::site_offset(1 - par, Vh), Vh, cbf[mu], hf);
+        char* p0 = links + L::link_offset(par, mu, Vh);
+        global_get<R, RECON>(p0, Vh, cb, U);
+        mul_left<3>(h, U, T);
+        mul_right_dagger<3>(T, hf, O);
+        global_put<R, RECON>(p0, Vh, cb, O);
+    }
+    if (gtot) {
+        char* g0 = gtot + blockIdx.y * copy_field_bytes + Layout<R, 18>::site_offset(par, Vh);
+        global_get<R, 18>(g0, Vh, cb, U);
+        mul_left<3>(h, U, O);
+        global_put<R, 18>(g0, Vh, cb, O);
+    }
 }
 
 }  // namespace gf

@@ -28,6 +28,8 @@ extern template cudaError_t launch_sweep<double, double, 12>(const SweepArgs&, i
 
 struct gf_ctx {
     int Nx, Ny, Nz, Nt;
+    int B;                  // gauge copies held by this context (gf_create_batch), 1 for gf_create
+    int NS;                 // B * Nt: (copy, time-slice) pairs = grid.y of the per-site kernels
     int precision, recon;
     unsigned flags;
     cudaStream_t stream;
@@ -36,7 +38,8 @@ struct gf_ctx {
     char* links;            // device link store
     char* gtot;             // tracked transform (18 reals/site) or nullptr
     char* gapplied;         // part of gtot already applied to the temporal links (Coulomb) or nullptr
-    bool have_links;
+    bool have_links;        // every copy has received links
+    std::vector<unsigned char> copies_set;
     bool temporal_stale;    // Coulomb sweeps ran since the temporal links were last finalised
     // reductions
     double* partial;        // per-block partial sums
@@ -52,6 +55,7 @@ struct gf_ctx {
     unsigned char* skip_dev;    // [Nt] 1 = slice stopped, its CTAs exit at once
     unsigned char* skip_host;   // pinned copy
     std::vector<int> slice_sweeps;   // sweeps applied to every slice by the last gf_run
+    std::vector<unsigned char> slice_frozen;   // slices of the units the last run stopped (converged)
     bool have_slice_sweeps;
     // host<->device staging for gf_set_links / gf_get_*
     void* staging;
@@ -87,6 +91,7 @@ static Dims dims_of(const gf_ctx* c) {
     Dims d = {c->Nt, c->Nx, c->Ny, c->Nz};
     return d;
 }
+// bytes of ONE gauge copy; the B copies of a context are contiguous
 static int64_t link_store_bytes(const gf_ctx* c) { return (int64_t)8 * c->recon * c->real_bytes * c->Vh; }
 static int64_t field_store_bytes(const gf_ctx* c) { return (int64_t)2 * 18 * c->real_bytes * c->Vh; }
 
@@ -114,8 +119,14 @@ int64_t gf_volume(const gf_ctx* ctx) { return ctx ? ctx->V : 0; }
 
 int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int recon, unsigned flags,
               void* cuda_stream) {
+    return gf_create_batch(out, Nx, Ny, Nz, Nt, 1, precision, recon, flags, cuda_stream);
+}
+
+int gf_create_batch(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int n_copies, int precision, int recon,
+                    unsigned flags, void* cuda_stream) {
     if (!out) return GF_EINVAL;
     *out = nullptr;
+    if (n_copies < 1 || (int64_t)n_copies * Nt > 65535) return GF_EINVAL;   // grid.y = n_copies * Nt
     const int n[4] = {Nx, Ny, Nz, Nt};
     for (int k = 0; k < 4; ++k)
         if (n[k] < 2 || (n[k] & 1)) return GF_EINVAL;
@@ -128,6 +139,8 @@ int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int r
     gf_ctx* ctx = new (std::nothrow) gf_ctx();
     if (!ctx) return GF_ENOMEM;
     ctx->Nx = Nx; ctx->Ny = Ny; ctx->Nz = Nz; ctx->Nt = Nt;
+    ctx->B = n_copies; ctx->NS = n_copies * Nt;
+    ctx->copies_set.assign((size_t)n_copies, 0);
     ctx->precision = precision; ctx->recon = recon; ctx->flags = flags;
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->V = (int64_t)Nx * Ny * Nz * Nt;
@@ -144,33 +157,34 @@ int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int r
     ctx->timing = false; ctx->ev_used = 0; ctx->launches = 0;
     ctx->err[0] = 0;
 
-    cudaError_t e = cudaMalloc((void**)&ctx->links, (size_t)link_store_bytes(ctx));
-    if (e == cudaSuccess) ctx->device_bytes += link_store_bytes(ctx);
+    const int B = n_copies, NS = n_copies * Nt;
+    cudaError_t e = cudaMalloc((void**)&ctx->links, (size_t)(B * link_store_bytes(ctx)));
+    if (e == cudaSuccess) ctx->device_bytes += B * link_store_bytes(ctx);
     if (e == cudaSuccess && (flags & GF_FLAG_TRACK_TRANSFORM)) {
-        e = cudaMalloc((void**)&ctx->gtot, (size_t)field_store_bytes(ctx));
-        if (e == cudaSuccess) ctx->device_bytes += field_store_bytes(ctx);
+        e = cudaMalloc((void**)&ctx->gtot, (size_t)(B * field_store_bytes(ctx)));
+        if (e == cudaSuccess) ctx->device_bytes += B * field_store_bytes(ctx);
     }
     ctx->meas_block = 128;
     const int Vsh = Nx * Ny * (Nz / 2);
     ctx->meas_gx = (Vsh + ctx->meas_block - 1) / ctx->meas_block;
-    const size_t npart = (size_t)ctx->meas_gx * Nt * 2;
+    const size_t npart = (size_t)ctx->meas_gx * NS * 2;
     if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->partial, npart * 2 * sizeof(double));
-    if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->slice_dev, (size_t)2 * Nt * sizeof(double));
-    if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->slice_host, (size_t)2 * Nt * sizeof(double));
-    const size_t nred = (size_t)((Vsh + 31) / 32) * Nt * 3;   // smallest CTA = 32 sites
+    if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->slice_dev, (size_t)2 * NS * sizeof(double));
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->slice_host, (size_t)2 * NS * sizeof(double));
+    const size_t nred = (size_t)((Vsh + 31) / 32) * NS * 3;   // smallest CTA = 32 sites
     for (int k = 0; k < 2; ++k)
         if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->red_part[k], nred * sizeof(double));
-    if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->red_dev, (size_t)6 * Nt * sizeof(double));
-    if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->red_host, (size_t)6 * Nt * sizeof(double));
-    if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->skip_dev, (size_t)Nt);
-    if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->skip_host, (size_t)Nt);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->red_dev, (size_t)6 * NS * sizeof(double));
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->red_host, (size_t)6 * NS * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->skip_dev, (size_t)NS);
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->skip_host, (size_t)NS);
     if (e != cudaSuccess) {
         const int code = (e == cudaErrorMemoryAllocation) ? GF_ENOMEM : GF_ECUDA;
         gf_destroy(ctx);
         cudaGetLastError();
         return code;
     }
-    ctx->device_bytes += (int64_t)(npart * 2 + 2 * Nt + 2 * nred + 6 * Nt) * sizeof(double);
+    ctx->device_bytes += (int64_t)(npart * 2 + 2 * NS + 2 * nred + 6 * NS) * sizeof(double);
     *out = ctx;
     return GF_OK;
 }
@@ -220,32 +234,62 @@ static const int64_t STAGE_SITES = 1 << 18;   // sites per host<->device staging
 
 #define CONVERT_IN(R, RECON, E, src, s0, ns)                                                            \
     convert_in_kernel<E, R, RECON><<<(unsigned)(((ns) * 4 + 255) / 256), 256, 0, ctx->stream>>>(        \
-        (const E*)(src), ctx->links, dims_of(ctx), (s0), (ns))
+        (const E*)(src), lbase, dims_of(ctx), (s0), (ns))
 #define CONVERT_OUT(R, RECON, E, dst, s0, ns)                                                           \
     convert_out_kernel<E, R, RECON><<<(unsigned)(((ns) * 4 + 255) / 256), 256, 0, ctx->stream>>>(       \
-        (E*)(dst), ctx->links, dims_of(ctx), (s0), (ns))
+        (E*)(dst), lbase, dims_of(ctx), (s0), (ns))
 
-static int reset_transform(gf_ctx* ctx) {
-    if (ctx->gtot) {
-        const unsigned g = (unsigned)((2 * ctx->Vh + 255) / 256);
-        if (ctx->real_bytes == 4) field_identity_kernel<float><<<g, 256, 0, ctx->stream>>>(ctx->gtot, ctx->Vh);
-        else field_identity_kernel<double><<<g, 256, 0, ctx->stream>>>(ctx->gtot, ctx->Vh);
-        CU(cudaGetLastError());
-        ++ctx->launches;
-    }
-    if (ctx->gapplied) {
-        CU(cudaStreamSynchronize(ctx->stream));
-        cudaFree(ctx->gapplied);
-        ctx->gapplied = nullptr;
-        ctx->device_bytes -= field_store_bytes(ctx);
-    }
-    ctx->temporal_stale = false;
+static int field_identity(gf_ctx* ctx, char* field) {
+    const unsigned g = (unsigned)((2 * ctx->Vh + 255) / 256);
+    if (ctx->real_bytes == 4) field_identity_kernel<float><<<g, 256, 0, ctx->stream>>>(field, ctx->Vh);
+    else field_identity_kernel<double><<<g, 256, 0, ctx->stream>>>(field, ctx->Vh);
+    CU(cudaGetLastError());
+    ++ctx->launches;
     return GF_OK;
 }
 
-int gf_set_links(gf_ctx* ctx, const void* links, int elem_bytes, int is_device) {
+// the accumulated transform of `copy` restarts at the identity (new links were just stored)
+static int reset_transform(gf_ctx* ctx, int copy) {
+    if (ctx->gtot) {
+        int rc = field_identity(ctx, ctx->gtot + copy * field_store_bytes(ctx));
+        if (rc) return rc;
+    }
+    if (ctx->gapplied) {
+        if (ctx->B == 1) {
+            CU(cudaStreamSynchronize(ctx->stream));
+            cudaFree(ctx->gapplied);
+            ctx->gapplied = nullptr;
+            ctx->device_bytes -= field_store_bytes(ctx);
+        } else {
+            int rc = field_identity(ctx, ctx->gapplied + copy * field_store_bytes(ctx));
+            if (rc) return rc;
+        }
+    }
+    if (ctx->B == 1) ctx->temporal_stale = false;
+    return GF_OK;
+}
+
+static int check_copy(gf_ctx* ctx, int copy, const char* who) {
+    if (copy < 0 || copy >= ctx->B) return fail(ctx, GF_EINVAL, "%s: copy %d not in [0, %d)", who, copy, ctx->B);
+    return GF_OK;
+}
+static int single_only(gf_ctx* ctx, const char* who) {
+    if (ctx->B != 1) return fail(ctx, GF_ESTATE, "%s: context holds %d gauge copies, use the _copy / _batch call", who, ctx->B);
+    return GF_OK;
+}
+
+int gf_num_copies(const gf_ctx* ctx) { return ctx ? ctx->B : 0; }
+
+int gf_set_links_copy(gf_ctx* ctx, int copy, const void* links, int elem_bytes, int is_device) {
     if (!ctx) return GF_EINVAL;
     if (!links || (elem_bytes != 4 && elem_bytes != 8)) return fail(ctx, GF_EINVAL, "gf_set_links: bad arguments");
+    int rc = check_copy(ctx, copy, "gf_set_links_copy");
+    if (rc) return rc;
+    if (ctx->B > 1 && ctx->temporal_stale && ctx->gtot) {   // the other copies keep their pending finalisation
+        rc = gf_coulomb_finalize(ctx);
+        if (rc) return rc;
+    }
+    char* lbase = ctx->links + copy * link_store_bytes(ctx);
     const int64_t link_elems = 4 * 18;
     if (is_device) {
         if (elem_bytes == 4) DISPATCH_RR(ctx, CONVERT_IN, float, links, (int64_t)0, ctx->V);
@@ -254,7 +298,7 @@ int gf_set_links(gf_ctx* ctx, const void* links, int elem_bytes, int is_device) 
         ++ctx->launches;
     } else {
         const int64_t chunk = ctx->V < STAGE_SITES ? ctx->V : STAGE_SITES;
-        int rc = ensure_staging(ctx, (size_t)(chunk * link_elems * elem_bytes));
+        rc = ensure_staging(ctx, (size_t)(chunk * link_elems * elem_bytes));
         if (rc) return rc;
         for (int64_t s0 = 0; s0 < ctx->V; s0 += chunk) {
             const int64_t ns = (ctx->V - s0 < chunk) ? ctx->V - s0 : chunk;
@@ -267,21 +311,43 @@ int gf_set_links(gf_ctx* ctx, const void* links, int elem_bytes, int is_device) 
             ++ctx->launches;
         }
     }
-    int rc = reset_transform(ctx);
+    rc = reset_transform(ctx, copy);
     if (rc) return rc;
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->copies_set[(size_t)copy] = 1;
+    ctx->have_links = true;
+    for (int c = 0; c < ctx->B; ++c) ctx->have_links = ctx->have_links && ctx->copies_set[(size_t)c];
+    return GF_OK;
+}
+
+// every copy of the context receives the same configuration
+int gf_set_links(gf_ctx* ctx, const void* links, int elem_bytes, int is_device) {
+    if (!ctx) return GF_EINVAL;
+    int rc = gf_set_links_copy(ctx, 0, links, elem_bytes, is_device);
+    if (rc) return rc;
+    for (int c = 1; c < ctx->B; ++c) {
+        CU(cudaMemcpyAsync(ctx->links + c * link_store_bytes(ctx), ctx->links, (size_t)link_store_bytes(ctx),
+                           cudaMemcpyDeviceToDevice, ctx->stream));
+        rc = reset_transform(ctx, c);
+        if (rc) return rc;
+        ctx->copies_set[(size_t)c] = 1;
+    }
     CU(cudaStreamSynchronize(ctx->stream));
     ctx->have_links = true;
     return GF_OK;
 }
 
-int gf_get_links(gf_ctx* ctx, void* links, int elem_bytes, int is_device) {
+int gf_get_links_copy(gf_ctx* ctx, int copy, void* links, int elem_bytes, int is_device) {
     if (!ctx) return GF_EINVAL;
     if (!links || (elem_bytes != 4 && elem_bytes != 8)) return fail(ctx, GF_EINVAL, "gf_get_links: bad arguments");
+    int rc = check_copy(ctx, copy, "gf_get_links_copy");
+    if (rc) return rc;
     if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_get_links: no links set");
     if (ctx->temporal_stale && ctx->gtot) {
-        int rc = gf_coulomb_finalize(ctx);
+        rc = gf_coulomb_finalize(ctx);
         if (rc) return rc;
     }
+    const char* lbase = ctx->links + copy * link_store_bytes(ctx);
     const int64_t link_elems = 4 * 18;
     if (is_device) {
         if (elem_bytes == 4) DISPATCH_RR(ctx, CONVERT_OUT, float, links, (int64_t)0, ctx->V);
@@ -290,7 +356,7 @@ int gf_get_links(gf_ctx* ctx, void* links, int elem_bytes, int is_device) {
         ++ctx->launches;
     } else {
         const int64_t chunk = ctx->V < STAGE_SITES ? ctx->V : STAGE_SITES;
-        int rc = ensure_staging(ctx, (size_t)(chunk * link_elems * elem_bytes));
+        rc = ensure_staging(ctx, (size_t)(chunk * link_elems * elem_bytes));
         if (rc) return rc;
         for (int64_t s0 = 0; s0 < ctx->V; s0 += chunk) {
             const int64_t ns = (ctx->V - s0 < chunk) ? ctx->V - s0 : chunk;
@@ -307,13 +373,23 @@ int gf_get_links(gf_ctx* ctx, void* links, int elem_bytes, int is_device) {
     return GF_OK;
 }
 
-int gf_get_gauge_transform(gf_ctx* ctx, void* g, int elem_bytes, int is_device) {
+int gf_get_links(gf_ctx* ctx, void* links, int elem_bytes, int is_device) {
+    if (!ctx) return GF_EINVAL;
+    int rc = single_only(ctx, "gf_get_links");
+    if (rc) return rc;
+    return gf_get_links_copy(ctx, 0, links, elem_bytes, is_device);
+}
+
+int gf_get_gauge_transform_copy(gf_ctx* ctx, int copy, void* g, int elem_bytes, int is_device) {
     if (!ctx) return GF_EINVAL;
     if (!g || (elem_bytes != 4 && elem_bytes != 8)) return fail(ctx, GF_EINVAL, "gf_get_gauge_transform: bad arguments");
+    int rc = check_copy(ctx, copy, "gf_get_gauge_transform_copy");
+    if (rc) return rc;
     if (!ctx->gtot) return fail(ctx, GF_ESTATE, "gf_get_gauge_transform: context created without GF_FLAG_TRACK_TRANSFORM");
+    const char* fbase = ctx->gtot + copy * field_store_bytes(ctx);
     const int64_t chunk = is_device ? ctx->V : (ctx->V < 4 * STAGE_SITES ? ctx->V : 4 * STAGE_SITES);
     if (!is_device) {
-        int rc = ensure_staging(ctx, (size_t)(chunk * 18 * elem_bytes));
+        rc = ensure_staging(ctx, (size_t)(chunk * 18 * elem_bytes));
         if (rc) return rc;
     }
     for (int64_t s0 = 0; s0 < ctx->V; s0 += chunk) {
@@ -321,11 +397,11 @@ int gf_get_gauge_transform(gf_ctx* ctx, void* g, int elem_bytes, int is_device) 
         void* dst = is_device ? (void*)((char*)g + s0 * 18 * elem_bytes) : ctx->staging;
         const unsigned grid = (unsigned)((ns + 255) / 256);
         if (ctx->real_bytes == 4) {
-            if (elem_bytes == 4) field_out_kernel<float, float><<<grid, 256, 0, ctx->stream>>>((float*)dst, ctx->gtot, dims_of(ctx), s0, ns);
-            else field_out_kernel<double, float><<<grid, 256, 0, ctx->stream>>>((double*)dst, ctx->gtot, dims_of(ctx), s0, ns);
+            if (elem_bytes == 4) field_out_kernel<float, float><<<grid, 256, 0, ctx->stream>>>((float*)dst, fbase, dims_of(ctx), s0, ns);
+            else field_out_kernel<double, float><<<grid, 256, 0, ctx->stream>>>((double*)dst, fbase, dims_of(ctx), s0, ns);
         } else {
-            if (elem_bytes == 4) field_out_kernel<float, double><<<grid, 256, 0, ctx->stream>>>((float*)dst, ctx->gtot, dims_of(ctx), s0, ns);
-            else field_out_kernel<double, double><<<grid, 256, 0, ctx->stream>>>((double*)dst, ctx->gtot, dims_of(ctx), s0, ns);
+            if (elem_bytes == 4) field_out_kernel<float, double><<<grid, 256, 0, ctx->stream>>>((float*)dst, fbase, dims_of(ctx), s0, ns);
+            else field_out_kernel<double, double><<<grid, 256, 0, ctx->stream>>>((double*)dst, fbase, dims_of(ctx), s0, ns);
         }
         CU(cudaGetLastError());
         ++ctx->launches;
@@ -335,6 +411,13 @@ int gf_get_gauge_transform(gf_ctx* ctx, void* g, int elem_bytes, int is_device) 
     }
     CU(cudaStreamSynchronize(ctx->stream));
     return GF_OK;
+}
+
+int gf_get_gauge_transform(gf_ctx* ctx, void* g, int elem_bytes, int is_device) {
+    if (!ctx) return GF_EINVAL;
+    int rc = single_only(ctx, "gf_get_gauge_transform");
+    if (rc) return rc;
+    return gf_get_gauge_transform_copy(ctx, 0, g, elem_bytes, is_device);
 }
 
 // ---- sweeps ----------------------------------------------------------------------------------
@@ -357,6 +440,9 @@ static int launch_half(gf_ctx* ctx, int gauge, int algo, double param, uint64_t 
     a.parity = parity; a.algo = algo; a.param = param; a.seed = seed; a.sweep_index = sweep_index;
     a.red = red;
     a.slice_skip = skip;
+    a.ncopies = ctx->B;
+    a.copy_links_bytes = link_store_bytes(ctx);
+    a.copy_gtot_bytes = field_store_bytes(ctx);
     const bool track = ctx->gtot != nullptr;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (ctx->timing) {
@@ -421,37 +507,40 @@ int gf_sweep(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint
 // ---- reductions --------------------------------------------------------------------------------
 #define MEASURE(R, RECON, gauge_)                                                                          \
     do {                                                                                                   \
-        dim3 grid((unsigned)ctx->meas_gx, (unsigned)ctx->Nt, 2);                                           \
+        dim3 grid((unsigned)ctx->meas_gx, (unsigned)ctx->NS, 2);                                           \
+        const int64_t cb_ = link_store_bytes(ctx);                                                         \
         if ((gauge_) == GF_LANDAU)                                                                         \
-            measure_kernel<R, RECON, GAUGE_LANDAU><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial); \
+            measure_kernel<R, RECON, GAUGE_LANDAU><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_); \
         else if ((gauge_) == GF_COULOMB)                                                                   \
-            measure_kernel<R, RECON, GAUGE_COULOMB><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial); \
+            measure_kernel<R, RECON, GAUGE_COULOMB><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_); \
         else                                                                                               \
-            measure_kernel<R, RECON, GAUGE_MAG><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial); \
+            measure_kernel<R, RECON, GAUGE_MAG><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_); \
     } while (0)
 
 // enqueue the reduction and the copy of the 2*Nt slice sums to pinned host memory
 static int enqueue_measure(gf_ctx* ctx, int gauge) {
     DISPATCH_RR(ctx, MEASURE, gauge);
     CU(cudaGetLastError());
-    slice_reduce_kernel<<<ctx->Nt, 128, 0, ctx->stream>>>(ctx->partial, 2 * ctx->meas_gx, ctx->Nt, ctx->slice_dev);
+    slice_reduce_kernel<<<ctx->NS, 128, 0, ctx->stream>>>(ctx->partial, 2 * ctx->meas_gx, ctx->NS, ctx->slice_dev);
     CU(cudaGetLastError());
     ctx->launches += 2;
-    CU(cudaMemcpyAsync(ctx->slice_host, ctx->slice_dev, (size_t)2 * ctx->Nt * sizeof(double), cudaMemcpyDeviceToHost,
+    CU(cudaMemcpyAsync(ctx->slice_host, ctx->slice_dev, (size_t)2 * ctx->NS * sizeof(double), cudaMemcpyDeviceToHost,
                        ctx->stream));
     return GF_OK;
 }
 
-// after a stream sync: normalise (Eqs. (4), (7), (11)) in a fixed order
-static void finish_measure(const gf_ctx* ctx, int gauge, double* F, double* theta, double* theta_slice,
+// after a stream sync: normalise (Eqs. (4), (7), (11)) the slice sums of gauge copy c in a fixed order
+static void finish_measure(const gf_ctx* ctx, int gauge, int c, double* F, double* theta, double* theta_slice,
                            double* theta_max) {
     const int nd = (gauge == GF_COULOMB) ? 3 : 4;
     const double Vs = (double)ctx->Nx * ctx->Ny * ctx->Nz;
+    const double* fs_ = ctx->slice_host + (size_t)c * ctx->Nt;
+    const double* th_ = ctx->slice_host + (size_t)ctx->NS + (size_t)c * ctx->Nt;
     double fs = 0.0, ths = 0.0, tmax = 0.0;
     for (int t = 0; t < ctx->Nt; ++t) {
-        fs += ctx->slice_host[t];
-        ths += ctx->slice_host[ctx->Nt + t];
-        const double th_t = ctx->slice_host[ctx->Nt + t] / (3.0 * Vs);
+        fs += fs_[t];
+        ths += th_[t];
+        const double th_t = th_[t] / (3.0 * Vs);
         if (theta_slice) theta_slice[t] = th_t;
         if (th_t > tmax) tmax = th_t;
     }
@@ -460,7 +549,7 @@ static void finish_measure(const gf_ctx* ctx, int gauge, double* F, double* thet
     if (theta_max) *theta_max = tmax;
 }
 
-int gf_measure(gf_ctx* ctx, int gauge, double* F, double* theta, double* theta_slice) {
+int gf_measure_batch(gf_ctx* ctx, int gauge, double* F, double* theta, double* theta_slice) {
     if (!ctx) return GF_EINVAL;
     if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_measure: no links set");
     if (gauge < GF_LANDAU || gauge > GF_MAG) return fail(ctx, GF_EINVAL, "unknown gauge %d", gauge);
@@ -471,13 +560,23 @@ int gf_measure(gf_ctx* ctx, int gauge, double* F, double* theta, double* theta_s
     int rc = enqueue_measure(ctx, gauge);
     if (rc) return rc;
     CU(cudaStreamSynchronize(ctx->stream));
-    finish_measure(ctx, gauge, F, theta, theta_slice, nullptr);
+    for (int c = 0; c < ctx->B; ++c)
+        finish_measure(ctx, gauge, c, F ? F + c : nullptr, theta ? theta + c : nullptr,
+                       theta_slice ? theta_slice + (size_t)c * ctx->Nt : nullptr, nullptr);
     return GF_OK;
+}
+
+int gf_measure(gf_ctx* ctx, int gauge, double* F, double* theta, double* theta_slice) {
+    if (!ctx) return GF_EINVAL;
+    int rc = single_only(ctx, "gf_measure");
+    if (rc) return rc;
+    return gf_measure_batch(ctx, gauge, F, theta, theta_slice);
 }
 
 // ---- reunitarisation -----------------------------------------------------------------------------
 #define REUNIT_LINKS(R, RECON, dummy)                                                                       \
-    reunit_kernel<R, RECON><<<(unsigned)((8 * ctx->Vh + 255) / 256), 256, 0, ctx->stream>>>(ctx->links, ctx->Vh, 8)
+    reunit_kernel<R, RECON><<<dim3((unsigned)((8 * ctx->Vh + 255) / 256), (unsigned)ctx->B), 256, 0, ctx->stream>>>( \
+        ctx->links, ctx->Vh, 8, link_store_bytes(ctx))
 
 int gf_reunitarize(gf_ctx* ctx) {
     if (!ctx) return GF_EINVAL;
@@ -486,9 +585,9 @@ int gf_reunitarize(gf_ctx* ctx) {
     CU(cudaGetLastError());
     ++ctx->launches;
     if (ctx->gtot) {
-        const unsigned g = (unsigned)((2 * ctx->Vh + 255) / 256);
-        if (ctx->real_bytes == 4) reunit_kernel<float, 18><<<g, 256, 0, ctx->stream>>>(ctx->gtot, ctx->Vh, 2);
-        else reunit_kernel<double, 18><<<g, 256, 0, ctx->stream>>>(ctx->gtot, ctx->Vh, 2);
+        const dim3 g((unsigned)((2 * ctx->Vh + 255) / 256), (unsigned)ctx->B);
+        if (ctx->real_bytes == 4) reunit_kernel<float, 18><<<g, 256, 0, ctx->stream>>>(ctx->gtot, ctx->Vh, 2, field_store_bytes(ctx));
+        else reunit_kernel<double, 18><<<g, 256, 0, ctx->stream>>>(ctx->gtot, ctx->Vh, 2, field_store_bytes(ctx));
         CU(cudaGetLastError());
         ++ctx->launches;
     }
@@ -497,8 +596,8 @@ int gf_reunitarize(gf_ctx* ctx) {
 
 // ---- Coulomb finalisation ------------------------------------------------------------------------
 #define FINALIZE(R, RECON, dummy)                                                                           \
-    coulomb_finalize_kernel<R, RECON><<<(unsigned)((2 * ctx->Vh + 127) / 128), 128, 0, ctx->stream>>>(       \
-        ctx->links, ctx->gtot, ctx->gapplied, dims_of(ctx))
+    coulomb_finalize_kernel<R, RECON><<<dim3((unsigned)((2 * ctx->Vh + 127) / 128), (unsigned)ctx->B), 128, 0, ctx->stream>>>( \
+        ctx->links, ctx->gtot, ctx->gapplied, dims_of(ctx), link_store_bytes(ctx), field_store_bytes(ctx))
 
 int gf_coulomb_finalize(gf_ctx* ctx) {
     if (!ctx) return GF_EINVAL;
@@ -509,10 +608,11 @@ int gf_coulomb_finalize(gf_ctx* ctx) {
     CU(cudaGetLastError());
     ++ctx->launches;
     if (!ctx->gapplied) {
-        CU(cudaMalloc((void**)&ctx->gapplied, (size_t)field_store_bytes(ctx)));
-        ctx->device_bytes += field_store_bytes(ctx);
+        CU(cudaMalloc((void**)&ctx->gapplied, (size_t)(ctx->B * field_store_bytes(ctx))));
+        ctx->device_bytes += ctx->B * field_store_bytes(ctx);
     }
-    CU(cudaMemcpyAsync(ctx->gapplied, ctx->gtot, (size_t)field_store_bytes(ctx), cudaMemcpyDeviceToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->gapplied, ctx->gtot, (size_t)(ctx->B * field_store_bytes(ctx)), cudaMemcpyDeviceToDevice,
+                       ctx->stream));
     ctx->temporal_stale = false;
     return GF_OK;
 }
@@ -525,34 +625,43 @@ static int sweep_gx(const gf_ctx* ctx) {
     return (Vsh + block - 1) / block;
 }
 
-// exact F / theta of the current links (measure kernels: double, both parities) -> host scalars
-static int exact_measure(gf_ctx* ctx, int gauge, double* F, double* stop) {
+// exact F / theta terms of the current links (measure kernels: double, both parities) -> slice_host
+static int exact_measure(gf_ctx* ctx, int gauge) {
     int rc = enqueue_measure(ctx, gauge);
     if (rc) return rc;
     CU(cudaStreamSynchronize(ctx->stream));
-    double theta = 0.0, tmax = 0.0;
-    finish_measure(ctx, gauge, F, &theta, nullptr, &tmax);
-    *stop = (gauge == GF_COULOMB) ? tmax : theta;
     return GF_OK;
 }
 
 /*
- * gf_run.  With the fused reductions (default) the odd half-sweep of a check sweep s
- * leaves, at no extra traffic, F(s) (every link touches exactly one odd site) and theta_odd(s), the odd
- * sites' share of theta(s); the even sites' share is what the even half-sweep of sweep s+1 sees before
- * it updates.  theta(s) >= theta_odd(s), so a check with theta_odd(s) >= eps cannot have converged and
- * costs nothing; only when theta_odd(s) < eps is the exact reduction (measure kernels) run, so the
- * stopping decision is the one a reduction after every check would take.  History entries carry
- * theta(s) = theta_odd(s) + theta_even(s), completed at the following check (or by the exact
- * reduction); the values returned in *out always come from the exact reduction of the final links.
+ * run_impl — Alg. 1's outer loop for every gauge copy of the context at once.
  *
- * Per-slice Coulomb fixing (GF_FLAG_FREEZE_SLICES): the same bound is used slice by
- * slice.  A slice whose theta_odd,t(s) < eps triggers the exact reduction; every not yet stopped slice
- * with exact theta_t(s) < eps is stopped at sweep s: its flag in skip_dev makes its CTAs exit at once
- * in all later half-sweeps, and its exact slice sums stand in for the (no longer written) partials.
+ * Units.  The lattice sites are grouped into independent optimisation problems ("units"), each with
+ * its own stopping quantity: a gauge copy (Landau, MAG: theta of Eq. (7)/(16); Coulomb: max_t theta_t),
+ * or, for Coulomb with GF_FLAG_FREEZE_SLICES, a single time-slice of a copy.  A
+ * unit is stopped ("frozen") at the first check at which its exact stopping quantity is < eps: the
+ * flags of its slices in skip_dev make its CTAs exit at once in all later half-sweeps, and its exact
+ * slice sums stand in for the partials those CTAs no longer write.  The loop ends when every unit is
+ * frozen or after max_sweeps.  With one copy and one unit this is the plain "sweep until theta < eps".
+ *
+ * Fused reductions (default).  The odd half-sweep of a check sweep s leaves, at no
+ * extra traffic, F(s) (every link touches exactly one odd site) and theta_odd(s), the odd sites' share
+ * of theta(s); the even sites' share is what the even half-sweep of sweep s+1 sees before it updates.
+ * theta(s) >= theta_odd(s), so a unit with theta_odd(s) >= eps cannot have converged and its check
+ * costs nothing; only when some running unit has theta_odd(s) < eps is the exact reduction (measure
+ * kernels) run, so every stopping decision is the one a reduction after every check would take.
+ * History entries carry theta(s) = theta_odd(s) + theta_even(s), completed at the following check (or
+ * by the exact reduction); the values returned in out[] always come from the exact reduction of the
+ * final links.
+ *
+ * skip_slice: NULL, or [B*Nt] flags of slices that are not to be touched by this run (gf_fix: units that
+ * converged in an earlier stage; a unit is left alone when all of its slices are flagged); they are
+ * reported with sweeps = 0.  ctx->slice_frozen receives the slices of the units stopped by this run.
+ * hist: NULL or [checks][B][3] = (sweep, F, stopping quantity).
  */
-int gf_run(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t first_sweep_index,
-           int max_sweeps, double eps, int check_every, int reunit_every, gf_result* out, double* hist) {
+static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t first_sweep_index,
+                    int max_sweeps, double eps, int check_every, int reunit_every, const unsigned char* skip_slice,
+                    gf_result* out, double* hist, bool* all_converged) {
     int rc = check_sweep_args(ctx, gauge, algo, param);
     if (rc) return rc;
     if (max_sweeps < 0 || check_every < 1 || reunit_every < 0) return fail(ctx, GF_EINVAL, "gf_run: bad loop arguments");
@@ -560,63 +669,92 @@ int gf_run(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32
     if (rc) return rc;
     const bool fused = ctx->fused != 0;
     const bool coulomb = gauge == GF_COULOMB;
-    const bool freeze = coulomb && (ctx->flags & GF_FLAG_FREEZE_SLICES);
+    const bool per_slice = coulomb && (ctx->flags & GF_FLAG_FREEZE_SLICES);
     const int nd = coulomb ? 3 : 4;
-    const int Nt = ctx->Nt;
+    const int Nt = ctx->Nt, B = ctx->B, NS = ctx->NS;
+    const int nunits = per_slice ? NS : B, uspan = per_slice ? 1 : Nt;   // unit u = slices [u*uspan, (u+1)*uspan)
     const int gx = sweep_gx(ctx);
     const double Vs = (double)ctx->Nx * ctx->Ny * ctx->Nz;
-    double F = 0.0, stop = 0.0;
-    bool have_exact = false, converged = false;
+    bool have_exact = false;
 
-    // slices already stopped, with the exact slice sums (F terms, theta terms) they were stopped at
-    std::vector<unsigned char> frozen((size_t)Nt, 0);
-    std::vector<double> fz_F((size_t)Nt, 0.0), fz_th((size_t)Nt, 0.0);
+    // frozen slices, with the exact slice sums (F terms, theta terms) they were stopped at
+    std::vector<unsigned char> frozen((size_t)NS, 0), unit_frozen((size_t)nunits, 0);
+    std::vector<double> fz_F((size_t)NS, 0.0), fz_th((size_t)NS, 0.0);
+    std::vector<double> Fc((size_t)B, 0.0), stopc((size_t)B, 0.0);
     int n_frozen = 0;
-    ctx->slice_sweeps.assign((size_t)Nt, 0);
+    ctx->slice_sweeps.assign((size_t)NS, 0);
     ctx->have_slice_sweeps = true;
-    const unsigned char* skip = nullptr;
-    if (freeze) {
-        memset(ctx->skip_host, 0, (size_t)Nt);
-        CU(cudaMemcpyAsync(ctx->skip_dev, ctx->skip_host, (size_t)Nt, cudaMemcpyHostToDevice, ctx->stream));
-        skip = ctx->skip_dev;
-    }
-    // stopping quantity from per-slice sums of theta terms a[t] (+ b[t]): theta (Eq. (7)), or max_t theta_t
-    auto stop_of = [&](const double* a, int sa, const double* b, int sb) {
+    const bool use_skip = nunits > 1 || skip_slice;
+    const unsigned char* skip = use_skip ? ctx->skip_dev : nullptr;
+    if (use_skip) memset(ctx->skip_host, 0, (size_t)NS);
+
+    // stopping quantity of slices [lo, hi) from per-slice sums of theta terms val(s): Eq. (7) over the
+    // slices' sites, or max_t theta_t for Coulomb
+    auto stop_range = [&](int lo, int hi, auto val) {
         double tot = 0.0, tmax = 0.0;
-        for (int t = 0; t < Nt; ++t) {
-            const double v = frozen[(size_t)t] ? fz_th[(size_t)t]
-                                               : a[(size_t)t * sa] + (b ? b[(size_t)t * sb] : 0.0);
+        for (int sl = lo; sl < hi; ++sl) {
+            const double v = frozen[(size_t)sl] ? fz_th[(size_t)sl] : val(sl);
             tot += v;
             if (v / (3.0 * Vs) > tmax) tmax = v / (3.0 * Vs);
         }
         return coulomb ? tmax : tot / (3.0 * (double)ctx->V);
     };
-    // stop every running slice whose exact theta_t (slice_host, just reduced) is below eps
-    auto apply_freeze = [&](int s_now) -> int {
-        bool changed = false;
-        for (int t = 0; t < Nt; ++t) {
-            if (frozen[(size_t)t]) continue;
-            if (ctx->slice_host[Nt + t] / (3.0 * Vs) < eps) {
-                frozen[(size_t)t] = 1;
-                fz_F[(size_t)t] = ctx->slice_host[t];
-                fz_th[(size_t)t] = ctx->slice_host[Nt + t];
-                ctx->slice_sweeps[(size_t)t] = s_now;
-                ctx->skip_host[t] = 1;
-                ++n_frozen;
-                changed = true;
-            }
+    auto freeze_unit = [&](int u, int s_now) {
+        unit_frozen[(size_t)u] = 1;
+        ++n_frozen;
+        for (int sl = u * uspan; sl < (u + 1) * uspan; ++sl) {
+            frozen[(size_t)sl] = 1;
+            fz_F[(size_t)sl] = ctx->slice_host[sl];
+            fz_th[(size_t)sl] = ctx->slice_host[NS + sl];
+            ctx->slice_sweeps[(size_t)sl] = s_now;
+            if (use_skip) ctx->skip_host[sl] = 1;
         }
-        if (changed)
-            CU(cudaMemcpyAsync(ctx->skip_dev, ctx->skip_host, (size_t)Nt, cudaMemcpyHostToDevice, ctx->stream));
+    };
+    // after an exact reduction (slice_host): stop every running unit whose exact stopping quantity is
+    // below eps, then fill F and the stopping quantity of every copy from the exact sums
+    auto after_exact = [&](int s_now) -> int {
+        bool changed = false;
+        for (int u = 0; u < nunits; ++u) {
+            if (unit_frozen[(size_t)u]) continue;
+            const double st = stop_range(u * uspan, (u + 1) * uspan, [&](int sl) { return ctx->slice_host[NS + sl]; });
+            if (st < eps) { freeze_unit(u, s_now); changed = true; }
+        }
+        if (changed && use_skip)
+            CU(cudaMemcpyAsync(ctx->skip_dev, ctx->skip_host, (size_t)NS, cudaMemcpyHostToDevice, ctx->stream));
+        for (int c = 0; c < B; ++c) {
+            double fs = 0.0;
+            for (int sl = c * Nt; sl < (c + 1) * Nt; ++sl) fs += frozen[(size_t)sl] ? fz_F[(size_t)sl] : ctx->slice_host[sl];
+            Fc[(size_t)c] = fs / (3.0 * nd * (double)ctx->V);
+            stopc[(size_t)c] = stop_range(c * Nt, (c + 1) * Nt, [&](int sl) { return ctx->slice_host[NS + sl]; });
+        }
+        have_exact = true;
         return GF_OK;
     };
+
+    if (skip_slice) {   // units left alone: frozen from the start with their exact sums
+        rc = exact_measure(ctx, gauge);
+        if (rc) return rc;
+        for (int u = 0; u < nunits; ++u) {
+            bool all = true;
+            for (int sl = u * uspan; sl < (u + 1) * uspan; ++sl) all = all && skip_slice[sl];
+            if (all) freeze_unit(u, 0);
+        }
+    }
+    if (use_skip) CU(cudaMemcpyAsync(ctx->skip_dev, ctx->skip_host, (size_t)NS, cudaMemcpyHostToDevice, ctx->stream));
 
     // history entry still waiting for the even sites' share of theta:
     //   stage 1 = the next even half-sweep must produce it, stage 2 = produced, reduced at the next check
     int pend_stage = 0, pend_entry = -1;
-    std::vector<double> pend_odd((size_t)Nt, 0.0);
+    std::vector<double> pend_odd((size_t)NS, 0.0);
+    auto complete_pending = [&](const double* ev) {   // ev = [NS][3] partial sums of the even half-sweep
+        if (hist)
+            for (int c = 0; c < B; ++c)
+                hist[3 * ((size_t)pend_entry * B + c) + 2] =
+                    stop_range(c * Nt, (c + 1) * Nt, [&](int sl) { return pend_odd[(size_t)sl] + ev[3 * sl + 2]; });
+        pend_stage = 0;
+    };
     int s = 0, nh = 0, last_entry_sweep = -1;
-    while (s < max_sweeps) {
+    while (s < max_sweeps && n_frozen < nunits) {
         const bool check_now = ((s + 1) % check_every == 0) || (s + 1 == max_sweeps);
         const bool red_even = fused && pend_stage == 1;
         const uint32_t idx = first_sweep_index + (uint32_t)s;
@@ -636,116 +774,237 @@ int gf_run(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32
         if (!check_now) continue;
         if (!fused || reunit_now) {   // links were just reprojected: reduce what is stored now
             if (pend_stage == 2) {
-                red_reduce_kernel<<<Nt, 128, 0, ctx->stream>>>(ctx->red_part[0], gx, ctx->red_dev);
+                red_reduce_kernel<<<NS, 128, 0, ctx->stream>>>(ctx->red_part[0], gx, ctx->red_dev);
                 CU(cudaGetLastError());
                 ++ctx->launches;
-                CU(cudaMemcpyAsync(ctx->red_host, ctx->red_dev, (size_t)3 * Nt * sizeof(double),
+                CU(cudaMemcpyAsync(ctx->red_host, ctx->red_dev, (size_t)3 * NS * sizeof(double),
                                    cudaMemcpyDeviceToHost, ctx->stream));
             }
-            rc = exact_measure(ctx, gauge, &F, &stop);
+            rc = exact_measure(ctx, gauge);
             if (rc) return rc;
-            if (pend_stage == 2 && hist)
-                hist[3 * pend_entry + 2] = stop_of(pend_odd.data(), 1, ctx->red_host + 2, 3);
+            if (pend_stage == 2) complete_pending(ctx->red_host);
             pend_stage = 0;
-            have_exact = true;
-            if (freeze) {
-                rc = apply_freeze(s);
-                if (rc) return rc;
-            }
+            rc = after_exact(s);
+            if (rc) return rc;
         } else {
-            red_reduce_kernel<<<Nt, 128, 0, ctx->stream>>>(ctx->red_part[1], gx, ctx->red_dev + 3 * Nt);
+            red_reduce_kernel<<<NS, 128, 0, ctx->stream>>>(ctx->red_part[1], gx, ctx->red_dev + 3 * NS);
             CU(cudaGetLastError());
             ++ctx->launches;
             if (pend_stage == 2) {
-                red_reduce_kernel<<<Nt, 128, 0, ctx->stream>>>(ctx->red_part[0], gx, ctx->red_dev);
+                red_reduce_kernel<<<NS, 128, 0, ctx->stream>>>(ctx->red_part[0], gx, ctx->red_dev);
                 CU(cudaGetLastError());
                 ++ctx->launches;
             }
-            CU(cudaMemcpyAsync(ctx->red_host, ctx->red_dev, (size_t)6 * Nt * sizeof(double), cudaMemcpyDeviceToHost,
+            CU(cudaMemcpyAsync(ctx->red_host, ctx->red_dev, (size_t)6 * NS * sizeof(double), cudaMemcpyDeviceToHost,
                                ctx->stream));
             CU(cudaStreamSynchronize(ctx->stream));
-            const double* ev = ctx->red_host;            // [t][3]: even half-sweep of this or an earlier sweep
-            const double* od = ctx->red_host + 3 * Nt;   // [t][3]: odd half-sweep of sweep s
-            if (pend_stage == 2) {
-                if (hist) hist[3 * pend_entry + 2] = stop_of(pend_odd.data(), 1, ev + 2, 3);
-                pend_stage = 0;
-            }
-            double fs = 0.0;
-            for (int t = 0; t < Nt; ++t) fs += frozen[(size_t)t] ? fz_F[(size_t)t] : od[3 * t];
-            F = fs / (3.0 * nd * (double)ctx->V);
-            stop = stop_of(od + 1, 3, nullptr, 0);   // lower bound of theta(s)
-            bool need_exact = stop < eps;
-            if (freeze)   // a running slice may have converged on its own
-                for (int t = 0; t < Nt && !need_exact; ++t)
-                    need_exact = !frozen[(size_t)t] && od[3 * t + 1] / (3.0 * Vs) < eps;
+            const double* ev = ctx->red_host;            // [sl][3]: even half-sweep of this or an earlier sweep
+            const double* od = ctx->red_host + 3 * NS;   // [sl][3]: odd half-sweep of sweep s
+            if (pend_stage == 2) complete_pending(ev);
+            // lower bounds theta_odd(s) of the running units
+            bool need_exact = false;
+            for (int u = 0; u < nunits && !need_exact; ++u)
+                need_exact = !unit_frozen[(size_t)u] &&
+                             stop_range(u * uspan, (u + 1) * uspan, [&](int sl) { return od[3 * sl + 1]; }) < eps;
             if (need_exact) {
-                rc = exact_measure(ctx, gauge, &F, &stop);
+                rc = exact_measure(ctx, gauge);
                 if (rc) return rc;
-                have_exact = true;
-                if (freeze) {
-                    rc = apply_freeze(s);
-                    if (rc) return rc;
-                }
+                rc = after_exact(s);
+                if (rc) return rc;
             } else {
-                for (int t = 0; t < Nt; ++t) pend_odd[(size_t)t] = od[3 * t + 1];
+                for (int c = 0; c < B; ++c) {
+                    double fs = 0.0;
+                    for (int sl = c * Nt; sl < (c + 1) * Nt; ++sl) fs += frozen[(size_t)sl] ? fz_F[(size_t)sl] : od[3 * sl];
+                    Fc[(size_t)c] = fs / (3.0 * nd * (double)ctx->V);
+                    stopc[(size_t)c] = stop_range(c * Nt, (c + 1) * Nt, [&](int sl) { return od[3 * sl + 1]; });
+                }
+                for (int sl = 0; sl < NS; ++sl) pend_odd[(size_t)sl] = od[3 * sl + 1];
                 pend_stage = 1;
                 pend_entry = nh;
             }
         }
-        if (hist) { hist[3 * nh] = (double)s; hist[3 * nh + 1] = F; hist[3 * nh + 2] = stop; }
+        if (hist)
+            for (int c = 0; c < B; ++c) {
+                double* h = hist + 3 * ((size_t)nh * B + c);
+                h[0] = (double)s; h[1] = Fc[(size_t)c]; h[2] = stopc[(size_t)c];
+            }
         last_entry_sweep = s;
         ++nh;
-        if (freeze ? (n_frozen == Nt) : (have_exact && stop < eps)) { converged = true; break; }
     }
     if (!have_exact) {
-        rc = exact_measure(ctx, gauge, &F, &stop);
+        rc = exact_measure(ctx, gauge);
         if (rc) return rc;
-        converged = freeze ? (n_frozen == Nt) : (stop < eps);
-        if (hist && nh > 0 && last_entry_sweep == s) { hist[3 * (nh - 1) + 1] = F; hist[3 * (nh - 1) + 2] = stop; }
+        rc = after_exact(s);
+        if (rc) return rc;
+        if (hist && nh > 0 && last_entry_sweep == s)
+            for (int c = 0; c < B; ++c) {
+                double* h = hist + 3 * ((size_t)(nh - 1) * B + c);
+                h[1] = Fc[(size_t)c]; h[2] = stopc[(size_t)c];
+            }
     }
-    for (int t = 0; t < Nt; ++t)
-        if (!frozen[(size_t)t]) ctx->slice_sweeps[(size_t)t] = s;
+    for (int sl = 0; sl < NS; ++sl)
+        if (!frozen[(size_t)sl]) ctx->slice_sweeps[(size_t)sl] = s;
+    ctx->slice_frozen = frozen;
     if (coulomb && ctx->gtot) {
         rc = gf_coulomb_finalize(ctx);
         if (rc) return rc;
         CU(cudaStreamSynchronize(ctx->stream));
     }
-    if (out) { out->sweeps = s; out->F = F; out->theta = stop; }
-    return converged ? GF_OK : GF_NOT_CONVERGED;
+    if (out)
+        for (int c = 0; c < B; ++c) {
+            int sw = 0;
+            for (int sl = c * Nt; sl < (c + 1) * Nt; ++sl)
+                if (ctx->slice_sweeps[(size_t)sl] > sw) sw = ctx->slice_sweeps[(size_t)sl];
+            out[c].sweeps = sw; out[c].F = Fc[(size_t)c]; out[c].theta = stopc[(size_t)c];
+        }
+    if (all_converged) *all_converged = (n_frozen == nunits);
+    return GF_OK;
+}
+
+int gf_run_batch(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t first_sweep_index,
+                 int max_sweeps, double eps, int check_every, int reunit_every, gf_result* out, double* hist) {
+    if (!ctx) return GF_EINVAL;
+    bool conv = false;
+    int rc = run_impl(ctx, gauge, algo, param, seed, first_sweep_index, max_sweeps, eps, check_every, reunit_every,
+                      nullptr, out, hist, &conv);
+    if (rc) return rc;
+    return conv ? GF_OK : GF_NOT_CONVERGED;
+}
+
+int gf_run(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t first_sweep_index,
+           int max_sweeps, double eps, int check_every, int reunit_every, gf_result* out, double* hist) {
+    if (!ctx) return GF_EINVAL;
+    int rc = single_only(ctx, "gf_run");
+    if (rc) return rc;
+    return gf_run_batch(ctx, gauge, algo, param, seed, first_sweep_index, max_sweeps, eps, check_every, reunit_every,
+                        out, hist);
 }
 
 int gf_get_slice_sweeps(gf_ctx* ctx, int* sweeps) {
     if (!ctx) return GF_EINVAL;
     if (!sweeps) return fail(ctx, GF_EINVAL, "gf_get_slice_sweeps: NULL pointer");
     if (!ctx->have_slice_sweeps) return fail(ctx, GF_ESTATE, "gf_get_slice_sweeps: no gf_run yet");
-    for (int t = 0; t < ctx->Nt; ++t) sweeps[t] = ctx->slice_sweeps[(size_t)t];
+    for (int t = 0; t < ctx->NS; ++t) sweeps[t] = ctx->slice_sweeps[(size_t)t];
+    return GF_OK;
+}
+
+// the annealing schedule; reunit_every > 0 reprojects after every reunit_every-th sweep of the schedule
+static int anneal_impl(gf_ctx* ctx, int gauge, double T_hi, double T_lo, int n_steps, int n_micro, uint64_t seed,
+                       uint32_t first_sweep_index, int reunit_every, uint32_t* next_sweep_index) {
+    int rc = check_sweep_args(ctx, gauge, GF_SA, T_hi);
+    if (rc) return rc;
+    if (!(T_lo > 0.0) || n_steps < 0 || n_micro < 0 || reunit_every < 0) return fail(ctx, GF_EINVAL, "gf_anneal: bad schedule");
+    rc = pre_sweep(ctx, gauge);
+    if (rc) return rc;
+    uint32_t idx = first_sweep_index;
+    int done = 0;
+    auto one = [&](int algo, double par) -> int {
+        for (int p = 0; p < 2; ++p) {
+            int r = launch_half(ctx, gauge, algo, par, seed, idx, p);
+            if (r) return r;
+        }
+        ++idx;
+        ++done;
+        if (reunit_every && done % reunit_every == 0) return gf_reunitarize(ctx);
+        return GF_OK;
+    };
+    for (int k = 0; k < n_steps; ++k) {
+        const double T = (n_steps <= 1) ? T_hi : T_hi - k * (T_hi - T_lo) / (n_steps - 1);
+        rc = one(GF_SA, T);
+        if (rc) return rc;
+        for (int m = 0; m < n_micro; ++m) {
+            rc = one(GF_MICRO, 0.0);
+            if (rc) return rc;
+        }
+    }
+    if (next_sweep_index) *next_sweep_index = idx;
     return GF_OK;
 }
 
 int gf_anneal(gf_ctx* ctx, int gauge, double T_hi, double T_lo, int n_steps, int n_micro, uint64_t seed,
               uint32_t first_sweep_index, uint32_t* next_sweep_index) {
-    int rc = check_sweep_args(ctx, gauge, GF_SA, T_hi);
-    if (rc) return rc;
-    if (!(T_lo > 0.0) || n_steps < 0 || n_micro < 0) return fail(ctx, GF_EINVAL, "gf_anneal: bad schedule");
-    rc = pre_sweep(ctx, gauge);
-    if (rc) return rc;
-    uint32_t idx = first_sweep_index;
-    for (int k = 0; k < n_steps; ++k) {
-        const double T = (n_steps <= 1) ? T_hi : T_hi - k * (T_hi - T_lo) / (n_steps - 1);
-        for (int p = 0; p < 2; ++p) {
-            rc = launch_half(ctx, gauge, GF_SA, T, seed, idx, p);
-            if (rc) return rc;
-        }
-        ++idx;
-        for (int m = 0; m < n_micro; ++m) {
-            for (int p = 0; p < 2; ++p) {
-                rc = launch_half(ctx, gauge, GF_MICRO, 0.0, seed, idx, p);
-                if (rc) return rc;
-            }
-            ++idx;
-        }
+    return anneal_impl(ctx, gauge, T_hi, T_lo, n_steps, n_micro, seed, first_sweep_index, 0, next_sweep_index);
+}
+
+// ---- the SA -> SR -> OR pipeline ------------------------------------------
+int gf_fix(gf_ctx* ctx, const gf_fix_params* p, gf_result* out) {
+    if (!ctx) return GF_EINVAL;
+    if (!p) return fail(ctx, GF_EINVAL, "gf_fix: NULL parameters");
+    if (p->sa_steps < 0 || p->sr_max_sweeps < 0 || p->or_max_sweeps < 0 || p->check_every < 1 || p->reunit_every < 0)
+        return fail(ctx, GF_EINVAL, "gf_fix: bad stage lengths");
+    const int B = ctx->B, Nt = ctx->Nt, NS = ctx->NS;
+    uint32_t idx = 0;
+    int rc;
+    std::vector<int> total((size_t)NS, 0);   // sweeps per slice, all stages
+    std::vector<unsigned char> done;
+    std::vector<gf_result> res((size_t)B);
+    bool have_res = false, all = false;
+    if (p->sa_steps > 0) {   // stage 1: simulated annealing, every copy
+        rc = anneal_impl(ctx, p->gauge, p->sa_T_hi, p->sa_T_lo, p->sa_steps, p->sa_micro, p->seed, idx, p->reunit_every, &idx);
+        if (rc) return rc;
+        for (int sl = 0; sl < NS; ++sl) total[(size_t)sl] += (int)idx;
     }
-    if (next_sweep_index) *next_sweep_index = idx;
+    if (p->sr_max_sweeps > 0) {   // stage 2: stochastic relaxation until theta < eps, at most sr_max_sweeps
+        rc = run_impl(ctx, p->gauge, GF_SR, p->sr_p, p->seed, idx, p->sr_max_sweeps, p->eps, p->check_every,
+                      p->reunit_every, nullptr, res.data(), nullptr, &all);
+        if (rc) return rc;
+        have_res = true;
+        for (int sl = 0; sl < NS; ++sl) total[(size_t)sl] += ctx->slice_sweeps[(size_t)sl];
+        done = ctx->slice_frozen;
+    }
+    if (p->or_max_sweeps > 0 && !(have_res && all)) {   // stage 3: overrelaxation of the units still running
+        rc = run_impl(ctx, p->gauge, GF_OR, p->or_omega, p->seed, idx, p->or_max_sweeps, p->eps, p->check_every,
+                      p->reunit_every, have_res ? done.data() : nullptr, res.data(), nullptr, &all);
+        if (rc) return rc;
+        for (int sl = 0; sl < NS; ++sl) total[(size_t)sl] += ctx->slice_sweeps[(size_t)sl];
+        have_res = true;
+    }
+    if (!have_res) {   // annealing only: report the exact F / theta of what it left
+        rc = run_impl(ctx, p->gauge, GF_OR, 1.0, p->seed, idx, 0, p->eps, 1, 0, nullptr, res.data(), nullptr, &all);
+        if (rc) return rc;
+    }
+    ctx->slice_sweeps = total;
+    if (out)
+        for (int c = 0; c < B; ++c) {
+            out[c] = res[(size_t)c];
+            int sw = 0;
+            for (int sl = c * Nt; sl < (c + 1) * Nt; ++sl)
+                if (total[(size_t)sl] > sw) sw = total[(size_t)sl];
+            out[c].sweeps = sw;
+        }
+    return all ? GF_OK : GF_NOT_CONVERGED;
+}
+
+// ---- random start on the gauge orbit ------------------------------------------
+#define GAUGE_APPLY(R, RECON, hf)                                                                               \
+    gauge_apply_kernel<R, RECON><<<dim3((unsigned)((ctx->Vh + 127) / 128), (unsigned)ctx->B, 2), 128, 0, ctx->stream>>>( \
+        ctx->links, ctx->gtot, (hf), dims_of(ctx), link_store_bytes(ctx), field_store_bytes(ctx))
+
+int gf_random_gauge(gf_ctx* ctx, uint64_t seed) {
+    if (!ctx) return GF_EINVAL;
+    if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_random_gauge: no links set");
+    if (ctx->temporal_stale && ctx->gtot) {
+        int rc = gf_coulomb_finalize(ctx);
+        if (rc) return rc;
+    }
+    char* h = nullptr;
+    CU(cudaMalloc((void**)&h, (size_t)(ctx->B * field_store_bytes(ctx))));
+    const dim3 g((unsigned)((ctx->V + 127) / 128), (unsigned)ctx->B);
+    if (ctx->real_bytes == 4) haar_field_kernel<float><<<g, 128, 0, ctx->stream>>>(h, dims_of(ctx), seed, field_store_bytes(ctx));
+    else haar_field_kernel<double><<<g, 128, 0, ctx->stream>>>(h, dims_of(ctx), seed, field_store_bytes(ctx));
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) {
+        DISPATCH_RR(ctx, GAUGE_APPLY, h);
+        e = cudaGetLastError();
+    }
+    ctx->launches += 2;
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    cudaFree(h);
+    CU(e);
+    // the transform just applied counts as already applied to the temporal links
+    if (ctx->gapplied)
+        CU(cudaMemcpyAsync(ctx->gapplied, ctx->gtot, (size_t)(ctx->B * field_store_bytes(ctx)), cudaMemcpyDeviceToDevice,
+                           ctx->stream));
     return GF_OK;
 }
 

@@ -38,7 +38,11 @@ struct SweepArgs {
     //   (F term after the update, theta term after the update, theta term before the update)
     // of the sites this launch updates (fused reductions)
     double* red;
-    const unsigned char* slice_skip;   // nullptr, or [Nt]: 1 = leave this time-slice alone (frozen)
+    const unsigned char* slice_skip;   // nullptr, or [ncopies*Nt]: 1 = leave this time-slice alone (frozen)
+    // batched gauge copies: blockIdx.y = copy*Nt + t; copy c lives at links + c*copy_links_bytes
+    // (gtot + c*copy_gtot_bytes) and draws its random numbers with the Philox key seed + c
+    int ncopies;
+    int64_t copy_links_bytes, copy_gtot_bytes;
 };
 
 // ---- asynchronous global -> shared copies -------------------------------------------------
@@ -122,25 +126,25 @@ GF_DEV void global_get(const char* plane0, int64_t Vh, int64_t cb, Mat<R>& m) {
 
 // ---- Step 1 for one subgroup (I,J), index S in the Cabibbo-Marinari order (0,1),(0,2),(1,2) ----
 template <bool STOCH, class A>
-GF_DEV void choose_rule(const A a[4], A g[4], bool mag, A Dm, A Em, A Fm, const SweepArgs& args, uint32_t site,
-                        int sub) {
+GF_DEV void choose_rule(const A a[4], A g[4], bool mag, A Dm, A Em, A Fm, const SweepArgs& args, uint64_t seed,
+                        uint32_t site, int sub) {
     if (!STOCH) {
         if (args.algo == ALGO_MICRO) rule_micro<A>(a, g);
         else rule_or<A>(a, (A)args.param, g);
     } else {
         if (args.algo == ALGO_SR) {
             // stochastic relaxation: g^2 with probability p, else g
-            const double u = uniform01(rng_draw(args.seed, site, args.sweep_index, sub, 0, 0).x);
+            const double u = uniform01(rng_draw(seed, site, args.sweep_index, sub, 0, 0).x);
             if (u < args.param) rule_micro<A>(a, g);
             else rule_or<A>(a, A(1), g);
         } else {
             double gd[4];
             if (mag) {
-                rule_heatbath_mag((double)Dm, (double)Em, (double)Fm, args.param, args.seed, site, args.sweep_index,
+                rule_heatbath_mag((double)Dm, (double)Em, (double)Fm, args.param, seed, site, args.sweep_index,
                                   sub, gd);
             } else {
                 const double ad[4] = {(double)a[0], (double)a[1], (double)a[2], (double)a[3]};
-                rule_heatbath_landau(ad, args.param, args.seed, site, args.sweep_index, sub, gd);
+                rule_heatbath_landau(ad, args.param, seed, site, args.sweep_index, sub, gd);
             }
             g[0] = (A)gd[0]; g[1] = (A)gd[1]; g[2] = (A)gd[2]; g[3] = (A)gd[3];
         }
@@ -148,20 +152,20 @@ GF_DEV void choose_rule(const A a[4], A g[4], bool mag, A Dm, A Em, A Fm, const 
 }
 
 template <int I, int J, int S, bool STOCH, class A>
-GF_DEV void subgroup_landau(Mat<A>& K, Mat<A>& G, const SweepArgs& args, uint32_t site) {
+GF_DEV void subgroup_landau(Mat<A>& K, Mat<A>& G, const SweepArgs& args, uint64_t seed, uint32_t site) {
     // Fig. A.10 on K, signs per Eq. (15)
     A a[4], g[4];
     a[0] = K.v[RE(I, I)] + K.v[RE(J, J)];
     a[3] = K.v[IM(I, I)] - K.v[IM(J, J)];
     a[2] = K.v[RE(I, J)] - K.v[RE(J, I)];
     a[1] = K.v[IM(I, J)] + K.v[IM(J, I)];
-    choose_rule<STOCH, A>(a, g, false, A(0), A(0), A(0), args, site, S);
+    choose_rule<STOCH, A>(a, g, false, A(0), A(0), A(0), args, seed, site, S);
     sub_left<I, J>(K, g);   // applying g at x maps K(x) -> g K(x)
     sub_left<I, J>(G, g);
 }
 
 template <int I, int J, int S, bool STOCH, class A>
-GF_DEV void subgroup_mag(Herm<A> (&M)[3], Mat<A>& G, const SweepArgs& args, uint32_t site) {
+GF_DEV void subgroup_mag(Herm<A> (&M)[3], Mat<A>& G, const SweepArgs& args, uint64_t seed, uint32_t site) {
     // f(g) = const + g^T [[D,E,F],[E,-D,0],[F,0,-D]] g  (Eqs. (25)-(28), SU(3) form)
     // (I,J) with I < J: off-diagonal element (I,J) of a Herm is o[2*OFF], o[2*OFF+1]
     constexpr int OFF = (I == 0) ? (J - 1) : 2;
@@ -172,7 +176,7 @@ GF_DEV void subgroup_mag(Herm<A> (&M)[3], Mat<A>& G, const SweepArgs& args, uint
     const A Fm = M[I].o[2 * OFF] - M[J].o[2 * OFF];
     const A lam = sqrt_t(Dm * Dm + Em * Em + Fm * Fm);   // Eq. (29)
     A a[4] = {Dm + lam, -Em, -Fm, A(0)}, g[4];
-    choose_rule<STOCH, A>(a, g, true, Dm, Em, Fm, args, site, S);
+    choose_rule<STOCH, A>(a, g, true, Dm, Em, Fm, args, seed, site, S);
 #pragma unroll
     for (int k = 0; k < 3; ++k) {   // M_k -> g M_k g^dagger
         Mat<A> F;
@@ -240,14 +244,18 @@ sweep_kernel(const SweepArgs args) {
     constexpr int NL = 2 * ND;
     extern __shared__ __align__(16) unsigned char smem[];
 
-    // grid = (ceil(Vsh / block), Nt): blockIdx.y is the time-slice, so a CTA never straddles slices
-    // (per-slice reductions, frozen slices).  Threads past the end of the slice redo the last site
-    // without storing, so that every thread reaches the block reduction.
+    // grid = (ceil(Vsh / block), ncopies*Nt): blockIdx.y is (gauge copy, time-slice), so a CTA never
+    // straddles slices (per-slice reductions, frozen slices).  Threads past the end of the slice redo
+    // the last site without storing, so that every thread reaches the block reduction.
     const int Nzh = args.Nz >> 1;
     const int Vsh = args.Nx * args.Ny * Nzh;
     const int64_t Vh = (int64_t)args.Nt * Vsh;
-    const int t = blockIdx.y;
-    if (args.slice_skip && args.slice_skip[t]) return;   // block-uniform
+    if (args.slice_skip && args.slice_skip[blockIdx.y]) return;   // block-uniform
+    const int copy = blockIdx.y / args.Nt;
+    const int t = blockIdx.y - copy * args.Nt;
+    char* const links = args.links + copy * args.copy_links_bytes;
+    char* const gtot = TRACK ? args.gtot + copy * args.copy_gtot_bytes : nullptr;
+    const uint64_t seed = args.seed + (uint64_t)copy;
     const int i_raw = blockIdx.x * blockDim.x + threadIdx.x;
     const bool active = i_raw < Vsh;
     const int i_s = active ? i_raw : Vsh - 1;
@@ -280,8 +288,8 @@ sweep_kernel(const SweepArgs args) {
     const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem) + (uint32_t)tid * 16;
     const int64_t plane = 16 * Vh;
     const int64_t lstride = (int64_t)L::LINK_BYTES * Vh;
-    char* const up0 = args.links + L::link_offset(par, MU0, Vh);        // U_mu(x): own parity
-    char* const dn0 = args.links + L::link_offset(1 - par, MU0, Vh);    // U_mu(x - mu): other parity
+    char* const up0 = links + L::link_offset(par, MU0, Vh);        // U_mu(x): own parity
+    char* const dn0 = links + L::link_offset(1 - par, MU0, Vh);    // U_mu(x - mu): other parity
     {
         const char* pu = up0;
         const char* pd = dn0;
@@ -305,7 +313,7 @@ sweep_kernel(const SweepArgs args) {
         }
     }
     Mat<R> Gt;
-    if (TRACK) global_get<R, 18>(args.gtot + Layout<R, 18>::site_offset(par, Vh), Vh, cb, Gt);
+    if (TRACK) global_get<R, 18>(gtot + Layout<R, 18>::site_offset(par, Vh), Vh, cb, Gt);
     cp_async_wait_all();
 
     // ---- a3: neighbourhood summary, pass 1 over the links ----
@@ -337,13 +345,13 @@ sweep_kernel(const SweepArgs args) {
 
     // ---- a4/a5: Step 1 through the three SU(2) subgroups, G = g3 g2 g1 ----
     if (GAUGE == GAUGE_MAG) {
-        subgroup_mag<0, 1, 0, STOCH, A>(M, G, args, site);
-        subgroup_mag<0, 2, 1, STOCH, A>(M, G, args, site);
-        subgroup_mag<1, 2, 2, STOCH, A>(M, G, args, site);
+        subgroup_mag<0, 1, 0, STOCH, A>(M, G, args, seed, site);
+        subgroup_mag<0, 2, 1, STOCH, A>(M, G, args, seed, site);
+        subgroup_mag<1, 2, 2, STOCH, A>(M, G, args, seed, site);
     } else {
-        subgroup_landau<0, 1, 0, STOCH, A>(K, G, args, site);
-        subgroup_landau<0, 2, 1, STOCH, A>(K, G, args, site);
-        subgroup_landau<1, 2, 2, STOCH, A>(K, G, args, site);
+        subgroup_landau<0, 1, 0, STOCH, A>(K, G, args, seed, site);
+        subgroup_landau<0, 2, 1, STOCH, A>(K, G, args, seed, site);
+        subgroup_landau<1, 2, 2, STOCH, A>(K, G, args, seed, site);
     }
 
     // the summary now is that of the updated site (K -> G K, M_k -> G M_k G^dag): its F and theta terms
@@ -380,7 +388,7 @@ sweep_kernel(const SweepArgs args) {
     if (TRACK) {
         Mat<R> O;
         mul_left<3>(G, Gt, O);
-        if (active) global_put<R, 18>(args.gtot + Layout<R, 18>::site_offset(par, Vh), Vh, cb, O);
+        if (active) global_put<R, 18>(gtot + Layout<R, 18>::site_offset(par, Vh), Vh, cb, O);
     }
 
     // ---- a9 fused: block partials of (F, theta after, theta before), double, fixed order ----

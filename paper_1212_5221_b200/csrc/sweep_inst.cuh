@@ -22,7 +22,7 @@ static cudaError_t launch_one(const SweepArgs& args, int block, cudaStream_t str
         if (e != cudaSuccess) return e;
         smem_set = smem;
     }
-    const dim3 grid((unsigned)((Vsh + block - 1) / block), (unsigned)args.Nt);
+    const dim3 grid((unsigned)((Vsh + block - 1) / block), (unsigned)(args.ncopies * args.Nt));
     kern<<<grid, block, smem, stream>>>(args);
     return cudaGetLastError();
 }

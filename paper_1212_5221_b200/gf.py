@@ -29,7 +29,8 @@ GF_OR, GF_SR, GF_SA, GF_MICRO = 0, 1, 2, 3
 GF_FLAG_TRACK_TRANSFORM = 1
 GF_FLAG_FREEZE_SLICES = 2
 
-EXPORTS = ["gf_create", "gf_destroy", "gf_set_links", "gf_get_links", "gf_get_gauge_transform", "gf_sweep",
+EXPORTS = ["gf_create", "gf_create_batch", "gf_num_copies", "gf_set_links_copy", "gf_get_links_copy",
+           "gf_get_gauge_transform_copy", "gf_measure_batch", "gf_run_batch", "gf_fix", "gf_random_gauge", "gf_destroy", "gf_set_links", "gf_get_links", "gf_get_gauge_transform", "gf_sweep",
            "gf_half_sweep", "gf_measure", "gf_run", "gf_get_slice_sweeps", "gf_anneal", "gf_reunitarize", "gf_coulomb_finalize",
            "gf_sync", "gf_kernel_timing", "gf_kernel_time_ms", "gf_launch_count", "gf_device_bytes", "gf_volume", "gf_last_error", "gf_version"]
 
@@ -38,7 +39,24 @@ class gf_result(ctypes.Structure):
     _fields_ = [("sweeps", ctypes.c_int), ("F", ctypes.c_double), ("theta", ctypes.c_double)]
 
 
+class gf_fix_params(ctypes.Structure):
+    _fields_ = [("gauge", ctypes.c_int), ("seed", ctypes.c_uint64), ("sa_steps", ctypes.c_int),
+                ("sa_T_hi", ctypes.c_double), ("sa_T_lo", ctypes.c_double), ("sa_micro", ctypes.c_int),
+                ("sr_max_sweeps", ctypes.c_int), ("sr_p", ctypes.c_double), ("or_omega", ctypes.c_double),
+                ("or_max_sweeps", ctypes.c_int), ("eps", ctypes.c_double), ("check_every", ctypes.c_int),
+                ("reunit_every", ctypes.c_int)]
+
+
 _vp, _ci, _cd, _u64, _u32 = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_uint64, ctypes.c_uint32
+_lib.gf_create_batch.argtypes = [ctypes.POINTER(_vp), _ci, _ci, _ci, _ci, _ci, _ci, _ci, ctypes.c_uint, _vp]
+_lib.gf_num_copies.argtypes = [_vp]
+_lib.gf_set_links_copy.argtypes = [_vp, _ci, _vp, _ci, _ci]
+_lib.gf_get_links_copy.argtypes = [_vp, _ci, _vp, _ci, _ci]
+_lib.gf_get_gauge_transform_copy.argtypes = [_vp, _ci, _vp, _ci, _ci]
+_lib.gf_measure_batch.argtypes = [_vp, _ci, _vp, _vp, _vp]
+_lib.gf_run_batch.argtypes = [_vp, _ci, _ci, _cd, _u64, _u32, _ci, _cd, _ci, _ci, _vp, _vp]
+_lib.gf_fix.argtypes = [_vp, ctypes.POINTER(gf_fix_params), _vp]
+_lib.gf_random_gauge.argtypes = [_vp, _u64]
 _lib.gf_create.argtypes = [ctypes.POINTER(_vp), _ci, _ci, _ci, _ci, _ci, _ci, ctypes.c_uint, _vp]
 _lib.gf_destroy.argtypes = [_vp]
 _lib.gf_set_links.argtypes = [_vp, _vp, _ci, _ci]
@@ -102,9 +120,7 @@ def gf_version() -> str:
     return _lib.gf_version().decode()
 
 
-def gf_create(Nx, Ny, Nz, Nt, precision, recon=18, flags=0, cuda_stream=None):
-    """-> opaque context handle.  cuda_stream: None (torch's current stream if torch has CUDA,
-    else the default stream), an int cudaStream_t, or a torch.cuda.Stream."""
+def _stream_handle(cuda_stream):
     if cuda_stream is None:
         try:
             import torch
@@ -113,10 +129,28 @@ def gf_create(Nx, Ny, Nz, Nt, precision, recon=18, flags=0, cuda_stream=None):
             cuda_stream = 0
     elif hasattr(cuda_stream, "cuda_stream"):
         cuda_stream = cuda_stream.cuda_stream
+    return cuda_stream
+
+
+def gf_create(Nx, Ny, Nz, Nt, precision, recon=18, flags=0, cuda_stream=None):
+    """-> opaque context handle.  cuda_stream: None (torch's current stream if torch has CUDA,
+    else the default stream), an int cudaStream_t, or a torch.cuda.Stream."""
     h = _vp()
-    rc = _lib.gf_create(ctypes.byref(h), Nx, Ny, Nz, Nt, precision, recon, flags, _vp(cuda_stream))
+    rc = _lib.gf_create(ctypes.byref(h), Nx, Ny, Nz, Nt, precision, recon, flags, _vp(_stream_handle(cuda_stream)))
     _check(None, rc)
     return h
+
+
+def gf_create_batch(Nx, Ny, Nz, Nt, n_copies, precision, recon=18, flags=0, cuda_stream=None):
+    h = _vp()
+    rc = _lib.gf_create_batch(ctypes.byref(h), Nx, Ny, Nz, Nt, n_copies, precision, recon, flags,
+                              _vp(_stream_handle(cuda_stream)))
+    _check(None, rc)
+    return h
+
+
+def gf_num_copies(ctx):
+    return int(_lib.gf_num_copies(ctx))
 
 
 def gf_destroy(ctx):
@@ -145,6 +179,71 @@ def gf_get_gauge_transform(ctx, out):
     p, eb, dev, n = _buffer(out)
     _sized(ctx, n, 18, "gf_get_gauge_transform")
     return _check(ctx, _lib.gf_get_gauge_transform(ctx, _vp(p), eb, dev))
+
+
+def gf_set_links_copy(ctx, copy, links):
+    p, eb, dev, n = _buffer(links)
+    _sized(ctx, n, 72, "gf_set_links_copy")
+    return _check(ctx, _lib.gf_set_links_copy(ctx, copy, _vp(p), eb, dev))
+
+
+def gf_get_links_copy(ctx, copy, out):
+    p, eb, dev, n = _buffer(out)
+    _sized(ctx, n, 72, "gf_get_links_copy")
+    return _check(ctx, _lib.gf_get_links_copy(ctx, copy, _vp(p), eb, dev))
+
+
+def gf_get_gauge_transform_copy(ctx, copy, out):
+    p, eb, dev, n = _buffer(out)
+    _sized(ctx, n, 18, "gf_get_gauge_transform_copy")
+    return _check(ctx, _lib.gf_get_gauge_transform_copy(ctx, copy, _vp(p), eb, dev))
+
+
+def gf_measure_batch(ctx, gauge, Nt=None):
+    """-> (F[n_copies], theta[n_copies]) or, with Nt given, (F, theta, theta_slice[n_copies, Nt])."""
+    B = gf_num_copies(ctx)
+    F, th = np.zeros(B), np.zeros(B)
+    ts = np.zeros((B, Nt)) if Nt else None
+    _check(ctx, _lib.gf_measure_batch(ctx, gauge, _vp(F.ctypes.data), _vp(th.ctypes.data),
+                                      _vp(ts.ctypes.data) if Nt else None))
+    return (F, th, ts) if Nt else (F, th)
+
+
+def gf_run_batch(ctx, gauge, algo, param, seed=0, first_sweep_index=0, max_sweeps=1000, eps=1e-12, check_every=1,
+                 reunit_every=0, history=False):
+    """-> list of dict(sweeps, F, theta, converged[, history]) per copy."""
+    B = gf_num_copies(ctx)
+    res = (gf_result * B)()
+    nchk = max_sweeps // check_every + 1
+    hist = np.zeros((nchk, B, 3)) if history else None
+    rc = _lib.gf_run_batch(ctx, gauge, algo, float(param), seed, first_sweep_index, max_sweeps, float(eps),
+                           check_every, reunit_every, ctypes.cast(res, _vp), _vp(hist.ctypes.data) if history else None)
+    _check(ctx, rc, ok=(GF_OK, GF_NOT_CONVERGED))
+    out = []
+    for c in range(B):
+        d = {"sweeps": res[c].sweeps, "F": res[c].F, "theta": res[c].theta, "converged": res[c].theta < eps}
+        if history:
+            n = int(np.count_nonzero(hist[:, c, 0]))
+            d["history"] = hist[:n, c]
+        out.append(d)
+    return out
+
+
+def gf_fix(ctx, gauge, seed=0, sa_steps=0, sa_T_hi=1.0, sa_T_lo=0.01, sa_micro=3, sr_max_sweeps=0, sr_p=0.5,
+           or_omega=1.7, or_max_sweeps=1000, eps=1e-12, check_every=1, reunit_every=0):
+    """SA -> SR -> OR pipeline.  -> list of dict(sweeps, F, theta, converged) per copy."""
+    B = gf_num_copies(ctx)
+    p = gf_fix_params(gauge, seed, sa_steps, float(sa_T_hi), float(sa_T_lo), sa_micro, sr_max_sweeps, float(sr_p),
+                      float(or_omega), or_max_sweeps, float(eps), check_every, reunit_every)
+    res = (gf_result * B)()
+    rc = _lib.gf_fix(ctx, ctypes.byref(p), ctypes.cast(res, _vp))
+    _check(ctx, rc, ok=(GF_OK, GF_NOT_CONVERGED))
+    return [{"sweeps": res[c].sweeps, "F": res[c].F, "theta": res[c].theta, "converged": res[c].theta < eps}
+            for c in range(B)]
+
+
+def gf_random_gauge(ctx, seed):
+    return _check(ctx, _lib.gf_random_gauge(ctx, seed))
 
 
 def gf_sweep(ctx, gauge, algo, param, seed=0, sweep_index=0):
@@ -179,7 +278,7 @@ def gf_run(ctx, gauge, algo, param, seed=0, first_sweep_index=0, max_sweeps=1000
 
 
 def gf_get_slice_sweeps(ctx, Nt):
-    out = np.zeros(Nt, dtype=np.int32)
+    out = np.zeros(Nt * gf_num_copies(ctx), dtype=np.int32)
     _check(ctx, _lib.gf_get_slice_sweeps(ctx, _vp(out.ctypes.data)))
     return out
 
@@ -243,11 +342,11 @@ class GaugeFixer:
     """Context manager around one gf_ctx.  Methods forward to the C entry points of the same name."""
 
     def __init__(self, Nx, Ny, Nz, Nt, precision=GF_DP, recon=18, track_transform=False, cuda_stream=None,
-                 freeze_slices=False):
+                 freeze_slices=False, n_copies=1):
         self.dims = (Nx, Ny, Nz, Nt)
-        self.precision, self.recon = precision, recon
+        self.precision, self.recon, self.n_copies = precision, recon, n_copies
         flags = (GF_FLAG_TRACK_TRANSFORM if track_transform else 0) | (GF_FLAG_FREEZE_SLICES if freeze_slices else 0)
-        self.ctx = gf_create(Nx, Ny, Nz, Nt, precision, recon, flags, cuda_stream)
+        self.ctx = gf_create_batch(Nx, Ny, Nz, Nt, n_copies, precision, recon, flags, cuda_stream)
 
     def close(self):
         if self.ctx is not None:
@@ -312,3 +411,31 @@ class GaugeFixer:
 
     def sync(self):
         return gf_sync(self.ctx)
+
+    # ---- batched gauge copies (gf_create_batch) ----
+    def set_links_copy(self, copy, links):
+        return gf_set_links_copy(self.ctx, copy, links)
+
+    def get_links_copy(self, copy, out=None, dtype=np.float64):
+        if out is None:
+            out = np.empty(self.shape, dtype=dtype)
+        gf_get_links_copy(self.ctx, copy, out)
+        return out
+
+    def get_gauge_transform_copy(self, copy, out=None, dtype=np.float64):
+        if out is None:
+            out = np.empty(self.shape[:4] + (3, 3, 2), dtype=dtype)
+        gf_get_gauge_transform_copy(self.ctx, copy, out)
+        return out
+
+    def measure_batch(self, gauge, slices=False):
+        return gf_measure_batch(self.ctx, gauge, self.dims[3] if slices else None)
+
+    def run_batch(self, gauge, algo, param, **kw):
+        return gf_run_batch(self.ctx, gauge, algo, param, **kw)
+
+    def fix(self, gauge, **kw):
+        return gf_fix(self.ctx, gauge, **kw)
+
+    def random_gauge(self, seed):
+        return gf_random_gauge(self.ctx, seed)
