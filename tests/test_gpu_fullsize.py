@@ -168,3 +168,83 @@ def test_full_size_sampled_sites_nonperiodic(gf, oracle, tile, dims, prec, recon
             W = up_out[..., 0] + 1j * up_out[..., 1]
             uni = np.abs(W @ np.conj(np.swapaxes(W, -1, -2)) - np.eye(3)).max()
             assert uni < (1e-12 if prec == DP else 2e-5)
+
+
+# ---- full runs at BASELINE.json's sizes ---------------------------------------------------------
+# A deterministic run (OR: no random numbers) of a periodic tiling follows the run of its tile sweep by
+# sweep, and F, theta and theta_t are intensive: the oracle runs the 16^4 tile, the GPU the full lattice.
+
+@pytest.mark.parametrize("prec,recon", [(SP, 12), (MP, 12)])
+def test_config2_full_run_coulomb_32x32x32x64(gf, oracle, prec, recon):
+    # BASELINE.json configs[2]: Coulomb OR 1.7, SP links / 12 reals, DP reunitarisation every 100 sweeps,
+    # DP reductions, eps = 0.6 links, per-time-slice theta < 1e-10, at most 5000 sweeps
+    import torch
+    dims = (32, 32, 32, 64)
+    t16 = inputs.as_real(inputs.make_config(16, 16, 16, 16, 0.6, 1002, 2002), np.float32)
+    ref = t16.copy()
+    s, F, th, hist, conv = oracle.run(ref, COULOMB, OR, 1.7, max_sweeps=5000, eps=1e-10, check_every=10,
+                                      reunit_every=100, mixed=(prec == MP))
+    dev = torch.device("cuda", 0)
+    src = torch.from_numpy(t16).to(dev).repeat(*reps(dims), 1, 1, 1, 1).contiguous()
+    with gf.GaugeFixer(*dims, precision=prec, recon=recon, track_transform=True) as fx:
+        fx.set_links(src)
+        r = fx.run(COULOMB, OR, 1.7, max_sweeps=5000, eps=1e-10, check_every=10, reunit_every=100)
+        F2, th2, ths = fx.measure(COULOMB, slices=True)
+    assert conv and r["converged"]
+    assert abs(r["F"] - F) <= 1e-5                      # BASELINE: F to 1e-5 in SP
+    assert r["theta"] < 1e-10 and ths.max() < 1e-10
+    assert abs(r["sweeps"] - s) <= 0.1 * s + 20         # SP: rounding decides which check first sees 1e-10
+    # the 64 slices are 4 periods of the tile's 16: equal slices, equal theta_t
+    np.testing.assert_allclose(ths[:16], ths[16:32], rtol=1e-6, atol=1e-16)
+
+
+@pytest.mark.parametrize("prec,recon,tolF", [(DP, 18, 1e-10), (SP, 12, 1e-5)])
+def test_config4_500_sweeps_64x64x64x256(gf, oracle, tile, prec, recon, tolF):
+    # BASELINE.json configs[4]: Landau OR 1.7 on 64^3 x 256, 500 sweeps + F/theta (what bench.py times)
+    import torch
+    dims = (64, 64, 64, 256)
+    dt = np.float64 if prec == DP else np.float32
+    ref = tile.astype(dt)
+    reunit = 0 if prec == DP else 100
+    s, F, th, hist, conv = oracle.run(ref, LANDAU, OR, 1.7, max_sweeps=500, eps=-1.0, check_every=100,
+                                      reunit_every=reunit)
+    dev = torch.device("cuda", 0)
+    src = torch.from_numpy(tile.astype(dt)).to(dev).repeat(*reps(dims), 1, 1, 1, 1).contiguous()
+    with gf.GaugeFixer(*dims, precision=prec, recon=recon) as fx:
+        fx.set_links(src)
+        del src
+        r = fx.run(LANDAU, OR, 1.7, max_sweeps=500, eps=-1.0, check_every=100, reunit_every=reunit, history=True)
+    assert r["sweeps"] == s == 500 and not r["converged"]
+    assert abs(r["F"] - F) <= tolF
+    assert abs(r["theta"] - th) <= (0.1 * th if prec == DP else max(0.1 * th, 1e-12))
+    np.testing.assert_allclose(r["history"][:, 1], [h[1] for h in hist], atol=tolF)
+
+
+def test_config3_mag_anneal_24x24x24x24(gf, oracle):
+    # BASELINE.json configs[3]: MAG, DP, 24^4, SA T 1.45 -> 0.01 over 2000 steps with 3 microcanonical
+    # sweeps each (Philox seed 1234), then OR 1.7 to theta < 1e-12.  The first annealing step is compared
+    # with the oracle link by link (draws identical: <= 1e-11); the whole schedule is chaotic (DESIGN.md
+    # R25), so after it the checks are the ones that hold for any Gribov copy: theta < eps, the links are
+    # the gauge transform of the input by the returned g (Eq. (1)), F well above the start.
+    dims = (24, 24, 24, 24)
+    U = inputs.config_k(3)
+    L = inputs.as_real(U)
+    ref = L.copy()
+    T0 = oracle.temperature(0, 2000, 1.45, 0.01)
+    oracle.sweep(ref, MAG, 2, T0, seed=1234, sweep_index=0)
+    F0 = oracle.measure(L, MAG)["F"]
+    with gf.GaugeFixer(*dims, precision=DP, track_transform=True) as fx:
+        fx.set_links(L)
+        fx.sweep(MAG, 2, T0, seed=1234, sweep_index=0)
+        assert np.abs(fx.get_links() - ref).max() <= 1e-11
+        fx.set_links(L)
+        res = fx.fix(MAG, seed=1234, sa_steps=2000, sa_T_hi=1.45, sa_T_lo=0.01, sa_micro=3, or_omega=1.7,
+                     or_max_sweeps=20000, eps=1e-12, check_every=10)[0]
+        got = fx.get_links()
+        g = fx.get_gauge_transform()
+    assert res["converged"] and res["theta"] < 1e-12 and res["sweeps"] > 8000
+    assert res["F"] > F0 + 0.1
+    m = oracle.measure(got, MAG)                        # the oracle's reductions on the GPU's result
+    assert abs(m["F"] - res["F"]) < 1e-12 and m["theta"] < 1e-12
+    gc = g[..., 0] + 1j * g[..., 1]
+    assert np.abs(inputs.as_complex(got) - inputs.gauge_transform(U, gc)).max() < 1e-9
