@@ -72,6 +72,7 @@ def parse_args():
     ap.add_argument("--no-variants", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-others", action="store_true", help="skip the 32^3x64 and batched-copies side measurements")
     ap.add_argument("--block", type=int, default=0, help="CTA size override of the half-sweep kernel (tuning)")
     return ap.parse_args()
 
@@ -383,9 +384,55 @@ def run_ours(args):
                              "bytes_per_site_update": v["roofline"]["bytes_per_site_update"],
                              "kernel_share_of_step": v["kernel_share_of_step"]})
 
+    def bench_other(dims_o, gauge, prec, recon, copies, sweeps, label):
+        """Side measurement (not the headline): `sweeps` OR sweeps of `copies` lattices of extent dims_o."""
+        ox, oy, oz, ot = dims_o
+        Vo = ox * oy * oz * ot
+        nd = 3 if gauge == 1 else 4
+        r_o = (ot // TILE[3], ox // TILE[0], oy // TILE[1], oz // TILE[2])
+        with torch.cuda.stream(stream):
+            src = torch.from_numpy(tile).to(dev).repeat(*r_o, 1, 1, 1, 1).contiguous()
+        with gf.GaugeFixer(ox, oy, oz, ot, precision=PREC_NAMES[prec], recon=recon, n_copies=copies,
+                           cuda_stream=stream) as fx:
+            fx.set_links(src)
+            del src
+            fx.run_batch(gauge, OR, OMEGA, max_sweeps=10, eps=-1.0, check_every=10)
+            gf.gf_kernel_timing(fx.ctx, True)
+            gf.gf_kernel_time_ms(fx.ctx, reset=True)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            fx.run_batch(gauge, OR, OMEGA, max_sweeps=sweeps, eps=-1.0, check_every=sweeps)
+            e1.record(stream)
+            stream.synchronize()
+            ms = e0.elapsed_time(e1)
+            kern_ms, kern_n = gf.gf_kernel_time_ms(fx.ctx, reset=True)
+            gf.gf_kernel_timing(fx.ctx, False)
+        bpsu = bytes_per_site_update(prec, recon, nd)
+        ach = bpsu * (copies * Vo // 2) / (kern_ms / kern_n * 1e-3) / 1e9
+        store = copies * Vo * 4 * recon * (8 if prec == "dp" else 4)
+        return {"workload": label, "lattice": list(dims_o), "copies": copies, "precision": prec, "recon": recon,
+                "sweeps": sweeps, "value": copies * Vo * sweeps / (ms * 1e-3), "unit": "site-updates/s",
+                "avg_launch_ms": kern_ms / kern_n, "roofline_achieved_gbs": ach, "roofline_frac": ach / peak,
+                "bytes_per_site_update": bpsu, "link_store_bytes": store,
+                "resident_in": "L2 (126 MB): not an HBM measurement" if store < 100e6 else "HBM"}
+
+    others = []
+    if rank == 0 and world == 1 and not args.no_others:
+        del links_dev
+        links_dev = None
+        torch.cuda.empty_cache()
+        others = [
+            bench_other((32, 32, 32, 64), 0, "dp", 18, 1, 200, "Landau OR, 32^3x64, DP-18"),
+            bench_other((32, 32, 32, 64), 0, "sp", 12, 1, 200, "Landau OR, 32^3x64, SP-12"),
+            bench_other((32, 32, 32, 64), 1, "sp", 12, 1, 200, "Coulomb OR, 32^3x64, SP-12 (BASELINE.json configs[2])"),
+            bench_other((16, 16, 16, 16), 0, "dp", 18, 1, 200, "Landau OR, 16^4, DP-18, one copy (configs[1])"),
+            bench_other((16, 16, 16, 16), 0, "dp", 18, 64, 100, "Landau OR, 64 gauge copies of 16^4 per launch, DP-18"),
+            bench_other((32, 32, 32, 32), 0, "sp", 12, 16, 100, "Landau OR, 16 gauge copies of 32^4 per launch, SP-12"),
+        ]
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        del links_dev
+        links_dev = None
         torch.cuda.empty_cache()
         r = oracle_leg(tile, args.precision, 5, 6, 1)
         cpu = {"value": r["value"], "unit": "site-updates/s", "cores": r["cores"], "kind": "oracle",
@@ -413,6 +460,7 @@ def run_ours(args):
             "kernel_share_of_step": head["kernel_share_of_step"],
             "roofline": head["roofline"], "clocks": head.get("clocks"),
             "e2e": head.get("e2e"), "cpu_baseline": cpu, "variants": variants,
+            "other_workloads": others,
         }
         print(json.dumps(line), flush=True)
     ranks.close()
