@@ -747,3 +747,6 @@ int gfo_num_threads(void) {
 }
 
 }  // extern "C"
+
+// the N_c = 2 oracle uses the generator, rules and indexer defined above
+#include "gf_oracle_su2.hpp"

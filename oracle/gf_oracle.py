@@ -27,7 +27,8 @@ OR, SR, SA, MICRO = 0, 1, 2, 3
 
 def build(force: bool = False) -> str:
     """Compile the oracle with g++ (-O2, OpenMP).  Building the checker is not using it."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    newest = max(os.path.getmtime(_SRC), os.path.getmtime(os.path.join(_HERE, "gf_oracle_su2.hpp")))
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < newest:
         cmd = ["g++", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c++17",
                "-ffp-contract=off", "-o", _LIB, _SRC]
         subprocess.run(cmd, check=True)
@@ -77,6 +78,21 @@ def lib():
         L.gfo_apply_subgroup_d.argtypes = [vp, vp, ci, ci, ci]
         L.gfo_apply_subgroup_d.restype = None
         L.gfo_num_threads.restype = ci
+        # N_c = 2 (gf_oracle_su2.hpp)
+        L.gfo2_sweep_d.argtypes = [vp, vp, ci, ci, ci, cd, u64, u32, vp]
+        L.gfo2_sweep_f.argtypes = [vp, vp, ci, ci, ci, cd, u64, u32, ci, vp]
+        L.gfo2_measure_d.argtypes = [vp, vp, ci, vp, vp, vp]
+        L.gfo2_measure_f.argtypes = [vp, vp, ci, vp, vp, vp]
+        L.gfo2_reunitarize_d.argtypes = [vp, i64]
+        L.gfo2_reunitarize_f.argtypes = [vp, i64]
+        L.gfo2_reunitarize_d.restype = None
+        L.gfo2_reunitarize_f.restype = None
+        L.gfo2_coulomb_finalize_d.argtypes = [vp, vp, vp]
+        L.gfo2_coulomb_finalize_f.argtypes = [vp, vp, vp]
+        L.gfo2_site_update_d.argtypes = [vp, vp, ci, ci, ci, cd, u64, u32, u32]
+        L.gfo2_site_update_d.restype = None
+        L.gfo2_haar_field_d.argtypes = [vp, vp, u64]
+        L.gfo2_haar_field_d.restype = None
         L.gfo_haar_field_d.argtypes = [vp, vp, u64]
         L.gfo_haar_field_d.restype = None
         _lib = L
@@ -88,9 +104,14 @@ def _p(a: np.ndarray):
 
 
 def _dims(links: np.ndarray) -> np.ndarray:
-    assert links.ndim == 8 and links.shape[4:] == (4, 3, 3, 2), links.shape
+    assert links.ndim == 8 and links.shape[4:] in ((4, 3, 3, 2), (4, 2, 2, 2)), links.shape
     assert links.flags.c_contiguous
     return np.array(links.shape[:4], dtype=np.int32)
+
+
+def nc_of(a: np.ndarray) -> int:
+    """Gauge group of a links / transform array: N_c = 3 ([...,3,3,2]) or 2 ([...,2,2,2])."""
+    return int(a.shape[-2])
 
 
 def num_threads() -> int:
@@ -101,7 +122,7 @@ def _check_gtot(links, gtot):
     if gtot is None:
         return None
     assert gtot.dtype == links.dtype and gtot.flags.c_contiguous
-    assert gtot.shape == links.shape[:4] + (3, 3, 2)
+    assert gtot.shape == links.shape[:4] + links.shape[-3:]
     return _p(gtot)
 
 
@@ -111,11 +132,13 @@ def sweep(links: np.ndarray, gauge: int, algo: int, param: float, seed: int = 0,
     float (SP) or, with ``mixed``, in double (MP).  float64 links: DP."""
     d = _dims(links)
     g = _check_gtot(links, gtot)
+    su2 = nc_of(links) == 2
     if links.dtype == np.float64:
-        rc = lib().gfo_sweep_d(_p(links), _p(d), parity_mask, gauge, algo, float(param), seed, sweep_index, g)
+        fn = lib().gfo2_sweep_d if su2 else lib().gfo_sweep_d
+        rc = fn(_p(links), _p(d), parity_mask, gauge, algo, float(param), seed, sweep_index, g)
     elif links.dtype == np.float32:
-        rc = lib().gfo_sweep_f(_p(links), _p(d), parity_mask, gauge, algo, float(param), seed, sweep_index,
-                               1 if mixed else 0, g)
+        fn = lib().gfo2_sweep_f if su2 else lib().gfo_sweep_f
+        rc = fn(_p(links), _p(d), parity_mask, gauge, algo, float(param), seed, sweep_index, 1 if mixed else 0, g)
     else:
         raise TypeError(links.dtype)
     if rc != 0:
@@ -129,17 +152,23 @@ def measure(links: np.ndarray, gauge: int):
     out = np.zeros(3)
     ths = np.zeros(int(d[0]))
     fs = np.zeros(int(d[0]))
-    fn = lib().gfo_measure_d if links.dtype == np.float64 else lib().gfo_measure_f
+    if nc_of(links) == 2:
+        fn = lib().gfo2_measure_d if links.dtype == np.float64 else lib().gfo2_measure_f
+    else:
+        fn = lib().gfo_measure_d if links.dtype == np.float64 else lib().gfo_measure_f
     rc = fn(_p(links), _p(d), gauge, _p(out), _p(ths), _p(fs))
     if rc != 0:
         raise ValueError("oracle measure: invalid arguments")
-    return {"F": float(out[0]), "theta": float(out[1]), "theta_literal": float(out[2]),
-            "theta_slice": ths, "F_slice": fs}
+    third = "F_eq8" if nc_of(links) == 2 else "theta_literal"      # N_c = 2: F of Eq. (8) (MAG)
+    return {"F": float(out[0]), "theta": float(out[1]), third: float(out[2]), "theta_slice": ths, "F_slice": fs}
 
 
 def reunitarize(mats: np.ndarray) -> None:
     """Gram-Schmidt reprojection of every [...,3,3,2] matrix in place (R20)."""
-    assert mats.flags.c_contiguous and mats.shape[-3:] == (3, 3, 2)
+    assert mats.flags.c_contiguous and mats.shape[-3:] in ((3, 3, 2), (2, 2, 2))
+    if nc_of(mats) == 2:
+        (lib().gfo2_reunitarize_d if mats.dtype == np.float64 else lib().gfo2_reunitarize_f)(_p(mats), mats.size // 8)
+        return
     n = mats.size // 18
     if mats.dtype == np.float64:
         lib().gfo_reunitarize_d(_p(mats), n)
@@ -151,14 +180,17 @@ def coulomb_finalize(links: np.ndarray, gtot: np.ndarray) -> None:
     """U_0(x,t) <- G(x,t) U_0(x,t) G(x,t+1)^dagger (PAPER.md:448)."""
     d = _dims(links)
     g = _check_gtot(links, gtot)
-    fn = lib().gfo_coulomb_finalize_d if links.dtype == np.float64 else lib().gfo_coulomb_finalize_f
+    if nc_of(links) == 2:
+        fn = lib().gfo2_coulomb_finalize_d if links.dtype == np.float64 else lib().gfo2_coulomb_finalize_f
+    else:
+        fn = lib().gfo_coulomb_finalize_d if links.dtype == np.float64 else lib().gfo_coulomb_finalize_f
     if fn(_p(links), g, _p(d)) != 0:
         raise ValueError("oracle coulomb_finalize: invalid arguments")
 
 
 def identity_transform(links: np.ndarray) -> np.ndarray:
-    g = np.zeros(links.shape[:4] + (3, 3, 2), dtype=links.dtype)
-    for i in range(3):
+    g = np.zeros(links.shape[:4] + links.shape[-3:], dtype=links.dtype)
+    for i in range(nc_of(links)):
         g[..., i, i, 0] = 1
     return g
 
@@ -262,11 +294,11 @@ def anneal(links: np.ndarray, gauge: int, T_hi: float, T_lo: float, n_steps: int
     return idx
 
 
-def haar_field(dims_txyz, seed: int) -> np.ndarray:
-    """h[t,x,y,z,3,3,2] (float64), Haar on SU(3) from Philox normals (R27)."""
+def haar_field(dims_txyz, seed: int, nc: int = 3) -> np.ndarray:
+    """h[t,x,y,z,nc,nc,2] (float64), Haar on SU(nc) from Philox normals (R27)."""
     d = np.array(dims_txyz, dtype=np.int32)
-    h = np.zeros(tuple(int(v) for v in d) + (3, 3, 2))
-    lib().gfo_haar_field_d(_p(h), _p(d), seed)
+    h = np.zeros(tuple(int(v) for v in d) + (nc, nc, 2))
+    (lib().gfo2_haar_field_d if nc == 2 else lib().gfo_haar_field_d)(_p(h), _p(d), seed)
     return h
 
 
@@ -283,7 +315,7 @@ def gauge_transform(links: np.ndarray, h: np.ndarray) -> None:
 
 def random_gauge(links: np.ndarray, seed: int, gtot: np.ndarray | None = None) -> None:
     """A random start on the gauge orbit: Haar h(x), Eq. (1); g(x) <- h(x) g(x)."""
-    h = haar_field(links.shape[:4], seed).astype(links.dtype)
+    h = haar_field(links.shape[:4], seed, nc_of(links)).astype(links.dtype)
     gauge_transform(links, h)
     if gtot is not None:
         H = h[..., 0].astype(np.float64) + 1j * h[..., 1].astype(np.float64)
@@ -340,8 +372,11 @@ def site_update(up: np.ndarray, dn: np.ndarray, gauge: int, algo: int, param: fl
                 site_index: int = 0, sweep_index: int = 0, mixed: bool = False):
     """Update of one site from its gathered links up[m]=U_mu(x), dn[m]=U_mu(x-mu), shape [nd,3,3,2]."""
     nd = up.shape[0]
-    assert up.shape == (nd, 3, 3, 2) and dn.shape == up.shape and up.flags.c_contiguous and dn.flags.c_contiguous
-    if up.dtype == np.float64:
+    assert up.shape[1:] in ((3, 3, 2), (2, 2, 2)) and dn.shape == up.shape and up.flags.c_contiguous and dn.flags.c_contiguous
+    if nc_of(up) == 2:
+        assert up.dtype == np.float64
+        lib().gfo2_site_update_d(_p(up), _p(dn), nd, gauge, algo, float(param), seed, site_index, sweep_index)
+    elif up.dtype == np.float64:
         lib().gfo_site_update_d(_p(up), _p(dn), nd, gauge, algo, float(param), seed, site_index, sweep_index, None)
     else:
         lib().gfo_site_update_f(_p(up), _p(dn), nd, gauge, algo, float(param), seed, site_index, sweep_index,

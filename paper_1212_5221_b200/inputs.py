@@ -111,6 +111,41 @@ def config_k(k: int, dims_xyzt=None) -> np.ndarray:
     return make_config(d[0], d[1], d[2], d[3], eps, 1000 + k, 2000 + k)
 
 
+_PAULI = np.array([[[0, 1], [1, 0]], [[0, -1j], [1j, 0]], [[1, 0], [0, -1]]], dtype=np.complex128)
+
+
+def su2_from_quaternion(q: np.ndarray) -> np.ndarray:
+    """q[...,4] on S^3 -> q0 1 + i (q1 s1 + q2 s2 + q3 s3), the parametrisation of PAPER.md:124 Eq. (15)."""
+    out = np.einsum("...a,aij->...ij", q[..., 1:], _PAULI) * 1j
+    out[..., 0, 0] += q[..., 0]
+    out[..., 1, 1] += q[..., 0]
+    return out
+
+
+def random_algebra_links_su2(shape, eps: float, rng: np.random.Generator) -> np.ndarray:
+    """exp(i eps sum_a r_a sigma_a/2), r_a ~ N(0,1): the N_c = 2 analogue of random_algebra_links."""
+    r = rng.standard_normal(tuple(shape) + (3,)) * (0.5 * eps)
+    n = np.linalg.norm(r, axis=-1, keepdims=True)
+    q = np.concatenate([np.cos(n), np.sin(n) * r / np.where(n > 0, n, 1.0)], axis=-1)
+    return su2_from_quaternion(q)
+
+
+def haar_su2(shape, rng: np.random.Generator) -> np.ndarray:
+    """Haar-distributed SU(2): a uniform point of S^3."""
+    q = rng.standard_normal(tuple(shape) + (4,))
+    return su2_from_quaternion(q / np.linalg.norm(q, axis=-1, keepdims=True))
+
+
+def make_config_su2(Nx: int, Ny: int, Nz: int, Nt: int, eps: float, seed_links: int,
+                    seed_gauge: int | None = None) -> np.ndarray:
+    """Synthetic SU(2) lattice, the recipe of make_config with Pauli matrices: complex128 [Nt,Nx,Ny,Nz,4,2,2]."""
+    dims = (Nt, Nx, Ny, Nz)
+    links = random_algebra_links_su2(dims + (4,), eps, np.random.default_rng(seed_links))
+    if seed_gauge is not None:
+        links = gauge_transform(links, haar_su2(dims, np.random.default_rng(seed_gauge)))
+    return links
+
+
 def as_real(links: np.ndarray, dtype=np.float64) -> np.ndarray:
     """complex [...,3,3] -> real [...,3,3,2] (re, im) contiguous, StandardPattern order."""
     out = np.empty(links.shape + (2,), dtype=dtype)
