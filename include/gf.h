@@ -60,6 +60,7 @@ typedef struct gf_ctx gf_ctx; /* opaque */
 
 /* gf_create flags */
 #define GF_FLAG_TRACK_TRANSFORM 1u /* accumulate g(x) so that gf_get_gauge_transform / Coulomb finalisation work */
+#define GF_FLAG_SU2 4u /* gauge group SU(2) instead of SU(3) (Eqs. (8), (12)-(15), (20)-(29)); see "SU(2)" below */
 #define GF_FLAG_FREEZE_SLICES 2u   /* gf_run(Coulomb): stop sweeping a time-slice once its own theta_t < eps */
 
 /*
@@ -72,6 +73,19 @@ typedef struct gf_ctx gf_ctx; /* opaque */
 int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int recon, unsigned flags,
               void* cuda_stream);
 int gf_destroy(gf_ctx* ctx);
+
+/*
+ * SU(2) (contexts created with GF_FLAG_SU2).  The paper states its local problems
+ * for SU(2) — Eq. (20) for Landau/Coulomb, Eqs. (21)-(29) for the maximally
+ * Abelian gauge, theta of Eqs. (12)-(13) — and reaches SU(3) through the SU(2) subgroups;
+ * with this flag the links themselves are SU(2) matrices and Step 1 acts once, on the whole group.  Every
+ * call keeps its meaning with N_c = 2 in Eqs. (4), (7), (11), (13).  Host layouts become
+ * links[t][x][y][z][mu][i][j][c] and g[t][x][y][z][i][j][c] with i,j in {0,1} (8 reals per matrix); only
+ * the first row (u0 + i u3, u2 + i u1) of Eq. (15) is read, the device keeps those four reals
+ * per link (one float4 / two double2; `recon` is ignored) and the second row returned is (-conj b, conj a).
+ * gf_num_colors returns N_c (3 or 2).
+ */
+int gf_num_colors(const gf_ctx* ctx);
 
 /*
  * Batched gauge copies.  The paper's production use fixes many gauge copies

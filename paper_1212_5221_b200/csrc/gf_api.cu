@@ -12,7 +12,9 @@
 
 #include "../../include/gf.h"
 #include "aux_kernels.cuh"
+#include "aux_su2.cuh"
 #include "sweep.cuh"
+#include "sweep_su2.cuh"
 
 using namespace gf;
 
@@ -24,13 +26,17 @@ extern template cudaError_t launch_sweep<float, double, 18>(const SweepArgs&, in
 extern template cudaError_t launch_sweep<float, double, 12>(const SweepArgs&, int, bool, int, cudaStream_t);
 extern template cudaError_t launch_sweep<double, double, 18>(const SweepArgs&, int, bool, int, cudaStream_t);
 extern template cudaError_t launch_sweep<double, double, 12>(const SweepArgs&, int, bool, int, cudaStream_t);
+extern template cudaError_t launch_sweep_su2<float, float>(const SweepArgs&, int, bool, int, cudaStream_t);
+extern template cudaError_t launch_sweep_su2<float, double>(const SweepArgs&, int, bool, int, cudaStream_t);
+extern template cudaError_t launch_sweep_su2<double, double>(const SweepArgs&, int, bool, int, cudaStream_t);
 }  // namespace gf
 
 struct gf_ctx {
     int Nx, Ny, Nz, Nt;
     int B;                  // gauge copies held by this context (gf_create_batch), 1 for gf_create
     int NS;                 // B * Nt: (copy, time-slice) pairs = grid.y of the per-site kernels
-    int precision, recon;
+    int precision, recon;   // recon = reals stored per link: 18 | 12 (SU(3)), 4 (SU(2))
+    int nc;                 // gauge group SU(nc): 3, or 2 with GF_FLAG_SU2
     unsigned flags;
     cudaStream_t stream;
     int64_t V, Vh;
@@ -93,7 +99,9 @@ static Dims dims_of(const gf_ctx* c) {
 }
 // bytes of ONE gauge copy; the B copies of a context are contiguous
 static int64_t link_store_bytes(const gf_ctx* c) { return (int64_t)8 * c->recon * c->real_bytes * c->Vh; }
-static int64_t field_store_bytes(const gf_ctx* c) { return (int64_t)2 * 18 * c->real_bytes * c->Vh; }
+static int64_t field_store_bytes(const gf_ctx* c) { return (int64_t)2 * (c->nc == 2 ? 4 : 18) * c->real_bytes * c->Vh; }
+// reals per matrix in the host layout
+static int64_t host_mat_elems(const gf_ctx* c) { return c->nc == 2 ? 8 : 18; }
 
 // dispatch on (storage type, RECON)
 #define DISPATCH_RR(ctx, FN, ...)                                                  \
@@ -117,6 +125,8 @@ int64_t gf_device_bytes(const gf_ctx* ctx) { return ctx ? ctx->device_bytes : 0;
 
 int64_t gf_volume(const gf_ctx* ctx) { return ctx ? ctx->V : 0; }
 
+int gf_num_colors(const gf_ctx* ctx) { return ctx ? ctx->nc : 0; }
+
 int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int recon, unsigned flags,
               void* cuda_stream) {
     return gf_create_batch(out, Nx, Ny, Nz, Nt, 1, precision, recon, flags, cuda_stream);
@@ -134,6 +144,8 @@ int gf_create_batch(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int n_copies, 
     if (vol >= 4294967296.0) return GF_EINVAL;
     if (precision != GF_SP && precision != GF_DP && precision != GF_MP) return GF_EINVAL;
     if (recon != 18 && recon != 12) return GF_EINVAL;
+    const int nc = (flags & GF_FLAG_SU2) ? 2 : 3;
+    if (nc == 2) recon = 4;   // first row of the 2x2 matrix (csrc/su2.cuh)
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0) return GF_ECUDA;   // no CPU fallback
     gf_ctx* ctx = new (std::nothrow) gf_ctx();
@@ -141,7 +153,7 @@ int gf_create_batch(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int n_copies, 
     ctx->Nx = Nx; ctx->Ny = Ny; ctx->Nz = Nz; ctx->Nt = Nt;
     ctx->B = n_copies; ctx->NS = n_copies * Nt;
     ctx->copies_set.assign((size_t)n_copies, 0);
-    ctx->precision = precision; ctx->recon = recon; ctx->flags = flags;
+    ctx->precision = precision; ctx->recon = recon; ctx->nc = nc; ctx->flags = flags;
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->V = (int64_t)Nx * Ny * Nz * Nt;
     ctx->Vh = ctx->V / 2;
@@ -239,9 +251,39 @@ static const int64_t STAGE_SITES = 1 << 18;   // sites per host<->device staging
     convert_out_kernel<E, R, RECON><<<(unsigned)(((ns) * 4 + 255) / 256), 256, 0, ctx->stream>>>(       \
         (E*)(dst), lbase, dims_of(ctx), (s0), (ns))
 
+// the same for SU(2) contexts: E = host element type, storage type from the context
+#define CONVERT2(KERN, E, hostp, s0, ns)                                                                  \
+    do {                                                                                                  \
+        const unsigned g_ = (unsigned)(((ns) * 4 + 255) / 256);                                           \
+        if (ctx->real_bytes == 4) KERN<E, float><<<g_, 256, 0, ctx->stream>>>((hostp), lbase, dims_of(ctx), (s0), (ns)); \
+        else KERN<E, double><<<g_, 256, 0, ctx->stream>>>((hostp), lbase, dims_of(ctx), (s0), (ns));      \
+    } while (0)
+
+static void convert_in_any(gf_ctx* ctx, char* lbase, const void* src, int elem_bytes, int64_t s0, int64_t ns) {
+    if (ctx->nc == 2) {
+        if (elem_bytes == 4) CONVERT2(convert_in2_kernel, float, (const float*)src, s0, ns);
+        else CONVERT2(convert_in2_kernel, double, (const double*)src, s0, ns);
+    } else {
+        if (elem_bytes == 4) DISPATCH_RR(ctx, CONVERT_IN, float, src, s0, ns);
+        else DISPATCH_RR(ctx, CONVERT_IN, double, src, s0, ns);
+    }
+}
+static void convert_out_any(gf_ctx* ctx, const char* lbase, void* dst, int elem_bytes, int64_t s0, int64_t ns) {
+    if (ctx->nc == 2) {
+        if (elem_bytes == 4) CONVERT2(convert_out2_kernel, float, (float*)dst, s0, ns);
+        else CONVERT2(convert_out2_kernel, double, (double*)dst, s0, ns);
+    } else {
+        if (elem_bytes == 4) DISPATCH_RR(ctx, CONVERT_OUT, float, dst, s0, ns);
+        else DISPATCH_RR(ctx, CONVERT_OUT, double, dst, s0, ns);
+    }
+}
+
 static int field_identity(gf_ctx* ctx, char* field) {
     const unsigned g = (unsigned)((2 * ctx->Vh + 255) / 256);
-    if (ctx->real_bytes == 4) field_identity_kernel<float><<<g, 256, 0, ctx->stream>>>(field, ctx->Vh);
+    if (ctx->nc == 2) {
+        if (ctx->real_bytes == 4) field_identity2_kernel<float><<<g, 256, 0, ctx->stream>>>(field, ctx->Vh);
+        else field_identity2_kernel<double><<<g, 256, 0, ctx->stream>>>(field, ctx->Vh);
+    } else if (ctx->real_bytes == 4) field_identity_kernel<float><<<g, 256, 0, ctx->stream>>>(field, ctx->Vh);
     else field_identity_kernel<double><<<g, 256, 0, ctx->stream>>>(field, ctx->Vh);
     CU(cudaGetLastError());
     ++ctx->launches;
@@ -290,10 +332,9 @@ int gf_set_links_copy(gf_ctx* ctx, int copy, const void* links, int elem_bytes, 
         if (rc) return rc;
     }
     char* lbase = ctx->links + copy * link_store_bytes(ctx);
-    const int64_t link_elems = 4 * 18;
+    const int64_t link_elems = 4 * host_mat_elems(ctx);
     if (is_device) {
-        if (elem_bytes == 4) DISPATCH_RR(ctx, CONVERT_IN, float, links, (int64_t)0, ctx->V);
-        else DISPATCH_RR(ctx, CONVERT_IN, double, links, (int64_t)0, ctx->V);
+        convert_in_any(ctx, lbase, links, elem_bytes, 0, ctx->V);
         CU(cudaGetLastError());
         ++ctx->launches;
     } else {
@@ -305,8 +346,7 @@ int gf_set_links_copy(gf_ctx* ctx, int copy, const void* links, int elem_bytes, 
             const char* src = (const char*)links + s0 * link_elems * elem_bytes;
             CU(cudaMemcpyAsync(ctx->staging, src, (size_t)(ns * link_elems * elem_bytes), cudaMemcpyHostToDevice,
                                ctx->stream));
-            if (elem_bytes == 4) DISPATCH_RR(ctx, CONVERT_IN, float, ctx->staging, s0, ns);
-            else DISPATCH_RR(ctx, CONVERT_IN, double, ctx->staging, s0, ns);
+            convert_in_any(ctx, lbase, ctx->staging, elem_bytes, s0, ns);
             CU(cudaGetLastError());
             ++ctx->launches;
         }
@@ -348,10 +388,9 @@ int gf_get_links_copy(gf_ctx* ctx, int copy, void* links, int elem_bytes, int is
         if (rc) return rc;
     }
     const char* lbase = ctx->links + copy * link_store_bytes(ctx);
-    const int64_t link_elems = 4 * 18;
+    const int64_t link_elems = 4 * host_mat_elems(ctx);
     if (is_device) {
-        if (elem_bytes == 4) DISPATCH_RR(ctx, CONVERT_OUT, float, links, (int64_t)0, ctx->V);
-        else DISPATCH_RR(ctx, CONVERT_OUT, double, links, (int64_t)0, ctx->V);
+        convert_out_any(ctx, lbase, links, elem_bytes, 0, ctx->V);
         CU(cudaGetLastError());
         ++ctx->launches;
     } else {
@@ -361,8 +400,7 @@ int gf_get_links_copy(gf_ctx* ctx, int copy, void* links, int elem_bytes, int is
         for (int64_t s0 = 0; s0 < ctx->V; s0 += chunk) {
             const int64_t ns = (ctx->V - s0 < chunk) ? ctx->V - s0 : chunk;
             char* dst = (char*)links + s0 * link_elems * elem_bytes;
-            if (elem_bytes == 4) DISPATCH_RR(ctx, CONVERT_OUT, float, ctx->staging, s0, ns);
-            else DISPATCH_RR(ctx, CONVERT_OUT, double, ctx->staging, s0, ns);
+            convert_out_any(ctx, lbase, ctx->staging, elem_bytes, s0, ns);
             CU(cudaGetLastError());
             ++ctx->launches;
             CU(cudaMemcpyAsync(dst, ctx->staging, (size_t)(ns * link_elems * elem_bytes), cudaMemcpyDeviceToHost,
@@ -387,26 +425,30 @@ int gf_get_gauge_transform_copy(gf_ctx* ctx, int copy, void* g, int elem_bytes, 
     if (rc) return rc;
     if (!ctx->gtot) return fail(ctx, GF_ESTATE, "gf_get_gauge_transform: context created without GF_FLAG_TRACK_TRANSFORM");
     const char* fbase = ctx->gtot + copy * field_store_bytes(ctx);
+    const int64_t me = host_mat_elems(ctx);
     const int64_t chunk = is_device ? ctx->V : (ctx->V < 4 * STAGE_SITES ? ctx->V : 4 * STAGE_SITES);
     if (!is_device) {
-        rc = ensure_staging(ctx, (size_t)(chunk * 18 * elem_bytes));
+        rc = ensure_staging(ctx, (size_t)(chunk * me * elem_bytes));
         if (rc) return rc;
     }
     for (int64_t s0 = 0; s0 < ctx->V; s0 += chunk) {
         const int64_t ns = (ctx->V - s0 < chunk) ? ctx->V - s0 : chunk;
-        void* dst = is_device ? (void*)((char*)g + s0 * 18 * elem_bytes) : ctx->staging;
+        void* dst = is_device ? (void*)((char*)g + s0 * me * elem_bytes) : ctx->staging;
         const unsigned grid = (unsigned)((ns + 255) / 256);
-        if (ctx->real_bytes == 4) {
-            if (elem_bytes == 4) field_out_kernel<float, float><<<grid, 256, 0, ctx->stream>>>((float*)dst, fbase, dims_of(ctx), s0, ns);
-            else field_out_kernel<double, float><<<grid, 256, 0, ctx->stream>>>((double*)dst, fbase, dims_of(ctx), s0, ns);
-        } else {
-            if (elem_bytes == 4) field_out_kernel<float, double><<<grid, 256, 0, ctx->stream>>>((float*)dst, fbase, dims_of(ctx), s0, ns);
-            else field_out_kernel<double, double><<<grid, 256, 0, ctx->stream>>>((double*)dst, fbase, dims_of(ctx), s0, ns);
+#define FIELD_OUT(KERN)                                                                                              \
+        if (ctx->real_bytes == 4) {                                                                                  \
+            if (elem_bytes == 4) KERN<float, float><<<grid, 256, 0, ctx->stream>>>((float*)dst, fbase, dims_of(ctx), s0, ns);   \
+            else KERN<double, float><<<grid, 256, 0, ctx->stream>>>((double*)dst, fbase, dims_of(ctx), s0, ns);       \
+        } else {                                                                                                     \
+            if (elem_bytes == 4) KERN<float, double><<<grid, 256, 0, ctx->stream>>>((float*)dst, fbase, dims_of(ctx), s0, ns);  \
+            else KERN<double, double><<<grid, 256, 0, ctx->stream>>>((double*)dst, fbase, dims_of(ctx), s0, ns);      \
         }
+        if (ctx->nc == 2) { FIELD_OUT(field_out2_kernel) } else { FIELD_OUT(field_out_kernel) }
+#undef FIELD_OUT
         CU(cudaGetLastError());
         ++ctx->launches;
         if (!is_device)
-            CU(cudaMemcpyAsync((char*)g + s0 * 18 * elem_bytes, ctx->staging, (size_t)(ns * 18 * elem_bytes),
+            CU(cudaMemcpyAsync((char*)g + s0 * me * elem_bytes, ctx->staging, (size_t)(ns * me * elem_bytes),
                                cudaMemcpyDeviceToHost, ctx->stream));
     }
     CU(cudaStreamSynchronize(ctx->stream));
@@ -459,7 +501,11 @@ static int launch_half(gf_ctx* ctx, int gauge, int algo, double param, uint64_t 
     }
     cudaError_t e;
     const int blk = ctx->block_override;
-    if (ctx->precision == GF_DP) {
+    if (ctx->nc == 2) {
+        e = (ctx->precision == GF_DP)   ? launch_sweep_su2<double, double>(a, gauge, track, blk, ctx->stream)
+            : (ctx->precision == GF_MP) ? launch_sweep_su2<float, double>(a, gauge, track, blk, ctx->stream)
+                                        : launch_sweep_su2<float, float>(a, gauge, track, blk, ctx->stream);
+    } else if (ctx->precision == GF_DP) {
         e = (ctx->recon == 18) ? launch_sweep<double, double, 18>(a, gauge, track, blk, ctx->stream)
                                : launch_sweep<double, double, 12>(a, gauge, track, blk, ctx->stream);
     } else if (ctx->precision == GF_MP) {
@@ -518,8 +564,24 @@ int gf_sweep(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint
     } while (0)
 
 // enqueue the reduction and the copy of the 2*Nt slice sums to pinned host memory
+#define MEASURE2(R, gauge_)                                                                                \
+    do {                                                                                                   \
+        dim3 grid((unsigned)ctx->meas_gx, (unsigned)ctx->NS, 2);                                           \
+        const int64_t cb_ = link_store_bytes(ctx);                                                         \
+        if ((gauge_) == GF_LANDAU)                                                                         \
+            measure2_kernel<R, GAUGE_LANDAU><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_); \
+        else if ((gauge_) == GF_COULOMB)                                                                   \
+            measure2_kernel<R, GAUGE_COULOMB><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_); \
+        else                                                                                               \
+            measure2_kernel<R, GAUGE_MAG><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_); \
+    } while (0)
+
 static int enqueue_measure(gf_ctx* ctx, int gauge) {
-    DISPATCH_RR(ctx, MEASURE, gauge);
+    if (ctx->nc == 2) {
+        if (ctx->real_bytes == 4) MEASURE2(float, gauge);
+        else MEASURE2(double, gauge);
+    } else
+        DISPATCH_RR(ctx, MEASURE, gauge);
     CU(cudaGetLastError());
     slice_reduce_kernel<<<ctx->NS, 128, 0, ctx->stream>>>(ctx->partial, 2 * ctx->meas_gx, ctx->NS, ctx->slice_dev);
     CU(cudaGetLastError());
@@ -533,6 +595,7 @@ static int enqueue_measure(gf_ctx* ctx, int gauge) {
 static void finish_measure(const gf_ctx* ctx, int gauge, int c, double* F, double* theta, double* theta_slice,
                            double* theta_max) {
     const int nd = (gauge == GF_COULOMB) ? 3 : 4;
+    const double ncd = (double)ctx->nc;   // N_c of Eqs. (4), (7), (11)
     const double Vs = (double)ctx->Nx * ctx->Ny * ctx->Nz;
     const double* fs_ = ctx->slice_host + (size_t)c * ctx->Nt;
     const double* th_ = ctx->slice_host + (size_t)ctx->NS + (size_t)c * ctx->Nt;
@@ -540,12 +603,12 @@ static void finish_measure(const gf_ctx* ctx, int gauge, int c, double* F, doubl
     for (int t = 0; t < ctx->Nt; ++t) {
         fs += fs_[t];
         ths += th_[t];
-        const double th_t = th_[t] / (3.0 * Vs);
+        const double th_t = th_[t] / (ncd * Vs);
         if (theta_slice) theta_slice[t] = th_t;
         if (th_t > tmax) tmax = th_t;
     }
-    if (F) *F = fs / (3.0 * nd * (double)ctx->V);
-    if (theta) *theta = ths / (3.0 * (double)ctx->V);
+    if (F) *F = fs / (ncd * nd * (double)ctx->V);
+    if (theta) *theta = ths / (ncd * (double)ctx->V);
     if (theta_max) *theta_max = tmax;
 }
 
@@ -581,6 +644,20 @@ int gf_measure(gf_ctx* ctx, int gauge, double* F, double* theta, double* theta_s
 int gf_reunitarize(gf_ctx* ctx) {
     if (!ctx) return GF_EINVAL;
     if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_reunitarize: no links set");
+    if (ctx->nc == 2) {
+        const dim3 g8((unsigned)((8 * ctx->Vh + 255) / 256), (unsigned)ctx->B), g2((unsigned)((2 * ctx->Vh + 255) / 256), (unsigned)ctx->B);
+        if (ctx->real_bytes == 4) reunit2_kernel<float><<<g8, 256, 0, ctx->stream>>>(ctx->links, ctx->Vh, 8, link_store_bytes(ctx));
+        else reunit2_kernel<double><<<g8, 256, 0, ctx->stream>>>(ctx->links, ctx->Vh, 8, link_store_bytes(ctx));
+        CU(cudaGetLastError());
+        ++ctx->launches;
+        if (ctx->gtot) {
+            if (ctx->real_bytes == 4) reunit2_kernel<float><<<g2, 256, 0, ctx->stream>>>(ctx->gtot, ctx->Vh, 2, field_store_bytes(ctx));
+            else reunit2_kernel<double><<<g2, 256, 0, ctx->stream>>>(ctx->gtot, ctx->Vh, 2, field_store_bytes(ctx));
+            CU(cudaGetLastError());
+            ++ctx->launches;
+        }
+        return GF_OK;
+    }
     DISPATCH_RR(ctx, REUNIT_LINKS, 0);
     CU(cudaGetLastError());
     ++ctx->launches;
@@ -604,7 +681,16 @@ int gf_coulomb_finalize(gf_ctx* ctx) {
     if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_coulomb_finalize: no links set");
     if (!ctx->gtot) return fail(ctx, GF_ESTATE, "gf_coulomb_finalize: context created without GF_FLAG_TRACK_TRANSFORM");
     if (!ctx->temporal_stale) return GF_OK;
-    DISPATCH_RR(ctx, FINALIZE, 0);
+    if (ctx->nc == 2) {
+        const dim3 g((unsigned)((2 * ctx->Vh + 127) / 128), (unsigned)ctx->B);
+        if (ctx->real_bytes == 4)
+            coulomb_finalize2_kernel<float><<<g, 128, 0, ctx->stream>>>(ctx->links, ctx->gtot, ctx->gapplied, dims_of(ctx),
+                                                                        link_store_bytes(ctx), field_store_bytes(ctx));
+        else
+            coulomb_finalize2_kernel<double><<<g, 128, 0, ctx->stream>>>(ctx->links, ctx->gtot, ctx->gapplied, dims_of(ctx),
+                                                                         link_store_bytes(ctx), field_store_bytes(ctx));
+    } else
+        DISPATCH_RR(ctx, FINALIZE, 0);
     CU(cudaGetLastError());
     ++ctx->launches;
     if (!ctx->gapplied) {
@@ -620,8 +706,9 @@ int gf_coulomb_finalize(gf_ctx* ctx) {
 // ---- run loops -----------------------------------------------------------------------------------
 static int sweep_gx(const gf_ctx* ctx) {
     const int Vsh = ctx->Nx * ctx->Ny * (ctx->Nz / 2);
-    const int block = (ctx->real_bytes == 4) ? sweep_block<float>(Vsh, ctx->block_override)
-                                             : sweep_block<double>(Vsh, ctx->block_override);
+    const int block = (ctx->nc == 2)           ? sweep_su2_block(Vsh, ctx->block_override)
+                      : (ctx->real_bytes == 4) ? sweep_block<float>(Vsh, ctx->block_override)
+                                               : sweep_block<double>(Vsh, ctx->block_override);
     return (Vsh + block - 1) / block;
 }
 
@@ -675,6 +762,7 @@ static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t see
     const int nunits = per_slice ? NS : B, uspan = per_slice ? 1 : Nt;   // unit u = slices [u*uspan, (u+1)*uspan)
     const int gx = sweep_gx(ctx);
     const double Vs = (double)ctx->Nx * ctx->Ny * ctx->Nz;
+    const double ncd = (double)ctx->nc;
     bool have_exact = false;
 
     // frozen slices, with the exact slice sums (F terms, theta terms) they were stopped at
@@ -695,9 +783,9 @@ static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t see
         for (int sl = lo; sl < hi; ++sl) {
             const double v = frozen[(size_t)sl] ? fz_th[(size_t)sl] : val(sl);
             tot += v;
-            if (v / (3.0 * Vs) > tmax) tmax = v / (3.0 * Vs);
+            if (v / (ncd * Vs) > tmax) tmax = v / (ncd * Vs);
         }
-        return coulomb ? tmax : tot / (3.0 * (double)ctx->V);
+        return coulomb ? tmax : tot / (ncd * (double)ctx->V);
     };
     auto freeze_unit = [&](int u, int s_now) {
         unit_frozen[(size_t)u] = 1;
@@ -724,7 +812,7 @@ static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t see
         for (int c = 0; c < B; ++c) {
             double fs = 0.0;
             for (int sl = c * Nt; sl < (c + 1) * Nt; ++sl) fs += frozen[(size_t)sl] ? fz_F[(size_t)sl] : ctx->slice_host[sl];
-            Fc[(size_t)c] = fs / (3.0 * nd * (double)ctx->V);
+            Fc[(size_t)c] = fs / (ncd * nd * (double)ctx->V);
             stopc[(size_t)c] = stop_range(c * Nt, (c + 1) * Nt, [&](int sl) { return ctx->slice_host[NS + sl]; });
         }
         have_exact = true;
@@ -815,7 +903,7 @@ static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t see
                 for (int c = 0; c < B; ++c) {
                     double fs = 0.0;
                     for (int sl = c * Nt; sl < (c + 1) * Nt; ++sl) fs += frozen[(size_t)sl] ? fz_F[(size_t)sl] : od[3 * sl];
-                    Fc[(size_t)c] = fs / (3.0 * nd * (double)ctx->V);
+                    Fc[(size_t)c] = fs / (ncd * nd * (double)ctx->V);
                     stopc[(size_t)c] = stop_range(c * Nt, (c + 1) * Nt, [&](int sl) { return od[3 * sl + 1]; });
                 }
                 for (int sl = 0; sl < NS; ++sl) pend_odd[(size_t)sl] = od[3 * sl + 1];
@@ -990,12 +1078,27 @@ int gf_random_gauge(gf_ctx* ctx, uint64_t seed) {
     char* h = nullptr;
     CU(cudaMalloc((void**)&h, (size_t)(ctx->B * field_store_bytes(ctx))));
     const dim3 g((unsigned)((ctx->V + 127) / 128), (unsigned)ctx->B);
-    if (ctx->real_bytes == 4) haar_field_kernel<float><<<g, 128, 0, ctx->stream>>>(h, dims_of(ctx), seed, field_store_bytes(ctx));
-    else haar_field_kernel<double><<<g, 128, 0, ctx->stream>>>(h, dims_of(ctx), seed, field_store_bytes(ctx));
-    cudaError_t e = cudaGetLastError();
-    if (e == cudaSuccess) {
-        DISPATCH_RR(ctx, GAUGE_APPLY, h);
+    const dim3 ga((unsigned)((ctx->Vh + 127) / 128), (unsigned)ctx->B, 2);
+    cudaError_t e;
+    if (ctx->nc == 2) {
+        if (ctx->real_bytes == 4) haar_field2_kernel<float><<<g, 128, 0, ctx->stream>>>(h, dims_of(ctx), seed, field_store_bytes(ctx));
+        else haar_field2_kernel<double><<<g, 128, 0, ctx->stream>>>(h, dims_of(ctx), seed, field_store_bytes(ctx));
         e = cudaGetLastError();
+        if (e == cudaSuccess) {
+            if (ctx->real_bytes == 4)
+                gauge_apply2_kernel<float><<<ga, 128, 0, ctx->stream>>>(ctx->links, ctx->gtot, h, dims_of(ctx), link_store_bytes(ctx), field_store_bytes(ctx));
+            else
+                gauge_apply2_kernel<double><<<ga, 128, 0, ctx->stream>>>(ctx->links, ctx->gtot, h, dims_of(ctx), link_store_bytes(ctx), field_store_bytes(ctx));
+            e = cudaGetLastError();
+        }
+    } else {
+        if (ctx->real_bytes == 4) haar_field_kernel<float><<<g, 128, 0, ctx->stream>>>(h, dims_of(ctx), seed, field_store_bytes(ctx));
+        else haar_field_kernel<double><<<g, 128, 0, ctx->stream>>>(h, dims_of(ctx), seed, field_store_bytes(ctx));
+        e = cudaGetLastError();
+        if (e == cudaSuccess) {
+            DISPATCH_RR(ctx, GAUGE_APPLY, h);
+            e = cudaGetLastError();
+        }
     }
     ctx->launches += 2;
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);

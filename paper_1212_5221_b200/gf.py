@@ -28,8 +28,9 @@ GF_LANDAU, GF_COULOMB, GF_MAG = 0, 1, 2
 GF_OR, GF_SR, GF_SA, GF_MICRO = 0, 1, 2, 3
 GF_FLAG_TRACK_TRANSFORM = 1
 GF_FLAG_FREEZE_SLICES = 2
+GF_FLAG_SU2 = 4
 
-EXPORTS = ["gf_create", "gf_create_batch", "gf_num_copies", "gf_set_links_copy", "gf_get_links_copy",
+EXPORTS = ["gf_create", "gf_num_colors", "gf_create_batch", "gf_num_copies", "gf_set_links_copy", "gf_get_links_copy",
            "gf_get_gauge_transform_copy", "gf_measure_batch", "gf_run_batch", "gf_fix", "gf_random_gauge", "gf_destroy", "gf_set_links", "gf_get_links", "gf_get_gauge_transform", "gf_sweep",
            "gf_half_sweep", "gf_measure", "gf_run", "gf_get_slice_sweeps", "gf_anneal", "gf_reunitarize", "gf_coulomb_finalize",
            "gf_sync", "gf_kernel_timing", "gf_kernel_time_ms", "gf_launch_count", "gf_device_bytes", "gf_volume", "gf_last_error", "gf_version"]
@@ -50,6 +51,7 @@ class gf_fix_params(ctypes.Structure):
 _vp, _ci, _cd, _u64, _u32 = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_uint64, ctypes.c_uint32
 _lib.gf_create_batch.argtypes = [ctypes.POINTER(_vp), _ci, _ci, _ci, _ci, _ci, _ci, _ci, ctypes.c_uint, _vp]
 _lib.gf_num_copies.argtypes = [_vp]
+_lib.gf_num_colors.argtypes = [_vp]
 _lib.gf_set_links_copy.argtypes = [_vp, _ci, _vp, _ci, _ci]
 _lib.gf_get_links_copy.argtypes = [_vp, _ci, _vp, _ci, _ci]
 _lib.gf_get_gauge_transform_copy.argtypes = [_vp, _ci, _vp, _ci, _ci]
@@ -153,11 +155,18 @@ def gf_num_copies(ctx):
     return int(_lib.gf_num_copies(ctx))
 
 
+def gf_num_colors(ctx):
+    return int(_lib.gf_num_colors(ctx))
+
+
 def gf_destroy(ctx):
     return _lib.gf_destroy(ctx)
 
 
 def _sized(ctx, n, per_site, what):
+    """per_site is given for SU(3) (72 reals of links, 18 of a transform); SU(2) matrices hold 8 reals."""
+    if gf_num_colors(ctx) == 2:
+        per_site = per_site * 8 // 18
     want = gf_volume(ctx) * per_site
     if n != want:
         raise ValueError(f"{what}: buffer holds {n} reals, the context's lattice needs {want}")
@@ -342,10 +351,12 @@ class GaugeFixer:
     """Context manager around one gf_ctx.  Methods forward to the C entry points of the same name."""
 
     def __init__(self, Nx, Ny, Nz, Nt, precision=GF_DP, recon=18, track_transform=False, cuda_stream=None,
-                 freeze_slices=False, n_copies=1):
+                 freeze_slices=False, n_copies=1, su2=False):
         self.dims = (Nx, Ny, Nz, Nt)
         self.precision, self.recon, self.n_copies = precision, recon, n_copies
-        flags = (GF_FLAG_TRACK_TRANSFORM if track_transform else 0) | (GF_FLAG_FREEZE_SLICES if freeze_slices else 0)
+        self.nc = 2 if su2 else 3
+        flags = ((GF_FLAG_TRACK_TRANSFORM if track_transform else 0) | (GF_FLAG_FREEZE_SLICES if freeze_slices else 0)
+                 | (GF_FLAG_SU2 if su2 else 0))
         self.ctx = gf_create_batch(Nx, Ny, Nz, Nt, n_copies, precision, recon, flags, cuda_stream)
 
     def close(self):
@@ -368,7 +379,7 @@ class GaugeFixer:
     @property
     def shape(self):
         Nx, Ny, Nz, Nt = self.dims
-        return (Nt, Nx, Ny, Nz, 4, 3, 3, 2)
+        return (Nt, Nx, Ny, Nz, 4, self.nc, self.nc, 2)
 
     def set_links(self, links):
         return gf_set_links(self.ctx, links)
@@ -381,7 +392,7 @@ class GaugeFixer:
 
     def get_gauge_transform(self, out=None, dtype=np.float64):
         if out is None:
-            out = np.empty(self.shape[:4] + (3, 3, 2), dtype=dtype)
+            out = np.empty(self.shape[:4] + self.shape[-3:], dtype=dtype)
         gf_get_gauge_transform(self.ctx, out)
         return out
 
@@ -424,7 +435,7 @@ class GaugeFixer:
 
     def get_gauge_transform_copy(self, copy, out=None, dtype=np.float64):
         if out is None:
-            out = np.empty(self.shape[:4] + (3, 3, 2), dtype=dtype)
+            out = np.empty(self.shape[:4] + self.shape[-3:], dtype=dtype)
         gf_get_gauge_transform_copy(self.ctx, copy, out)
         return out
 
