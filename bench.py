@@ -384,16 +384,22 @@ def run_ours(args):
                              "bytes_per_site_update": v["roofline"]["bytes_per_site_update"],
                              "kernel_share_of_step": v["kernel_share_of_step"]})
 
-    def bench_other(dims_o, gauge, prec, recon, copies, sweeps, label):
+    def bench_other(dims_o, gauge, prec, recon, copies, sweeps, label, su2=False):
         """Side measurement (not the headline): `sweeps` OR sweeps of `copies` lattices of extent dims_o."""
         ox, oy, oz, ot = dims_o
         Vo = ox * oy * oz * ot
         nd = 3 if gauge == 1 else 4
         r_o = (ot // TILE[3], ox // TILE[0], oy // TILE[1], oz // TILE[2])
+        if su2:
+            from paper_1212_5221_b200 import inputs
+            recon = 4            # reals kept per SU(2) link (first row of the matrix)
+            src_tile = inputs.as_real(inputs.make_config_su2(*TILE, TILE_EPS, *TILE_SEEDS))
+        else:
+            src_tile = tile
         with torch.cuda.stream(stream):
-            src = torch.from_numpy(tile).to(dev).repeat(*r_o, 1, 1, 1, 1).contiguous()
-        with gf.GaugeFixer(ox, oy, oz, ot, precision=PREC_NAMES[prec], recon=recon, n_copies=copies,
-                           cuda_stream=stream) as fx:
+            src = torch.from_numpy(src_tile).to(dev).repeat(*r_o, 1, 1, 1, 1).contiguous()
+        with gf.GaugeFixer(ox, oy, oz, ot, precision=PREC_NAMES[prec], recon=18 if su2 else recon, n_copies=copies,
+                           cuda_stream=stream, su2=su2) as fx:
             fx.set_links(src)
             del src
             fx.run_batch(gauge, OR, OMEGA, max_sweeps=10, eps=-1.0, check_every=10)
@@ -410,7 +416,7 @@ def run_ours(args):
         bpsu = bytes_per_site_update(prec, recon, nd)
         ach = bpsu * (copies * Vo // 2) / (kern_ms / kern_n * 1e-3) / 1e9
         store = copies * Vo * 4 * recon * (8 if prec == "dp" else 4)
-        return {"workload": label, "lattice": list(dims_o), "copies": copies, "precision": prec, "recon": recon,
+        return {"workload": label, "gauge_group": "SU(2)" if su2 else "SU(3)", "lattice": list(dims_o), "copies": copies, "precision": prec, "recon": recon,
                 "sweeps": sweeps, "value": copies * Vo * sweeps / (ms * 1e-3), "unit": "site-updates/s",
                 "avg_launch_ms": kern_ms / kern_n, "roofline_achieved_gbs": ach, "roofline_frac": ach / peak,
                 "bytes_per_site_update": bpsu, "link_store_bytes": store,
@@ -428,6 +434,9 @@ def run_ours(args):
             bench_other((16, 16, 16, 16), 0, "dp", 18, 1, 200, "Landau OR, 16^4, DP-18, one copy (configs[1])"),
             bench_other((16, 16, 16, 16), 0, "dp", 18, 64, 100, "Landau OR, 64 gauge copies of 16^4 per launch, DP-18"),
             bench_other((32, 32, 32, 32), 0, "sp", 12, 16, 100, "Landau OR, 16 gauge copies of 32^4 per launch, SP-12"),
+            bench_other((64, 64, 64, 256), 0, "sp", 4, 1, 100, "SU(2) Landau OR, 64^3x256, SP (4 reals per link)", su2=True),
+            bench_other((64, 64, 64, 256), 0, "dp", 4, 1, 100, "SU(2) Landau OR, 64^3x256, DP (4 reals per link)", su2=True),
+            bench_other((64, 64, 64, 256), 2, "mp", 4, 1, 100, "SU(2) MAG OR, 64^3x256, MP", su2=True),
         ]
 
     cpu = None

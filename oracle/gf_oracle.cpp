@@ -750,3 +750,6 @@ int gfo_num_threads(void) {
 
 // the N_c = 2 oracle uses the generator, rules and indexer defined above
 #include "gf_oracle_su2.hpp"
+
+// the input generator's oracle: Wilson-action heatbath, plaquette
+#include "gf_oracle_wilson.hpp"

@@ -27,7 +27,8 @@ OR, SR, SA, MICRO = 0, 1, 2, 3
 
 def build(force: bool = False) -> str:
     """Compile the oracle with g++ (-O2, OpenMP).  Building the checker is not using it."""
-    newest = max(os.path.getmtime(_SRC), os.path.getmtime(os.path.join(_HERE, "gf_oracle_su2.hpp")))
+    newest = max(os.path.getmtime(_SRC), os.path.getmtime(os.path.join(_HERE, "gf_oracle_su2.hpp")),
+                 os.path.getmtime(os.path.join(_HERE, "gf_oracle_wilson.hpp")))
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < newest:
         cmd = ["g++", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c++17",
                "-ffp-contract=off", "-o", _LIB, _SRC]
@@ -78,6 +79,15 @@ def lib():
         L.gfo_apply_subgroup_d.argtypes = [vp, vp, ci, ci, ci]
         L.gfo_apply_subgroup_d.restype = None
         L.gfo_num_threads.restype = ci
+        # input generator (gf_oracle_wilson.hpp)
+        L.gfo_wilson_heatbath_d.argtypes = [vp, vp, cd, u64, u32]
+        L.gfo_wilson_heatbath_f.argtypes = [vp, vp, cd, u64, u32]
+        L.gfo_plaquette_d.argtypes = [vp, vp]
+        L.gfo_plaquette_d.restype = cd
+        L.gfo_plaquette_f.argtypes = [vp, vp]
+        L.gfo_plaquette_f.restype = cd
+        L.gfo_staple_d.argtypes = [vp, vp, ci, ci, ci, ci, ci, vp]
+        L.gfo_staple_d.restype = None
         # N_c = 2 (gf_oracle_su2.hpp)
         L.gfo2_sweep_d.argtypes = [vp, vp, ci, ci, ci, cd, u64, u32, vp]
         L.gfo2_sweep_f.argtypes = [vp, vp, ci, ci, ci, cd, u64, u32, ci, vp]
@@ -366,6 +376,30 @@ def fix(links: np.ndarray, gauge: int, seed: int = 0, sa_steps: int = 0, sa_T_hi
         m = (mm["F"], stop_value(mm, gauge))
         conv = m[1] < eps
     return total, m[0], m[1], conv
+
+
+def wilson_heatbath(links: np.ndarray, beta: float, seed: int, sweep_index: int = 0) -> None:
+    """One Cabibbo-Marinari heatbath sweep of the Wilson action at coupling beta (SU(3)), in place
+    (gf_oracle_wilson.hpp): the input generator standing in for the paper's beta = 5.7 ensemble."""
+    d = _dims(links)
+    assert nc_of(links) == 3
+    fn = lib().gfo_wilson_heatbath_d if links.dtype == np.float64 else lib().gfo_wilson_heatbath_f
+    if fn(_p(links), _p(d), float(beta), seed, sweep_index) != 0:
+        raise ValueError("oracle wilson_heatbath: invalid arguments")
+
+
+def plaquette(links: np.ndarray) -> float:
+    """<Re tr U_P> / 3 over all 6 V plaquettes (SU(3))."""
+    d = _dims(links)
+    assert nc_of(links) == 3
+    return float((lib().gfo_plaquette_d if links.dtype == np.float64 else lib().gfo_plaquette_f)(_p(links), _p(d)))
+
+
+def staple(links: np.ndarray, t: int, x: int, y: int, z: int, mu: int) -> np.ndarray:
+    d = _dims(links)
+    out = np.zeros((3, 3, 2))
+    lib().gfo_staple_d(_p(links), _p(d), t, x, y, z, mu, _p(out))
+    return out
 
 
 def site_update(up: np.ndarray, dn: np.ndarray, gauge: int, algo: int, param: float, seed: int = 0,
