@@ -15,6 +15,7 @@
 #include "aux_su2.cuh"
 #include "sweep.cuh"
 #include "sweep_su2.cuh"
+#include "wilson.cuh"
 
 using namespace gf;
 
@@ -1108,6 +1109,65 @@ int gf_random_gauge(gf_ctx* ctx, uint64_t seed) {
     if (ctx->gapplied)
         CU(cudaMemcpyAsync(ctx->gapplied, ctx->gtot, (size_t)(ctx->B * field_store_bytes(ctx)), cudaMemcpyDeviceToDevice,
                            ctx->stream));
+    return GF_OK;
+}
+
+// ---- input generator: Wilson-action heatbath, plaquette ---------------------
+#define WILSON_HB(R, RECON, mu_, par_, sw_)                                                                      \
+    wilson_heatbath_kernel<R, RECON><<<dim3((unsigned)((Vsh + 127) / 128), (unsigned)ctx->NS), 128, 0, ctx->stream>>>( \
+        ctx->links, dims_of(ctx), (mu_), (par_), beta, seed, (sw_), link_store_bytes(ctx))
+
+int gf_wilson_heatbath(gf_ctx* ctx, double beta, uint64_t seed, uint32_t first_sweep_index, int n_sweeps) {
+    if (!ctx) return GF_EINVAL;
+    if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_wilson_heatbath: no links set");
+    if (ctx->nc != 3) return fail(ctx, GF_ESTATE, "gf_wilson_heatbath: SU(3) contexts only");
+    if (!(beta > 0.0) || n_sweeps < 0) return fail(ctx, GF_EINVAL, "gf_wilson_heatbath: beta = %g, n_sweeps = %d", beta, n_sweeps);
+    if (ctx->temporal_stale && ctx->gtot) {
+        int rc = gf_coulomb_finalize(ctx);
+        if (rc) return rc;
+    }
+    const int Vsh = ctx->Nx * ctx->Ny * (ctx->Nz / 2);
+    for (int k = 0; k < n_sweeps; ++k)
+        for (int mu = 0; mu < 4; ++mu)
+            for (int par = 0; par < 2; ++par) {
+                DISPATCH_RR(ctx, WILSON_HB, mu, par, first_sweep_index + (uint32_t)k);
+                CU(cudaGetLastError());
+                ++ctx->launches;
+            }
+    // a new configuration, not a gauge transform of the old one: the accumulated g(x) restarts
+    for (int c = 0; c < ctx->B && ctx->gtot; ++c) {
+        int rc = reset_transform(ctx, c);
+        if (rc) return rc;
+    }
+    return GF_OK;
+}
+
+#define PLAQUETTE(R, RECON, dummy)                                                                               \
+    plaquette_kernel<R, RECON><<<dim3((unsigned)ctx->meas_gx, (unsigned)ctx->NS, 2), ctx->meas_block, 0, ctx->stream>>>( \
+        ctx->links, dims_of(ctx), ctx->partial, link_store_bytes(ctx))
+
+int gf_plaquette(gf_ctx* ctx, double* plaq) {
+    if (!ctx) return GF_EINVAL;
+    if (!plaq) return fail(ctx, GF_EINVAL, "gf_plaquette: NULL pointer");
+    if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_plaquette: no links set");
+    if (ctx->nc != 3) return fail(ctx, GF_ESTATE, "gf_plaquette: SU(3) contexts only");
+    if (ctx->temporal_stale && ctx->gtot) {
+        int rc = gf_coulomb_finalize(ctx);
+        if (rc) return rc;
+    }
+    DISPATCH_RR(ctx, PLAQUETTE, 0);
+    CU(cudaGetLastError());
+    slice_reduce_kernel<<<ctx->NS, 128, 0, ctx->stream>>>(ctx->partial, 2 * ctx->meas_gx, ctx->NS, ctx->slice_dev);
+    CU(cudaGetLastError());
+    ctx->launches += 2;
+    CU(cudaMemcpyAsync(ctx->slice_host, ctx->slice_dev, (size_t)2 * ctx->NS * sizeof(double), cudaMemcpyDeviceToHost,
+                       ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    for (int c = 0; c < ctx->B; ++c) {
+        double tot = 0.0;
+        for (int t = 0; t < ctx->Nt; ++t) tot += ctx->slice_host[(size_t)c * ctx->Nt + t];
+        plaq[c] = tot / (3.0 * 6.0 * (double)ctx->V);
+    }
     return GF_OK;
 }
 

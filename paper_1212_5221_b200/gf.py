@@ -31,7 +31,7 @@ GF_FLAG_FREEZE_SLICES = 2
 GF_FLAG_SU2 = 4
 
 EXPORTS = ["gf_create", "gf_num_colors", "gf_create_batch", "gf_num_copies", "gf_set_links_copy", "gf_get_links_copy",
-           "gf_get_gauge_transform_copy", "gf_measure_batch", "gf_run_batch", "gf_fix", "gf_random_gauge", "gf_destroy", "gf_set_links", "gf_get_links", "gf_get_gauge_transform", "gf_sweep",
+           "gf_get_gauge_transform_copy", "gf_measure_batch", "gf_run_batch", "gf_fix", "gf_random_gauge", "gf_wilson_heatbath", "gf_plaquette", "gf_destroy", "gf_set_links", "gf_get_links", "gf_get_gauge_transform", "gf_sweep",
            "gf_half_sweep", "gf_measure", "gf_run", "gf_get_slice_sweeps", "gf_anneal", "gf_reunitarize", "gf_coulomb_finalize",
            "gf_sync", "gf_kernel_timing", "gf_kernel_time_ms", "gf_launch_count", "gf_device_bytes", "gf_volume", "gf_last_error", "gf_version"]
 
@@ -59,6 +59,8 @@ _lib.gf_measure_batch.argtypes = [_vp, _ci, _vp, _vp, _vp]
 _lib.gf_run_batch.argtypes = [_vp, _ci, _ci, _cd, _u64, _u32, _ci, _cd, _ci, _ci, _vp, _vp]
 _lib.gf_fix.argtypes = [_vp, ctypes.POINTER(gf_fix_params), _vp]
 _lib.gf_random_gauge.argtypes = [_vp, _u64]
+_lib.gf_wilson_heatbath.argtypes = [_vp, _cd, _u64, _u32, _ci]
+_lib.gf_plaquette.argtypes = [_vp, _vp]
 _lib.gf_create.argtypes = [ctypes.POINTER(_vp), _ci, _ci, _ci, _ci, _ci, _ci, ctypes.c_uint, _vp]
 _lib.gf_destroy.argtypes = [_vp]
 _lib.gf_set_links.argtypes = [_vp, _vp, _ci, _ci]
@@ -253,6 +255,17 @@ def gf_fix(ctx, gauge, seed=0, sa_steps=0, sa_T_hi=1.0, sa_T_lo=0.01, sa_micro=3
 
 def gf_random_gauge(ctx, seed):
     return _check(ctx, _lib.gf_random_gauge(ctx, seed))
+
+
+def gf_wilson_heatbath(ctx, beta, seed, first_sweep_index=0, n_sweeps=1):
+    return _check(ctx, _lib.gf_wilson_heatbath(ctx, float(beta), seed, first_sweep_index, n_sweeps))
+
+
+def gf_plaquette(ctx):
+    """-> array[n_copies] of <Re tr U_P> / 3."""
+    out = np.zeros(gf_num_copies(ctx))
+    _check(ctx, _lib.gf_plaquette(ctx, _vp(out.ctypes.data)))
+    return out
 
 
 def gf_sweep(ctx, gauge, algo, param, seed=0, sweep_index=0):
@@ -450,3 +463,9 @@ class GaugeFixer:
 
     def random_gauge(self, seed):
         return gf_random_gauge(self.ctx, seed)
+
+    def wilson_heatbath(self, beta, seed, first_sweep_index=0, n_sweeps=1):
+        return gf_wilson_heatbath(self.ctx, beta, seed, first_sweep_index, n_sweeps)
+
+    def plaquette(self):
+        return gf_plaquette(self.ctx)
