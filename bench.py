@@ -68,6 +68,8 @@ def parse_args():
     ap.add_argument("--lattice", default="64,64,64,256", help="Nx,Ny,Nz,Nt")
     ap.add_argument("--precision", default="dp", choices=list(PREC_NAMES))
     ap.add_argument("--recon", type=int, default=18, choices=[12, 18])
+    ap.add_argument("--group", default="su3", choices=["su3", "su2"],
+                    help="gauge group of the headline line (su2: side study, GF_FLAG_SU2, 4 reals per link)")
     ap.add_argument("--sweeps-per-step", type=int, default=SWEEPS_PER_STEP)
     ap.add_argument("--no-variants", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -276,10 +278,17 @@ def run_ours(args):
     lat_name = "x".join(map(str, dims))
 
     tile = make_tile()
+    su2 = args.group == "su2"
+    if su2:
+        from paper_1212_5221_b200 import inputs
+        args.recon, args.no_variants, args.no_cpu_baseline = 4, True, True
+        head_tile = inputs.as_real(inputs.make_config_su2(*TILE, TILE_EPS, *TILE_SEEDS))
+    else:
+        head_tile = tile
     reps = reps_for(dims)
     stream = torch.cuda.Stream(device=dev)
     with torch.cuda.stream(stream):
-        tile_dev = torch.from_numpy(tile).to(dev)
+        tile_dev = torch.from_numpy(head_tile).to(dev)
         links_dev = tile_dev.repeat(*reps, 1, 1, 1, 1).contiguous()     # StandardPattern, f64, in HBM
     stream.synchronize()
     del tile_dev
@@ -287,7 +296,8 @@ def run_ours(args):
     def bench_one(prec: str, recon: int, steps: int, warmup: int, e2e: bool, sample_clocks: bool):
         reunit = 100 if prec != "dp" else 0
         out = {}
-        with gf.GaugeFixer(Nx, Ny, Nz, Nt, precision=PREC_NAMES[prec], recon=recon, cuda_stream=stream) as fx:
+        with gf.GaugeFixer(Nx, Ny, Nz, Nt, precision=PREC_NAMES[prec], recon=18 if su2 else recon, cuda_stream=stream,
+                           su2=su2) as fx:
             if args.block:
                 gf.gf_debug_set_block(fx.ctx, args.block)
             fx.set_links(links_dev)
@@ -328,7 +338,8 @@ def run_ours(args):
                 "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                              "frac": achieved / peak, "frac_of_8TBps_nominal": achieved / 8000.0,
                              "traffic": NCU_TRAFFIC.get((prec, recon, lat_name)),
-                             "kernel": "gf::sweep_kernel (one half-sweep)", "peak_source": peak_src,
+                             "kernel": "gf::sweep_su2_kernel (one half-sweep)" if su2 else "gf::sweep_kernel (one half-sweep)",
+                             "peak_source": peak_src,
                              "algorithmic_bytes_per_launch": per_launch_bytes,
                              "bytes_per_site_update": bpsu, "avg_launch_ms": kern_ms / kern_n,
                              "launches_timed": kern_n},
@@ -336,7 +347,7 @@ def run_ours(args):
             if e2e:
                 eb = 8 if prec == "dp" else 4
                 tdt = torch.float64 if prec == "dp" else torch.float32
-                nbytes = V * 72 * eb
+                nbytes = V * (32 if su2 else 72) * eb
                 import psutil
                 need = 2 * nbytes * max(1, world)
                 if psutil.virtual_memory().available < 1.15 * need:
@@ -443,9 +454,9 @@ def run_ours(args):
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         links_dev = None
         torch.cuda.empty_cache()
-        r = oracle_leg(tile, args.precision, 5, 6, 1)
+        r = oracle_leg(tile, args.precision, 20, 5, 1)
         cpu = {"value": r["value"], "unit": "site-updates/s", "cores": r["cores"], "kind": "oracle",
-               "sample": f"6 x 5 Landau OR sweeps + F/theta of oracle/gf_oracle.cpp ({args.precision.upper()}) on a "
+               "sample": f"5 x 20 Landau OR sweeps + F/theta of oracle/gf_oracle.cpp ({args.precision.upper()}) on a "
                          f"{'x'.join(map(str, ORACLE_SAMPLE_DIMS))} sample (V={r['V']}) of the workload, "
                          f"{r['seconds']:.1f} s"}
 
@@ -455,7 +466,7 @@ def run_ours(args):
             "unit": "site-updates/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": DTYPE_NAMES[args.precision], "data": "synthetic",
-            "config": {"workload": f"Landau OR omega=1.7, {lat_name} (BASELINE.json configs[4]), "
+            "config": {"workload": f"{'SU(2) ' if su2 else ''}Landau OR omega=1.7, {lat_name} (BASELINE.json configs[4]), "
                                    f"{args.precision.upper()}-{args.recon}, one lattice per GPU",
                        "lattice": list(dims), "precision": args.precision, "recon": args.recon,
                        "step": f"{S} sweeps (= {2 * S} half-sweep kernels) + "
