@@ -257,6 +257,13 @@ int gf_wilson_heatbath(gf_ctx* ctx, double beta, uint64_t seed, uint32_t first_s
 int gf_plaquette(gf_ctx* ctx, double* plaq);
 
 /*
+ * gf_unitarity — the unitarity measure of Eq. (33): avg[c] = (1/4V) sum_{mu,x} |1 - det U_mu(x)| and
+ * max[c] = max_{mu,x} |1 - det U_mu(x)| for every copy c (n_copies entries each, either may be NULL), evaluated in
+ * double from the stored links (recon = 12: with the rebuilt third row).  SU(3) contexts.  Synchronous.
+ */
+int gf_unitarity(gf_ctx* ctx, double* avg, double* max);
+
+/*
  * gf_reunitarize — reproject every link (and the tracked transform) onto SU(3): Gram-Schmidt on rows
  * 0,1 in double, third row (u x v)^* (R20).  Asynchronous.
  */

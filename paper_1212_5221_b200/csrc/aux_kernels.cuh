@@ -299,6 +299,67 @@ __global__ void coulomb_finalize_kernel(char* links, const char* gtot, const cha
     global_put<R, RECON>(p0, Vh, cb, O);
 }
 
+// ---- unitarity measure of Eq. (33): |1 - det U| per link ---------------------------
+// one thread per stored link (slot = (parity, mu), cb), blockIdx.y = gauge copy; partial[(copy*gridDim.x + bx)*2]
+// = (sum, max) of the block.  With RECON = 12 the third row is the rebuilt one (what every kernel uses).
+template <class R, int RECON>
+__global__ void unitarity_kernel(const char* base, int64_t Vh, int64_t copy_bytes, double* partial) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    double dev = 0.0;
+    if (i < 8 * Vh) {
+        const char* p0 = base + blockIdx.y * copy_bytes + (i / Vh) * Layout<R, RECON>::LINK_BYTES * Vh;
+        Mat<R> m;
+        global_get<R, RECON>(p0, Vh, i % Vh, m);
+        double dr = 0.0, di = 0.0;   // det = sum_j U_0j (U_1a U_2b - U_1b U_2a), (j,a,b) cyclic
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            const int a = (j + 1) % 3, b = (j + 2) % 3;
+            const double cr = (double)m.v[RE(1, a)] * m.v[RE(2, b)] - (double)m.v[IM(1, a)] * m.v[IM(2, b)] -
+                              ((double)m.v[RE(1, b)] * m.v[RE(2, a)] - (double)m.v[IM(1, b)] * m.v[IM(2, a)]);
+            const double ci = (double)m.v[RE(1, a)] * m.v[IM(2, b)] + (double)m.v[IM(1, a)] * m.v[RE(2, b)] -
+                              ((double)m.v[RE(1, b)] * m.v[IM(2, a)] + (double)m.v[IM(1, b)] * m.v[RE(2, a)]);
+            dr += (double)m.v[RE(0, j)] * cr - (double)m.v[IM(0, j)] * ci;
+            di += (double)m.v[RE(0, j)] * ci + (double)m.v[IM(0, j)] * cr;
+        }
+        dev = sqrt((1.0 - dr) * (1.0 - dr) + di * di);
+    }
+    __shared__ double smax[32];
+    double mx = dev;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_down_sync(0xffffffffu, mx, o));
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    if (lane == 0) smax[w] = mx;
+    double zero = 0.0;
+    block_sum2(dev, zero);   // contains a __syncthreads after smax is written
+    if (threadIdx.x == 0) {
+        double m2 = 0.0;
+        for (int k = 0; k < nw; ++k) m2 = fmax(m2, smax[k]);
+        double* p = partial + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * 2;
+        p[0] = dev; p[1] = m2;
+    }
+}
+// one block per copy: out[copy*2] = sum, out[copy*2+1] = max over the copy's nblocks partials
+__global__ void unitarity_reduce_kernel(const double* partial, int nblocks, double* out) {
+    __shared__ double smax[32];
+    double s = 0.0, mx = 0.0;
+    for (int k = threadIdx.x; k < nblocks; k += blockDim.x) {
+        const double* p = partial + ((size_t)blockIdx.x * nblocks + k) * 2;
+        s += p[0];
+        mx = fmax(mx, p[1]);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_down_sync(0xffffffffu, mx, o));
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    if (lane == 0) smax[w] = mx;
+    double zero = 0.0;
+    block_sum2(s, zero);
+    if (threadIdx.x == 0) {
+        double m2 = 0.0;
+        for (int k = 0; k < nw; ++k) m2 = fmax(m2, smax[k]);
+        out[blockIdx.x * 2] = s; out[blockIdx.x * 2 + 1] = m2;
+    }
+}
+
 // ---- random start on the gauge orbit (R27) ------------------------
 // h(x) Haar-distributed on SU(3): two rows of independent complex standard normals (Box-Muller on
 // Philox uniforms, counter = (site, 0, k | 3 << 8, 0), k = 0..2, key = seed + copy), Gram-Schmidt,

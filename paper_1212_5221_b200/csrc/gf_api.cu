@@ -1171,6 +1171,41 @@ int gf_plaquette(gf_ctx* ctx, double* plaq) {
     return GF_OK;
 }
 
+// ---- unitarity measure, Eq. (33) ------------------------------------------------------------------
+int gf_unitarity(gf_ctx* ctx, double* avg, double* max) {
+    if (!ctx) return GF_EINVAL;
+    if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_unitarity: no links set");
+    if (ctx->nc != 3) return fail(ctx, GF_ESTATE, "gf_unitarity: SU(3) contexts only");
+    const int nb = (int)((8 * ctx->Vh + 255) / 256);
+    double* part = nullptr;
+    double* out = nullptr;
+    CU(cudaMalloc((void**)&part, (size_t)nb * ctx->B * 2 * sizeof(double)));
+    cudaError_t e = cudaMalloc((void**)&out, (size_t)ctx->B * 2 * sizeof(double));
+    std::vector<double> h((size_t)ctx->B * 2, 0.0);
+    if (e == cudaSuccess) {
+        const dim3 g((unsigned)nb, (unsigned)ctx->B);
+#define UNITARITY(R, RECON, dummy) unitarity_kernel<R, RECON><<<g, 256, 0, ctx->stream>>>(ctx->links, ctx->Vh, link_store_bytes(ctx), part)
+        DISPATCH_RR(ctx, UNITARITY, 0);
+#undef UNITARITY
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) {
+        unitarity_reduce_kernel<<<ctx->B, 256, 0, ctx->stream>>>(part, nb, out);
+        e = cudaGetLastError();
+        ctx->launches += 2;
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h.data(), out, h.size() * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    cudaFree(part);
+    cudaFree(out);
+    CU(e);
+    for (int c = 0; c < ctx->B; ++c) {
+        if (avg) avg[c] = h[(size_t)c * 2] / (4.0 * (double)ctx->V);
+        if (max) max[c] = h[(size_t)c * 2 + 1];
+    }
+    return GF_OK;
+}
+
 // ---- instrumentation -----------------------------------------------------------------------------
 int gf_kernel_timing(gf_ctx* ctx, int enable) {
     if (!ctx) return GF_EINVAL;

@@ -31,7 +31,7 @@ GF_FLAG_FREEZE_SLICES = 2
 GF_FLAG_SU2 = 4
 
 EXPORTS = ["gf_create", "gf_num_colors", "gf_create_batch", "gf_num_copies", "gf_set_links_copy", "gf_get_links_copy",
-           "gf_get_gauge_transform_copy", "gf_measure_batch", "gf_run_batch", "gf_fix", "gf_random_gauge", "gf_wilson_heatbath", "gf_plaquette", "gf_destroy", "gf_set_links", "gf_get_links", "gf_get_gauge_transform", "gf_sweep",
+           "gf_get_gauge_transform_copy", "gf_measure_batch", "gf_run_batch", "gf_fix", "gf_random_gauge", "gf_wilson_heatbath", "gf_plaquette", "gf_unitarity", "gf_destroy", "gf_set_links", "gf_get_links", "gf_get_gauge_transform", "gf_sweep",
            "gf_half_sweep", "gf_measure", "gf_run", "gf_get_slice_sweeps", "gf_anneal", "gf_reunitarize", "gf_coulomb_finalize",
            "gf_sync", "gf_kernel_timing", "gf_kernel_time_ms", "gf_launch_count", "gf_device_bytes", "gf_volume", "gf_last_error", "gf_version"]
 
@@ -61,6 +61,7 @@ _lib.gf_fix.argtypes = [_vp, ctypes.POINTER(gf_fix_params), _vp]
 _lib.gf_random_gauge.argtypes = [_vp, _u64]
 _lib.gf_wilson_heatbath.argtypes = [_vp, _cd, _u64, _u32, _ci]
 _lib.gf_plaquette.argtypes = [_vp, _vp]
+_lib.gf_unitarity.argtypes = [_vp, _vp, _vp]
 _lib.gf_create.argtypes = [ctypes.POINTER(_vp), _ci, _ci, _ci, _ci, _ci, _ci, ctypes.c_uint, _vp]
 _lib.gf_destroy.argtypes = [_vp]
 _lib.gf_set_links.argtypes = [_vp, _vp, _ci, _ci]
@@ -268,6 +269,14 @@ def gf_plaquette(ctx):
     return out
 
 
+def gf_unitarity(ctx):
+    """-> (avg[n_copies], max[n_copies]) of |1 - det U| (Eq. (33))."""
+    B = gf_num_copies(ctx)
+    a, m = np.zeros(B), np.zeros(B)
+    _check(ctx, _lib.gf_unitarity(ctx, _vp(a.ctypes.data), _vp(m.ctypes.data)))
+    return a, m
+
+
 def gf_sweep(ctx, gauge, algo, param, seed=0, sweep_index=0):
     return _check(ctx, _lib.gf_sweep(ctx, gauge, algo, float(param), seed, sweep_index))
 
@@ -469,3 +478,6 @@ class GaugeFixer:
 
     def plaquette(self):
         return gf_plaquette(self.ctx)
+
+    def unitarity(self):
+        return gf_unitarity(self.ctx)
