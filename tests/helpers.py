@@ -85,3 +85,15 @@ def to_real(c, dtype=np.float64):
     out[..., 0] = c.real
     out[..., 1] = c.imag
     return out
+
+
+def paper_values():
+    """The numbers printed in the paper that tests compare against (tests/golden/paper_printed_values.txt)."""
+    import os
+    out = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "paper_printed_values.txt")) as fh:
+        for line in fh:
+            line = line.split("#")[0].split()
+            if len(line) == 2:
+                out[line[0]] = float(line[1])
+    return out

@@ -74,8 +74,13 @@ def test_bytes_model_matches_the_papers_counts():
     # 8 links x 18 (12) reals x 4 B = 576 (384) B loaded per site in SP, the same stored
     sys.path.insert(0, ROOT)
     import bench
-    assert bench.bytes_per_site_update("sp", 18) == 2 * 576
-    assert bench.bytes_per_site_update("sp", 12) == 2 * 384
+    from tests.helpers import paper_values
+    pv = paper_values()
+    assert bench.bytes_per_site_update("sp", 18) == 2 * pv["bytes_loaded_per_site_sp_18"] == 2 * 576
+    assert bench.bytes_per_site_update("sp", 12) == 2 * pv["bytes_loaded_per_site_sp_12"] == 2 * 384
+    # App. A flop model used for paper_gflops
+    assert pv["flop_gather_landau"] + pv["flop_or_update"] + pv["flop_apply"] == pv["flop_per_site_landau_or"] == 2274
+    assert pv["flop_apply"] == 3 * 8 * pv["flop_per_link_subgroup"]
     assert bench.bytes_per_site_update("dp", 18) == 2304
     assert bench.bytes_per_site_update("sp", 12, nd=3) == 576
     line = json.dumps({"ok": True})

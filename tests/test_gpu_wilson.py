@@ -7,6 +7,7 @@ import numpy as np
 import pytest
 
 from paper_1212_5221_b200 import inputs
+from tests.helpers import paper_values
 
 pytestmark = pytest.mark.gpu
 LANDAU, COULOMB, MAG = 0, 1, 2
@@ -103,20 +104,24 @@ def test_table4_in_miniature(gf, oracle):
         conf = g1.get_links()
     del cold
     assert abs(P - 0.549) < 0.002
+    pv = paper_values()
     F = {}
-    for name, kw in (("sa", dict(sa_steps=2000, sa_T_hi=1.45, sa_T_lo=0.01, sa_micro=3, sr_max_sweeps=2000, sr_p=0.5)),
+    for name, kw in (("sa", dict(sa_steps=int(pv["table4_sa_steps"]), sa_T_hi=1.45, sa_T_lo=0.01,
+                                 sa_micro=int(pv["table4_micro_per_step"]), sr_max_sweeps=int(pv["table4_sr_max"]), sr_p=0.5)),
                      ("or", dict())):
         with gf.GaugeFixer(*dims, precision=DP, n_copies=B) as fx:
             fx.set_links(conf)
             fx.random_gauge(99)
             F0 = fx.measure_batch(MAG)[0]
             assert np.abs(F0 - 1 / 3).max() < 2e-3            # Haar-rotated links: E |U_ii|^2 = 1/3
-            res = fx.fix(MAG, seed=1234, or_omega=1.35, or_max_sweeps=60000, eps=1e-12, check_every=20, **kw)
+            res = fx.fix(MAG, seed=1234, or_omega=pv["table4_omega"], or_max_sweeps=60000, eps=pv["table4_eps"],
+                         check_every=20, **kw)
             assert all(r["converged"] for r in res)
             assert np.abs(fx.plaquette() - P).max() < 1e-10   # still the same orbit (rounding of ~10^4 sweeps)
             F[name] = np.array([r["F"] for r in res])
             if name == "sa":
                 assert all(r["sweeps"] >= 8000 for r in res)
+    assert pv["table4_F_sa_sr_or"] > pv["table4_F_or"] and pv["table4_F_spread_sa_sr_or"] < pv["table4_F_spread_or"]
     assert F["sa"].min() > F["or"].max()                      # Table 4: higher functional ...
     assert F["sa"].std() < 10 * F["or"].std() + 1e-4          # ... and no larger a spread
     assert 0.70 < F["or"].mean() < 0.85
