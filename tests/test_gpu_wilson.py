@@ -125,3 +125,32 @@ def test_table4_in_miniature(gf, oracle):
     assert F["sa"].min() > F["or"].max()                      # Table 4: higher functional ...
     assert F["sa"].std() < 10 * F["or"].std() + 1e-4          # ... and no larger a spread
     assert 0.70 < F["or"].mean() < 0.85
+
+
+def test_fig8_in_miniature(gf):
+    # PAPER.md:578-592 (Sec. 6.6, Fig. 8, Eq. (34)): Landau Gribov copies from random starts on the gauge orbit of a
+    # beta = 5.7 configuration; simulated annealing (T: 4 -> 1e-4, 3 microcanonical sweeps per step) before the
+    # overrelaxation to theta < 1e-10 "increases the chance to find the global maximum": the copies reached with
+    # annealing have a smaller relative deviation F_rel from the best functional of all runs.  16^4, 8 starts,
+    # 0 vs 3000 annealing steps.
+    pv = paper_values()
+    dims = (16, 16, 16, 16)
+    B = 8
+    cold = inputs.as_real(np.broadcast_to(np.eye(3, dtype=np.complex128), (16, 16, 16, 16, 4, 3, 3)).copy())
+    with gf.GaugeFixer(*dims, precision=DP) as g1:
+        g1.set_links(cold)
+        g1.wilson_heatbath(5.7, seed=88, n_sweeps=200)
+        conf = g1.get_links()
+    F = {}
+    for steps in (0, int(pv["fig8_sa_steps_mid"])):
+        with gf.GaugeFixer(*dims, precision=DP, n_copies=B) as fx:
+            fx.set_links(conf)
+            fx.random_gauge(17)
+            res = fx.fix(LANDAU, seed=3, sa_steps=steps, sa_T_hi=pv["fig8_T_hi"], sa_T_lo=pv["fig8_T_lo"], sa_micro=3,
+                         or_omega=1.7, or_max_sweeps=40000, eps=pv["fig8_eps"], check_every=10)
+            assert all(r["converged"] for r in res)
+            F[steps] = np.array([r["F"] for r in res])
+    Fmax = max(F[0].max(), F[3000].max())
+    rel0, rel1 = (Fmax - F[0]) / Fmax, (Fmax - F[3000]) / Fmax          # Eq. (34)
+    assert rel1.mean() < rel0.mean() and F[3000].max() >= F[0].max()
+    assert len(set(np.round(F[0], 9))) > 1                              # several distinct Gribov copies without annealing
