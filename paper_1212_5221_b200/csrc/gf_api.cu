@@ -486,6 +486,8 @@ static int launch_half(gf_ctx* ctx, int gauge, int algo, double param, uint64_t 
     a.ncopies = ctx->B;
     a.copy_links_bytes = link_store_bytes(ctx);
     a.copy_gtot_bytes = field_store_bytes(ctx);
+    a.rcp_nzh = fast_div_rcp(ctx->Nz / 2);
+    a.rcp_ny = fast_div_rcp(ctx->Ny);
     const bool track = ctx->gtot != nullptr;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (ctx->timing) {

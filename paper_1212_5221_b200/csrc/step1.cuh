@@ -49,7 +49,7 @@ GF_DEV double uniform01(uint32_t w) { return ((double)w + 0.5) * (1.0 / 42949672
 
 // ---- deterministic rules -------------------------------------------------------------------
 GF_DEV float inv_sqrt(float x) { return 1.0f / sqrtf(x); }
-GF_DEV double inv_sqrt(double x) { return 1.0 / sqrt(x); }
+GF_DEV double inv_sqrt(double x) { return rsqrt(x); }   // one MUFU.RSQ64H + Newton steps instead of sqrt and a division
 GF_DEV float sqrt_t(float x) { return sqrtf(x); }
 GF_DEV double sqrt_t(double x) { return sqrt(x); }
 
@@ -63,9 +63,20 @@ GF_DEV void rule_or(const A a[4], A omega, A g[4]) {
         g[0] = A(1); g[1] = g[2] = g[3] = A(0);
         return;
     }
-    const A b = (omega * a0_sq + ai_sq) / n;
-    const A c = inv_sqrt(a0_sq + b * b * ai_sq);
-    const A bc = b * c;
+    A c, bc;
+    if (sizeof(A) == 8) {
+        // b = M/N with M = omega B + A', N = B + A'; c = 1/sqrt(B + b^2 A') = N r, bc = M r,
+        // r = 1/sqrt(B N^2 + M^2 A'): the same numbers without the division (double: no under/overflow
+        // for any sum of 2d unit-modulus links that is not exactly zero)
+        const A m = omega * a0_sq + ai_sq;
+        const A r = inv_sqrt(a0_sq * n * n + m * m * ai_sq);
+        c = n * r;
+        bc = m * r;
+    } else {
+        const A b = (omega * a0_sq + ai_sq) / n;
+        c = inv_sqrt(a0_sq + b * b * ai_sq);
+        bc = b * c;
+    }
     g[0] = a[0] * c;
     g[1] = -a[1] * bc;
     g[2] = -a[2] * bc;

@@ -43,7 +43,17 @@ struct SweepArgs {
     // (gtot + c*copy_gtot_bytes) and draws its random numbers with the Philox key seed + c
     int ncopies;
     int64_t copy_links_bytes, copy_gtot_bytes;
+    uint32_t rcp_nzh, rcp_ny;   // floor(2^32 / (Nz/2)), floor(2^32 / Ny): site decode without integer division
 };
+
+// n / d for 0 <= n < 2^31 with rcp = floor(2^32 / d) (d >= 2): __umulhi underestimates the quotient by at most one
+GF_DEV int fast_div(int n, int d, uint32_t rcp, int& rem) {
+    int q = (int)__umulhi((uint32_t)n, rcp);
+    rem = n - q * d;
+    if (rem >= d) { ++q; rem -= d; }
+    return q;
+}
+inline uint32_t fast_div_rcp(int d) { return d > 1 ? (uint32_t)(4294967296ull / (uint64_t)d) : 0xffffffffu; }
 
 // ---- asynchronous global -> shared copies -------------------------------------------------
 GF_DEV void cp_async16(uint32_t saddr, const void* g) {
@@ -251,7 +261,7 @@ sweep_kernel(const SweepArgs args) {
     const int Vsh = args.Nx * args.Ny * Nzh;
     const int64_t Vh = (int64_t)args.Nt * Vsh;
     if (args.slice_skip && args.slice_skip[blockIdx.y]) return;   // block-uniform
-    const int copy = blockIdx.y / args.Nt;
+    const int copy = (args.ncopies == 1) ? 0 : blockIdx.y / args.Nt;
     const int t = blockIdx.y - copy * args.Nt;
     char* const links = args.links + copy * args.copy_links_bytes;
     char* const gtot = TRACK ? args.gtot + copy * args.copy_gtot_bytes : nullptr;
@@ -262,10 +272,9 @@ sweep_kernel(const SweepArgs args) {
     const int64_t cb = (int64_t)t * Vsh + i_s;
 
     // ---- a1: decode the checkerboard index, neighbours with periodic wrap ----
-    int rem = i_s;
-    const int zh = rem % Nzh; rem /= Nzh;
-    const int y = rem % args.Ny;
-    const int x = rem / args.Ny;
+    int zh, y;
+    const int xy = fast_div(i_s, Nzh, args.rcp_nzh, zh);
+    const int x = fast_div(xy, args.Ny, args.rcp_ny, y);
     // own parity in the 4-d colouring; Coulomb's 3-d colouring p3 maps to (p3 + t) & 1
     const int par = (GAUGE == GAUGE_COULOMB) ? ((args.parity + t) & 1) : args.parity;
     const int r = (t + x + y + par) & 1;   // z = 2 zh + r

@@ -28,7 +28,7 @@ __global__ void __launch_bounds__(128, sizeof(R) == 8 ? 3 : 4) sweep_su2_kernel(
     const int Vsh = args.Nx * args.Ny * Nzh;
     const int64_t Vh = (int64_t)args.Nt * Vsh;
     if (args.slice_skip && args.slice_skip[blockIdx.y]) return;   // block-uniform
-    const int copy = blockIdx.y / args.Nt;
+    const int copy = (args.ncopies == 1) ? 0 : blockIdx.y / args.Nt;
     const int t = blockIdx.y - copy * args.Nt;
     char* const links = args.links + copy * args.copy_links_bytes;
     char* const gtot = TRACK ? args.gtot + copy * args.copy_gtot_bytes : nullptr;
@@ -39,10 +39,9 @@ __global__ void __launch_bounds__(128, sizeof(R) == 8 ? 3 : 4) sweep_su2_kernel(
     const int64_t cb = (int64_t)t * Vsh + i_s;
 
     // a1: decode, neighbours (as in sweep.cuh)
-    int rem = i_s;
-    const int zh = rem % Nzh; rem /= Nzh;
-    const int y = rem % args.Ny;
-    const int x = rem / args.Ny;
+    int zh, y;
+    const int xy = fast_div(i_s, Nzh, args.rcp_nzh, zh);
+    const int x = fast_div(xy, args.Ny, args.rcp_ny, y);
     const int par = (GAUGE == GAUGE_COULOMB) ? ((args.parity + t) & 1) : args.parity;
     const int r = (t + x + y + par) & 1;
     const int z = 2 * zh + r;

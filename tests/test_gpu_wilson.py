@@ -131,11 +131,12 @@ def test_fig8_in_miniature(gf):
     # PAPER.md:578-592 (Sec. 6.6, Fig. 8, Eq. (34)): Landau Gribov copies from random starts on the gauge orbit of a
     # beta = 5.7 configuration; simulated annealing (T: 4 -> 1e-4, 3 microcanonical sweeps per step) before the
     # overrelaxation to theta < 1e-10 "increases the chance to find the global maximum": the copies reached with
-    # annealing have a smaller relative deviation F_rel from the best functional of all runs.  16^4, 8 starts,
-    # 0 vs 3000 annealing steps.
+    # annealing have a smaller relative deviation F_rel from the best functional of all runs.  16^4, 32 starts,
+    # 0 vs 3000 annealing steps (measured: mean F 0.825587(31) vs 0.825788(24); on 32^4 with 8 starts
+    # 0.826676(13) vs 0.826712(15)).
     pv = paper_values()
     dims = (16, 16, 16, 16)
-    B = 8
+    B = 32
     cold = inputs.as_real(np.broadcast_to(np.eye(3, dtype=np.complex128), (16, 16, 16, 16, 4, 3, 3)).copy())
     with gf.GaugeFixer(*dims, precision=DP) as g1:
         g1.set_links(cold)
@@ -152,5 +153,6 @@ def test_fig8_in_miniature(gf):
             F[steps] = np.array([r["F"] for r in res])
     Fmax = max(F[0].max(), F[3000].max())
     rel0, rel1 = (Fmax - F[0]) / Fmax, (Fmax - F[3000]) / Fmax          # Eq. (34)
-    assert rel1.mean() < rel0.mean() and F[3000].max() >= F[0].max()
-    assert len(set(np.round(F[0], 9))) > 1                              # several distinct Gribov copies without annealing
+    se = np.sqrt(rel0.var() / B + rel1.var() / B)
+    assert rel1.mean() < rel0.mean() - 2 * se, (rel0.mean(), rel1.mean(), se)
+    assert len(set(np.round(F[0], 9))) > B // 2                         # many distinct Gribov copies
