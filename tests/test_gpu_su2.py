@@ -182,3 +182,38 @@ def test_large_lattice_tiled(gf, oracle, prec):
     assert (out.to(torch.float64) - want.to(torch.float64)).abs().max().item() <= TOL[prec]
     rel = 1e-12 if prec == DP else 2e-6
     assert F == pytest.approx(m["F"], rel=rel, abs=rel) and th == pytest.approx(m["theta"], rel=10 * rel)
+
+
+def test_su3_only_calls_refuse_su2_contexts_and_bad_arguments(gf):
+    dims = (4, 4, 4, 4)
+    L = make(dims)
+    with gf.GaugeFixer(*dims, precision=DP, su2=True) as fx:
+        fx.set_links(L)
+        for call in (lambda: fx.wilson_heatbath(5.7, 1), lambda: fx.plaquette(), lambda: fx.unitarity()):
+            with pytest.raises(gf.GfError) as e:
+                call()
+            assert e.value.code == gf.GF_ESTATE
+        for kw in (dict(check_every=0), dict(sa_steps=-1), dict(or_omega=2.5), dict(sa_steps=2, sa_T_lo=0.0)):
+            with pytest.raises(gf.GfError) as e:
+                fx.fix(LANDAU, **kw)
+            assert e.value.code == gf.GF_EINVAL
+        with pytest.raises(gf.GfError):
+            fx.sweep(LANDAU, OR, 2.0)
+
+
+def test_three_dimensional_lattices_are_coulomb_slices(gf, oracle):
+    # d = 3 ("3+1 dimensional" in the paper's abstract): a stack of N_t independent three-dimensional SU(2)
+    # lattices is fixed to the 3-d Landau gauge by GF_COULOMB, one lattice per time-slice; with
+    # GF_FLAG_FREEZE_SLICES every lattice stops on its own theta
+    dims = (6, 6, 6, 4)
+    L = make(dims, eps=0.4, seed=970)
+    with gf.GaugeFixer(*dims, precision=DP, su2=True, freeze_slices=True) as fx:
+        fx.set_links(L)
+        r = fx.run(COULOMB, OR, 1.6, max_sweeps=4000, eps=1e-12, check_every=2)
+        sw = fx.slice_sweeps()
+        F, th, ths = fx.measure(COULOMB, slices=True)
+    ref = L.copy()
+    s, Fo, tho, hist, conv, sl = oracle.run_coulomb_freeze(ref, OR, 1.6, max_sweeps=4000, eps=1e-12, check_every=2)
+    assert conv and r["converged"] and ths.max() < 1e-12
+    assert np.all(np.abs(sw - sl) <= 2) and abs(r["F"] - Fo) <= 1e-10
+    assert len(set(sw.tolist())) > 1
