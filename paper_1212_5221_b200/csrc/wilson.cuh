@@ -59,8 +59,11 @@ GF_DEV void wilson_subgroup(Mat<R>& W, Mat<R>& U, double T, uint64_t seed, uint3
 }
 
 // grid = (ceil(Vsh / block), ncopies * Nt); links U_mu(x) for x of parity `parity`
+#ifndef GF_HB_MIN_CTAS
+#define GF_HB_MIN_CTAS 2
+#endif
 template <class R, int RECON>
-__global__ void __launch_bounds__(128) wilson_heatbath_kernel(char* links_all, Dims d, int mu, int parity, double beta,
+__global__ void __launch_bounds__(128, GF_HB_MIN_CTAS) wilson_heatbath_kernel(char* links_all, Dims d, int mu, int parity, double beta,
                                                               uint64_t seed0, uint32_t sweep_index, int64_t copy_bytes) {
     typedef Layout<R, RECON> L;
     const int Nzh = d.Nz >> 1;
