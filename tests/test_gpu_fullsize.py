@@ -63,6 +63,7 @@ def max_diff_against_tiling(torch, out_dev, ref_tile_dev, r):
     ((64, 64, 64, 256), SP, 18, LANDAU),
     ((64, 64, 64, 256), DP, 12, LANDAU),
     ((64, 64, 64, 256), MP, 12, LANDAU),
+    ((96, 96, 96, 192), SP, 12, LANDAU),      # 1.7e8 sites: the largest lattice whose in/out buffers also fit in 180 GB
     ((32, 32, 32, 64), SP, 12, COULOMB),      # BASELINE.json configs[2]
     ((32, 32, 32, 64), DP, 18, MAG),
 ])
