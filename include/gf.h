@@ -1,5 +1,5 @@
 /*
- * gf.h — C ABI of libgf.so: SU(3) lattice gauge fixing by checkerboard local updates on one B200.
+ * gf.h — C ABI of libgf.so: SU(3) (and SU(2)) lattice gauge fixing by checkerboard local updates on one B200.
  *
  * The operations are those of Schroeck & Vogt, "Coulomb, Landau and Maximally Abelian Gauge Fixing
  * in Lattice QCD with Multi-GPUs" (arxiv 1212.5221; line numbers below refer to the text of the
@@ -12,10 +12,12 @@
  *     the last error (valid until the next call on that ctx).
  *   - A context owns all of its device memory.  The caller owns every pointer it passes in; the
  *     library never keeps a caller pointer beyond the call.
+ *   - A context holds one lattice (gf_create) or n_copies lattices of the same extents (gf_create_batch), of
+ *     the gauge group SU(3) or, with GF_FLAG_SU2, SU(2).
  *   - One context per stream, not thread-safe.  Kernels are enqueued on the cudaStream_t given to
- *     gf_create (NULL = the legacy default stream).  gf_set_links, gf_get_*, gf_measure, gf_run and
- *     gf_anneal(with history) synchronise that stream before returning; gf_sweep, gf_half_sweep,
- *     gf_reunitarize and gf_coulomb_finalize only enqueue.
+ *     gf_create (NULL = the legacy default stream).  gf_set_links, gf_get_*, gf_measure*, gf_run*, gf_fix,
+ *     gf_random_gauge, gf_plaquette and gf_unitarity synchronise that stream before returning; gf_sweep,
+ *     gf_half_sweep, gf_anneal, gf_wilson_heatbath, gf_reunitarize and gf_coulomb_finalize only enqueue.
  *   - Host-side link layout ("StandardPattern", Sec. 4.2.1; mu = 0 is the temporal
  *     direction): links[t][x][y][z][mu][i][j][c], c = 0 real / 1 imaginary, i.e. real
  *     offset ((((((t*Nx + x)*Ny + y)*Nz + z)*4 + mu)*3 + i)*3 + j)*2 + c.  mu = 1,2,3 are x,y,z.
