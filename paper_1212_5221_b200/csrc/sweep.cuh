@@ -236,13 +236,19 @@ GF_DEV double warp_sum_d(double v) {
 }
 
 // ---- the kernel ----------------------------------------------------------------------------
+#ifndef GF_SP_BLOCK
+#define GF_SP_BLOCK 128     // CTA size of the float-storage kernels
+#endif
+#ifndef GF_SP_MIN_CTAS
+#define GF_SP_MIN_CTAS 3
+#endif
 #ifndef GF_MIN_CTAS_MP
 #define GF_MIN_CTAS_MP 4
 #endif
 template <class R, class A = R>
 struct SweepLaunch {   // CTA shape per storage type
-    static constexpr int MAX_BLOCK = sizeof(R) == 4 ? 128 : 64;
-    static constexpr int MIN_CTAS = (sizeof(R) == 4 && sizeof(A) == 8) ? GF_MIN_CTAS_MP : 3;
+    static constexpr int MAX_BLOCK = sizeof(R) == 4 ? GF_SP_BLOCK : 64;
+    static constexpr int MIN_CTAS = (sizeof(R) == 4 && sizeof(A) == 8) ? GF_MIN_CTAS_MP : (sizeof(R) == 4 ? GF_SP_MIN_CTAS : 3);
 };
 
 template <class R, class A, int RECON, int GAUGE, bool STOCH, bool TRACK, bool RED>
