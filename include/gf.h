@@ -14,6 +14,8 @@
  *     library never keeps a caller pointer beyond the call.
  *   - A context holds one lattice (gf_create) or n_copies lattices of the same extents (gf_create_batch), of
  *     the gauge group SU(3) or, with GF_FLAG_SU2, SU(2).
+ *   - A context lives on the CUDA device that is current when it is created; the caller keeps that device
+ *     current for every later call on the context.
  *   - One context per stream, not thread-safe.  Kernels are enqueued on the cudaStream_t given to
  *     gf_create (NULL = the legacy default stream).  gf_set_links, gf_get_*, gf_measure*, gf_run*, gf_fix,
  *     gf_random_gauge, gf_plaquette and gf_unitarity synchronise that stream before returning; gf_sweep,

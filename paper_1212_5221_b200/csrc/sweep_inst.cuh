@@ -14,13 +14,17 @@ static cudaError_t launch_one(const SweepArgs& args, int block, cudaStream_t str
     block = sweep_block<R>(Vsh, block);
     // the slice stride is the maximal CTA size whatever the block (sweep.cuh, smem_get)
     const size_t smem = (size_t)SweepLaunch<R, A>::MAX_BLOCK * 2 * ND * Layout<R, RECON>::LINK_BYTES;
-    static size_t smem_set = 0;   // per instantiation
-    if (smem > smem_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    // function attributes are per device: remember what was set for this instantiation on each device
+    static size_t smem_set[64] = {0};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64 || smem > smem_set[dev]) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
         if (e != cudaSuccess) return e;
-        smem_set = smem;
+        if (dev >= 0 && dev < 64) smem_set[dev] = smem;
     }
     const dim3 grid((unsigned)((Vsh + block - 1) / block), (unsigned)(args.ncopies * args.Nt));
     kern<<<grid, block, smem, stream>>>(args);
