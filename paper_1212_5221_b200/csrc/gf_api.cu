@@ -69,6 +69,7 @@ struct gf_ctx {
     size_t staging_bytes;
     int64_t device_bytes;
     int block_override;     // 0 = default CTA size
+    int pdl;                // half-sweeps launched with programmatic stream serialization (default 1)
     // kernel timing (gf_kernel_timing)
     bool timing;
     std::vector<cudaEvent_t> ev;   // pairs (start, stop)
@@ -166,7 +167,7 @@ int gf_create_batch(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int n_copies, 
     ctx->fused = 1;
     ctx->skip_dev = nullptr; ctx->skip_host = nullptr; ctx->have_slice_sweeps = false;
     ctx->staging = nullptr; ctx->staging_bytes = 0;
-    ctx->device_bytes = 0; ctx->block_override = 0;
+    ctx->device_bytes = 0; ctx->block_override = 0; ctx->pdl = 1;
     ctx->timing = false; ctx->ev_used = 0; ctx->launches = 0;
     ctx->err[0] = 0;
 
@@ -488,6 +489,7 @@ static int launch_half(gf_ctx* ctx, int gauge, int algo, double param, uint64_t 
     a.copy_gtot_bytes = field_store_bytes(ctx);
     a.rcp_nzh = fast_div_rcp(ctx->Nz / 2);
     a.rcp_ny = fast_div_rcp(ctx->Ny);
+    a.pdl = ctx->pdl;
     const bool track = ctx->gtot != nullptr;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (ctx->timing) {
@@ -1241,6 +1243,13 @@ int gf_launch_count(gf_ctx* ctx, int64_t* launches, int reset) {
 int gf_debug_set_fused(gf_ctx* ctx, int fused) {
     if (!ctx) return GF_EINVAL;
     ctx->fused = fused != 0;
+    return GF_OK;
+}
+
+// tuning hook (not declared in gf.h): 0 = half-sweeps launched without programmatic dependent launch
+int gf_debug_set_pdl(gf_ctx* ctx, int pdl) {
+    if (!ctx) return GF_EINVAL;
+    ctx->pdl = pdl != 0;
     return GF_OK;
 }
 

@@ -44,7 +44,16 @@ struct SweepArgs {
     int ncopies;
     int64_t copy_links_bytes, copy_gtot_bytes;
     uint32_t rcp_nzh, rcp_ny;   // floor(2^32 / (Nz/2)), floor(2^32 / Ny): site decode without integer division
+    int pdl;                    // launch with programmatic stream serialization (host side only)
 };
+
+// Programmatic dependent launch (sm_90+): a half-sweep lets the next kernel in the stream be scheduled as soon as
+// all of its own CTAs have started (launch_dependents), and touches no link before the previous kernel has
+// completed and flushed (wait).  The next half-sweep's CTAs thus fill the SMs that the tail of this one leaves
+// idle and have their site decode done when the data dependency resolves: the inter-kernel bubble that
+// dominates small lattices shrinks.  Without the launch attribute both instructions are no-ops.
+GF_DEV void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+GF_DEV void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 // n / d for 0 <= n < 2^31 with rcp = floor(2^32 / d) (d >= 2): __umulhi underestimates the quotient by at most one
 GF_DEV int fast_div(int n, int d, uint32_t rcp, int& rem) {
@@ -263,10 +272,11 @@ sweep_kernel(const SweepArgs args) {
     // grid = (ceil(Vsh / block), ncopies*Nt): blockIdx.y is (gauge copy, time-slice), so a CTA never
     // straddles slices (per-slice reductions, frozen slices).  Threads past the end of the slice redo
     // the last site without storing, so that every thread reaches the block reduction.
+    pdl_launch_dependents();
     const int Nzh = args.Nz >> 1;
     const int Vsh = args.Nx * args.Ny * Nzh;
     const int64_t Vh = (int64_t)args.Nt * Vsh;
-    if (args.slice_skip && args.slice_skip[blockIdx.y]) return;   // block-uniform
+    if (args.slice_skip && args.slice_skip[blockIdx.y]) return;   // block-uniform (flags are set by the host between runs of kernels)
     const int copy = (args.ncopies == 1) ? 0 : blockIdx.y / args.Nt;
     const int t = blockIdx.y - copy * args.Nt;
     char* const links = args.links + copy * args.copy_links_bytes;
@@ -305,6 +315,7 @@ sweep_kernel(const SweepArgs args) {
     const int64_t lstride = (int64_t)L::LINK_BYTES * Vh;
     char* const up0 = links + L::link_offset(par, MU0, Vh);        // U_mu(x): own parity
     char* const dn0 = links + L::link_offset(1 - par, MU0, Vh);    // U_mu(x - mu): other parity
+    pdl_wait();   // nothing of the previous kernel's output is read above this line
     {
         const char* pu = up0;
         const char* pd = dn0;
@@ -432,6 +443,22 @@ inline int sweep_block(int Vsh, int block_override) {
     if (block <= 0 || block > SweepLaunch<R>::MAX_BLOCK) block = SweepLaunch<R>::MAX_BLOCK;
     const int need = ((Vsh + 31) / 32) * 32;
     return block < need ? block : need;
+}
+
+// launch a half-sweep kernel, with the programmatic-stream-serialization attribute when args.pdl is set
+template <class K>
+inline cudaError_t launch_with_pdl(K kern, dim3 grid, dim3 block, size_t smem, cudaStream_t stream, const SweepArgs& args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = args.pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, args);
 }
 
 // host-side launcher of one (R, A, RECON) family; defined in sweep_inst.cuh

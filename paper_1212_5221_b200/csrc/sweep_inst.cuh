@@ -27,8 +27,7 @@ static cudaError_t launch_one(const SweepArgs& args, int block, cudaStream_t str
         if (dev >= 0 && dev < 64) smem_set[dev] = smem;
     }
     const dim3 grid((unsigned)((Vsh + block - 1) / block), (unsigned)(args.ncopies * args.Nt));
-    kern<<<grid, block, smem, stream>>>(args);
-    return cudaGetLastError();
+    return launch_with_pdl(kern, grid, dim3((unsigned)block), smem, stream, args);
 }
 
 template <class R, class A, int RECON, int GAUGE>

@@ -24,6 +24,7 @@ __global__ void __launch_bounds__(128, sizeof(R) == 8 ? 3 : 4) sweep_su2_kernel(
     typedef Layout<R, 4> L;
     constexpr int MU0 = (GAUGE == GAUGE_COULOMB) ? 1 : 0;
     constexpr int ND = 4 - MU0;
+    pdl_launch_dependents();
     const int Nzh = args.Nz >> 1;
     const int Vsh = args.Nx * args.Ny * Nzh;
     const int64_t Vh = (int64_t)args.Nt * Vsh;
@@ -59,6 +60,7 @@ __global__ void __launch_bounds__(128, sizeof(R) == 8 ? 3 : 4) sweep_su2_kernel(
     char* const up0 = links + L::link_offset(par, MU0, Vh);
     char* const dn0 = links + L::link_offset(1 - par, MU0, Vh);
     Quat<R> up[ND], dn[ND];
+    pdl_wait();   // nothing of the previous kernel's output is read above this line
 #pragma unroll
     for (int m = 0; m < ND; ++m) {
         global_get_q(up0 + m * lstride, Vh, cb, up[m]);
@@ -157,8 +159,7 @@ static cudaError_t launch_su2_one(const SweepArgs& args, int block, cudaStream_t
     const int Vsh = args.Nx * args.Ny * (args.Nz / 2);
     block = sweep_su2_block(Vsh, block);
     const dim3 grid((unsigned)((Vsh + block - 1) / block), (unsigned)(args.ncopies * args.Nt));
-    sweep_su2_kernel<R, A, GAUGE, STOCH, TRACK, RED><<<grid, block, 0, stream>>>(args);
-    return cudaGetLastError();
+    return launch_with_pdl(sweep_su2_kernel<R, A, GAUGE, STOCH, TRACK, RED>, grid, dim3((unsigned)block), 0, stream, args);
 }
 template <class R, class A, int GAUGE>
 static cudaError_t launch_su2_gauge(const SweepArgs& args, bool track, int block, cudaStream_t stream) {

@@ -88,6 +88,7 @@ _lib.gf_last_error.restype = ctypes.c_char_p
 _lib.gf_version.restype = ctypes.c_char_p
 _lib.gf_debug_set_block.argtypes = [_vp, _ci]
 _lib.gf_debug_set_fused.argtypes = [_vp, _ci]
+_lib.gf_debug_set_pdl.argtypes = [_vp, _ci]
 
 
 class GfError(RuntimeError):
@@ -363,6 +364,10 @@ def gf_last_error(ctx) -> str:
 
 def gf_debug_set_fused(ctx, fused):
     return _check(ctx, _lib.gf_debug_set_fused(ctx, 1 if fused else 0))
+
+
+def gf_debug_set_pdl(ctx, pdl):
+    return _check(ctx, _lib.gf_debug_set_pdl(ctx, 1 if pdl else 0))
 
 
 def gf_debug_set_block(ctx, block):
