@@ -155,7 +155,7 @@ GF_DEV void acc_dagger(Mat<A>& K, const Mat<T>& W) {
         }
 }
 
-// MAG neighbourhood summary (DESIGN.md §6.3): Hermitian M_k = sum_up col_k col_k^dag + sum_down r r^dag,
+// MAG neighbourhood summary (DESIGN.md §6.1): Hermitian M_k = sum_up col_k col_k^dag + sum_down r r^dag,
 // r = conj(row_k)^T, so that the local functional of Eq. (11) is sum_k (g M_k g^dag)_kk.
 // Stored as its upper triangle: d = real diagonal, o = (0,1),(0,2),(1,2) complex.
 template <class T>

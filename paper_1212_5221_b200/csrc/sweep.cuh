@@ -5,7 +5,7 @@
 // private slice of shared memory with 16-byte cp.async (no register staging, 2d*R*s bytes in flight
 // per thread), then
 //   pass 1  builds the neighbourhood summary in registers: K(x) of Eq. (19) for
-//           Landau/Coulomb, the three Hermitian M_k for MAG (DESIGN.md §6.3);
+//           Landau/Coulomb, the three Hermitian M_k for MAG (DESIGN.md §6.1);
 //   Step 1  runs the three Cabibbo-Marinari subgroup updates on the summary
 //           alone (K -> g K, M_k -> g M_k g^dagger), accumulating G = g3 g2 g1;
 //   pass 2  re-reads each link from shared memory, rotates it once with the SU(3) matrix G
@@ -39,7 +39,7 @@ struct SweepArgs {
     // of the sites this launch updates (fused reductions)
     double* red;
     const unsigned char* slice_skip;   // nullptr, or [ncopies*Nt]: 1 = leave this time-slice alone (frozen)
-    // batched gauge copies (DESIGN.md §6.7): blockIdx.y = copy*Nt + t; copy c lives at links + c*copy_links_bytes
+    // batched gauge copies (DESIGN.md §6.5): blockIdx.y = copy*Nt + t; copy c lives at links + c*copy_links_bytes
     // (gtot + c*copy_gtot_bytes) and draws its random numbers with the Philox key seed + c
     int ncopies;
     int64_t copy_links_bytes, copy_gtot_bytes;
