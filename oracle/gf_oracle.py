@@ -86,6 +86,12 @@ def lib():
         L.gfo_plaquette_d.restype = cd
         L.gfo_plaquette_f.argtypes = [vp, vp]
         L.gfo_plaquette_f.restype = cd
+        L.gfo2_wilson_heatbath_d.argtypes = [vp, vp, cd, u64, u32]
+        L.gfo2_wilson_heatbath_f.argtypes = [vp, vp, cd, u64, u32]
+        L.gfo2_plaquette_d.argtypes = [vp, vp]
+        L.gfo2_plaquette_d.restype = cd
+        L.gfo2_plaquette_f.argtypes = [vp, vp]
+        L.gfo2_plaquette_f.restype = cd
         L.gfo_staple_d.argtypes = [vp, vp, ci, ci, ci, ci, ci, vp]
         L.gfo_staple_d.restype = None
         # N_c = 2 (gf_oracle_su2.hpp)
@@ -382,16 +388,19 @@ def wilson_heatbath(links: np.ndarray, beta: float, seed: int, sweep_index: int 
     """One Cabibbo-Marinari heatbath sweep of the Wilson action at coupling beta (SU(3)), in place
     (gf_oracle_wilson.hpp): the input generator standing in for the paper's beta = 5.7 ensemble."""
     d = _dims(links)
-    assert nc_of(links) == 3
-    fn = lib().gfo_wilson_heatbath_d if links.dtype == np.float64 else lib().gfo_wilson_heatbath_f
+    if nc_of(links) == 2:
+        fn = lib().gfo2_wilson_heatbath_d if links.dtype == np.float64 else lib().gfo2_wilson_heatbath_f
+    else:
+        fn = lib().gfo_wilson_heatbath_d if links.dtype == np.float64 else lib().gfo_wilson_heatbath_f
     if fn(_p(links), _p(d), float(beta), seed, sweep_index) != 0:
         raise ValueError("oracle wilson_heatbath: invalid arguments")
 
 
 def plaquette(links: np.ndarray) -> float:
-    """<Re tr U_P> / 3 over all 6 V plaquettes (SU(3))."""
+    """<Re tr U_P> / N_c over all 6 V plaquettes."""
     d = _dims(links)
-    assert nc_of(links) == 3
+    if nc_of(links) == 2:
+        return float((lib().gfo2_plaquette_d if links.dtype == np.float64 else lib().gfo2_plaquette_f)(_p(links), _p(d)))
     return float((lib().gfo_plaquette_d if links.dtype == np.float64 else lib().gfo_plaquette_f)(_p(links), _p(d)))
 
 

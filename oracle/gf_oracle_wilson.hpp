@@ -125,6 +125,72 @@ double plaquette_mean(const R* links, const Lattice& L) {
     return tot / (3.0 * 6.0 * (double)L.V());
 }
 
+// ---- the same for the gauge group SU(2): one "subgroup", weight exp((beta/2) Re tr[U A]), T = 2/beta ----
+template <class R>
+inline Mat2<R> staple_sum2(const R* links, const Lattice& L, const int c[4], int mu) {
+    Mat2<R> A;
+    for (int i = 0; i < 2; ++i)
+        for (int j = 0; j < 2; ++j) A.m[i][j] = std::complex<R>(0, 0);
+    const int64_t x = L.site(c[0], c[1], c[2], c[3]);
+    const int64_t xmu = site_shift2(L, c, mu, +1, mu, 0);
+    for (int nu = 0; nu < 4; ++nu) {
+        if (nu == mu) continue;
+        const int64_t xnu = site_shift2(L, c, nu, +1, nu, 0), xmnu = site_shift2(L, c, nu, -1, nu, 0);
+        const int64_t xmu_mnu = site_shift2(L, c, mu, +1, nu, -1);
+        Mat2<R> up = mul2<R>(mul2<R>(load2<R>(link_ptr2(links, xmu, nu)), dagger2<R>(load2<R>(link_ptr2(links, xnu, mu)))),
+                             dagger2<R>(load2<R>(link_ptr2(links, x, nu))));
+        Mat2<R> lo = mul2<R>(mul2<R>(dagger2<R>(load2<R>(link_ptr2(links, xmu_mnu, nu))),
+                                     dagger2<R>(load2<R>(link_ptr2(links, xmnu, mu)))),
+                             load2<R>(link_ptr2(links, xmnu, nu)));
+        for (int i = 0; i < 2; ++i)
+            for (int j = 0; j < 2; ++j) A.m[i][j] += up.m[i][j] + lo.m[i][j];
+    }
+    return A;
+}
+
+template <class R>
+void wilson_heatbath_sweep2(R* links, const Lattice& L, double beta, uint64_t seed, uint32_t sweep_index) {
+    const double T = 2.0 / beta;
+    for (int mu = 0; mu < 4; ++mu)
+        for (int parity = 0; parity < 2; ++parity)
+            for (int t = 0; t < L.Nt; ++t)
+                for (int x = 0; x < L.Nx; ++x)
+                    for (int y = 0; y < L.Ny; ++y)
+                        for (int z = 0; z < L.Nz; ++z) {
+                            if (((t + x + y + z) & 1) != parity) continue;
+                            const int c[4] = {t, x, y, z};
+                            const int64_t s = L.site(t, x, y, z);
+                            Mat2<R> U = load2<R>(link_ptr2(links, s, mu));
+                            const Mat2<R> W = mul2<R>(U, staple_sum2<R>(links, L, c, mu));
+                            double a[4] = {0, 0, 0, 0}, g[4];
+                            add_quaternion2<R, double>(a, W);
+                            rule_heatbath_landau(a, T, seed, (uint32_t)s, 4u * sweep_index + (uint32_t)mu, 0, g);
+                            R gr[4] = {(R)g[0], (R)g[1], (R)g[2], (R)g[3]};
+                            store2<R>(link_ptr2(links, s, mu), mul2<R>(su2_matrix<R>(gr), U));
+                        }
+}
+
+template <class R>
+double plaquette_mean2(const R* links, const Lattice& L) {
+    double tot = 0.0;
+    for (int t = 0; t < L.Nt; ++t)
+        for (int x = 0; x < L.Nx; ++x)
+            for (int y = 0; y < L.Ny; ++y)
+                for (int z = 0; z < L.Nz; ++z) {
+                    const int c[4] = {t, x, y, z};
+                    const int64_t s = L.site(t, x, y, z);
+                    for (int mu = 0; mu < 4; ++mu)
+                        for (int nu = mu + 1; nu < 4; ++nu) {
+                            const int64_t xmu = site_shift2(L, c, mu, +1, mu, 0), xnu = site_shift2(L, c, nu, +1, nu, 0);
+                            Mat2<R> P = mul2<R>(mul2<R>(load2<R>(link_ptr2(links, s, mu)), load2<R>(link_ptr2(links, xmu, nu))),
+                                                mul2<R>(dagger2<R>(load2<R>(link_ptr2(links, xnu, mu))),
+                                                        dagger2<R>(load2<R>(link_ptr2(links, s, nu)))));
+                            tot += (double)P.m[0][0].real() + (double)P.m[1][1].real();
+                        }
+                }
+    return tot / (2.0 * 6.0 * (double)L.V());
+}
+
 }  // namespace
 
 extern "C" {
@@ -148,6 +214,26 @@ double gfo_plaquette_d(const double* links, const int* dims) {
 double gfo_plaquette_f(const float* links, const int* dims) {
     Lattice L = {dims[0], dims[1], dims[2], dims[3]};
     return plaquette_mean<float>(links, L);
+}
+int gfo2_wilson_heatbath_d(double* links, const int* dims, double beta, uint64_t seed, uint32_t sweep_index) {
+    if (!dims_ok(dims) || !(beta > 0)) return -1;
+    Lattice L = {dims[0], dims[1], dims[2], dims[3]};
+    wilson_heatbath_sweep2<double>(links, L, beta, seed, sweep_index);
+    return 0;
+}
+int gfo2_wilson_heatbath_f(float* links, const int* dims, double beta, uint64_t seed, uint32_t sweep_index) {
+    if (!dims_ok(dims) || !(beta > 0)) return -1;
+    Lattice L = {dims[0], dims[1], dims[2], dims[3]};
+    wilson_heatbath_sweep2<float>(links, L, beta, seed, sweep_index);
+    return 0;
+}
+double gfo2_plaquette_d(const double* links, const int* dims) {
+    Lattice L = {dims[0], dims[1], dims[2], dims[3]};
+    return plaquette_mean2<double>(links, L);
+}
+double gfo2_plaquette_f(const float* links, const int* dims) {
+    Lattice L = {dims[0], dims[1], dims[2], dims[3]};
+    return plaquette_mean2<float>(links, L);
 }
 // staple sum of one link, for the pins
 void gfo_staple_d(const double* links, const int* dims, int t, int x, int y, int z, int mu, double* out18) {

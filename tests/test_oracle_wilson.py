@@ -89,3 +89,34 @@ def test_infinite_beta_is_a_monotone_cooling(oracle):
         oracle.wilson_heatbath(L, 1e9, seed=17, sweep_index=s)
         P.append(oracle.plaquette(L))
     assert np.all(np.diff(P) > 0) and P[-1] > P[0] + 0.2
+
+
+# ---- gauge group SU(2): <P> = beta/4 + O(beta^3) at strong coupling, 1 - <P> -> 3/(4 beta) at weak coupling ----
+def cold2(dims_txyz):
+    U = np.broadcast_to(np.eye(2, dtype=np.complex128), tuple(dims_txyz) + (4, 2, 2)).copy()
+    return inputs.as_real(U)
+
+
+def test_su2_plaquette_matches_numpy(oracle):
+    U = inputs.make_config_su2(4, 6, 4, 4, 0.5, 3, 4)
+    assert abs(oracle.plaquette(inputs.as_real(U)) - plaquettes(U).mean() * 3 / 2) < 1e-14      # helper divides by 3
+    assert abs(oracle.plaquette(cold2((4, 4, 4, 4))) - 1.0) < 1e-15
+
+
+def test_su2_strong_and_weak_coupling(oracle):
+    L = inputs.as_real(inputs.make_config_su2(4, 4, 4, 4, 3.0, 9, 10))
+    vals = []
+    for s in range(45):
+        oracle.wilson_heatbath(L, 0.4, seed=11, sweep_index=s)
+        if s >= 5:
+            vals.append(oracle.plaquette(L))
+    assert abs(np.mean(vals) - 0.4 / 4) < 0.005, np.mean(vals)
+    L = cold2((4, 4, 4, 4))
+    vals = []
+    for s in range(40):
+        oracle.wilson_heatbath(L, 30.0, seed=13, sweep_index=s)
+        if s >= 15:
+            vals.append(oracle.plaquette(L))
+    assert 0.85 * 3 / (4 * 30.0) < 1 - np.mean(vals) < 1.1 * 3 / (4 * 30.0), 1 - np.mean(vals)
+    V = inputs.as_complex(L)
+    assert np.abs(V @ dag(V) - np.eye(2)).max() < 1e-13 and np.abs(np.linalg.det(V) - 1).max() < 1e-13
