@@ -248,13 +248,14 @@ int gf_random_gauge(gf_ctx* ctx, uint64_t seed);
  * Input generator.  The paper's production input is a thermalised beta = 5.7 32^4
  * configuration of the Wilson gauge action, which is not distributed with it.
  * gf_wilson_heatbath runs n_sweeps Cabibbo-Marinari pseudo-heatbath sweeps (the SU(2)-subgroup method of the
- * paper's ref. [31]) of S = beta sum_P (1 - Re tr U_P / 3) on every copy of an SU(3) context: for mu = 0..3,
+ * paper's ref. [31]) of S = beta sum_P (1 - Re tr U_P / N_c) on every copy of a context (SU(3) in what follows): for mu = 0..3,
  * for parity even, odd, every link U_mu(x) of that parity is multiplied from the left, subgroup by subgroup
  * ((0,1),(0,2),(1,2)), by g drawn with P(g) ~ exp((beta/3) Re tr[g~ U A]), A the sum of the six staples
  * (Kennedy-Pendleton / Creutz sampler of GF_SA at T = 3/beta).  Philox counter (site, 4 * sweep + mu,
  * sub | purpose << 8, trial), key seed + copy, sweeps first_sweep_index .. first_sweep_index + n_sweeps - 1.
  * The result is a new configuration, so a tracked transform restarts at the identity.  Asynchronous.
- * gf_plaquette: plaq[n_copies] receives <Re tr U_P> / 3 over the 6 V plaquettes (gauge invariant under
+ * On SU(2) contexts the same with the single subgroup and the weight exp((beta/2) Re tr[U A]) (T = 2/beta).
+ * gf_plaquette: plaq[n_copies] receives <Re tr U_P> / N_c over the 6 V plaquettes (gauge invariant under
  * Eq. (1): it does not change under any sweep of this library).  Synchronous.
  */
 int gf_wilson_heatbath(gf_ctx* ctx, double beta, uint64_t seed, uint32_t first_sweep_index, int n_sweeps);

@@ -1124,7 +1124,6 @@ int gf_random_gauge(gf_ctx* ctx, uint64_t seed) {
 int gf_wilson_heatbath(gf_ctx* ctx, double beta, uint64_t seed, uint32_t first_sweep_index, int n_sweeps) {
     if (!ctx) return GF_EINVAL;
     if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_wilson_heatbath: no links set");
-    if (ctx->nc != 3) return fail(ctx, GF_ESTATE, "gf_wilson_heatbath: SU(3) contexts only");
     if (!(beta > 0.0) || n_sweeps < 0) return fail(ctx, GF_EINVAL, "gf_wilson_heatbath: beta = %g, n_sweeps = %d", beta, n_sweeps);
     if (ctx->temporal_stale && ctx->gtot) {
         int rc = gf_coulomb_finalize(ctx);
@@ -1134,7 +1133,16 @@ int gf_wilson_heatbath(gf_ctx* ctx, double beta, uint64_t seed, uint32_t first_s
     for (int k = 0; k < n_sweeps; ++k)
         for (int mu = 0; mu < 4; ++mu)
             for (int par = 0; par < 2; ++par) {
-                DISPATCH_RR(ctx, WILSON_HB, mu, par, first_sweep_index + (uint32_t)k);
+                if (ctx->nc == 2) {
+                    const dim3 g2((unsigned)((Vsh + 127) / 128), (unsigned)ctx->NS);
+                    if (ctx->real_bytes == 4)
+                        wilson_heatbath2_kernel<float><<<g2, 128, 0, ctx->stream>>>(ctx->links, dims_of(ctx), mu, par, beta, seed,
+                                                                                     first_sweep_index + (uint32_t)k, link_store_bytes(ctx));
+                    else
+                        wilson_heatbath2_kernel<double><<<g2, 128, 0, ctx->stream>>>(ctx->links, dims_of(ctx), mu, par, beta, seed,
+                                                                                      first_sweep_index + (uint32_t)k, link_store_bytes(ctx));
+                } else
+                    DISPATCH_RR(ctx, WILSON_HB, mu, par, first_sweep_index + (uint32_t)k);
                 CU(cudaGetLastError());
                 ++ctx->launches;
             }
@@ -1154,12 +1162,16 @@ int gf_plaquette(gf_ctx* ctx, double* plaq) {
     if (!ctx) return GF_EINVAL;
     if (!plaq) return fail(ctx, GF_EINVAL, "gf_plaquette: NULL pointer");
     if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_plaquette: no links set");
-    if (ctx->nc != 3) return fail(ctx, GF_ESTATE, "gf_plaquette: SU(3) contexts only");
     if (ctx->temporal_stale && ctx->gtot) {
         int rc = gf_coulomb_finalize(ctx);
         if (rc) return rc;
     }
-    DISPATCH_RR(ctx, PLAQUETTE, 0);
+    if (ctx->nc == 2) {
+        const dim3 g2((unsigned)ctx->meas_gx, (unsigned)ctx->NS, 2);
+        if (ctx->real_bytes == 4) plaquette2_kernel<float><<<g2, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, link_store_bytes(ctx));
+        else plaquette2_kernel<double><<<g2, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, link_store_bytes(ctx));
+    } else
+        DISPATCH_RR(ctx, PLAQUETTE, 0);
     CU(cudaGetLastError());
     slice_reduce_kernel<<<ctx->NS, 128, 0, ctx->stream>>>(ctx->partial, 2 * ctx->meas_gx, ctx->NS, ctx->slice_dev);
     CU(cudaGetLastError());
@@ -1170,7 +1182,7 @@ int gf_plaquette(gf_ctx* ctx, double* plaq) {
     for (int c = 0; c < ctx->B; ++c) {
         double tot = 0.0;
         for (int t = 0; t < ctx->Nt; ++t) tot += ctx->slice_host[(size_t)c * ctx->Nt + t];
-        plaq[c] = tot / (3.0 * 6.0 * (double)ctx->V);
+        plaq[c] = tot / ((double)ctx->nc * 6.0 * (double)ctx->V);
     }
     return GF_OK;
 }

@@ -10,6 +10,7 @@
 #pragma once
 #include "aux_kernels.cuh"
 #include "step1.cuh"
+#include "su2.cuh"
 
 namespace gf {
 
@@ -157,6 +158,102 @@ __global__ void plaquette_kernel(const char* links, Dims d, double* partial, int
                 // Re tr[T2 b^dag] = sum_ij Re(T2_ij conj(b_ij))
 #pragma unroll
                 for (int k = 0; k < 18; ++k) acc += (double)T2.v[k] * (double)b.v[k];
+            }
+    }
+    block_sum2(acc, zero);
+    if (threadIdx.x == 0) {
+        const int64_t bidx = ((int64_t)(blockIdx.y * 2 + par)) * gridDim.x + blockIdx.x;
+        partial[2 * bidx] = acc;
+        partial[2 * bidx + 1] = 0.0;
+    }
+}
+
+// ---- the same for the gauge group SU(2) (links as quaternions, su2.cuh): weight exp((beta/2) Re tr[U A]) ----
+template <class R>
+__global__ void __launch_bounds__(128) wilson_heatbath2_kernel(char* links_all, Dims d, int mu, int parity, double beta,
+                                                               uint64_t seed0, uint32_t sweep_index, int64_t copy_bytes) {
+    typedef Layout<R, 4> L;
+    const int Nzh = d.Nz >> 1;
+    const int Vsh = d.Nx * d.Ny * Nzh;
+    const int64_t Vh = (int64_t)d.Nt * Vsh;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= Vsh) return;
+    const int copy = blockIdx.y / d.Nt;
+    const int t = blockIdx.y - copy * d.Nt;
+    char* links = links_all + copy * copy_bytes;
+    int rem = i;
+    const int zh = rem % Nzh; rem /= Nzh;
+    const int y = rem % d.Ny;
+    const int x = rem / d.Ny;
+    SiteCoord s;
+    s.c[0] = t; s.c[1] = x; s.c[2] = y; s.c[3] = 2 * zh + ((t + x + y + parity) & 1);
+    const int64_t cb = (int64_t)t * Vsh + i;
+    const uint32_t site = (uint32_t)(((t * d.Nx + x) * d.Ny + y) * d.Nz + s.c[3]);
+    const int q = 1 - parity;
+    Quat<R> U, a, b, c;
+    global_get_q(links + L::link_offset(parity, mu, Vh), Vh, cb, U);
+    R A[4] = {R(0), R(0), R(0), R(0)};
+    const int64_t cb_mu = cb_shift(d, s, mu, +1, mu, 0);
+#pragma unroll 1
+    for (int nu = 0; nu < 4; ++nu) {
+        if (nu == mu) continue;
+        global_get_q(links + L::link_offset(q, nu, Vh), Vh, cb_mu, a);
+        global_get_q(links + L::link_offset(q, mu, Vh), Vh, cb_shift(d, s, nu, +1, nu, 0), b);
+        global_get_q(links + L::link_offset(parity, nu, Vh), Vh, cb, c);
+        Quat<R> st = qmul_dagger(qmul_dagger(a, b), c);              // U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag
+#pragma unroll
+        for (int k = 0; k < 4; ++k) A[k] += st.v[k];
+        const int64_t cb_mnu = cb_shift(d, s, nu, -1, nu, 0);
+        global_get_q(links + L::link_offset(parity, nu, Vh), Vh, cb_shift(d, s, mu, +1, nu, -1), a);
+        global_get_q(links + L::link_offset(q, mu, Vh), Vh, cb_mnu, b);
+        global_get_q(links + L::link_offset(q, nu, Vh), Vh, cb_mnu, c);
+        st = qmul(qconj(qmul(b, a)), c);                             // [U_mu(x-nu) U_nu(x+mu-nu)]^dag U_nu(x-nu)
+#pragma unroll
+        for (int k = 0; k < 4; ++k) A[k] += st.v[k];
+    }
+    Quat<R> Aq;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) Aq.v[k] = A[k];
+    const Quat<R> W = qmul(U, Aq);                                   // the product is bilinear: A need not be unit
+    const double aw[4] = {2.0 * (double)W.v[0], 2.0 * (double)W.v[1], 2.0 * (double)W.v[2], 2.0 * (double)W.v[3]};
+    double gd[4];
+    rule_heatbath_landau(aw, 2.0 / beta, seed0 + (uint64_t)copy, site, 4u * sweep_index + (uint32_t)mu, 0, gd);
+    Quat<R> g;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) g.v[k] = (R)gd[k];
+    global_put_q(links + L::link_offset(parity, mu, Vh), Vh, cb, qmul(g, U));
+}
+
+template <class R>
+__global__ void plaquette2_kernel(const char* links, Dims d, double* partial, int64_t copy_bytes) {
+    typedef Layout<R, 4> L;
+    const int Nzh = d.Nz >> 1;
+    const int Vsh = d.Nx * d.Ny * Nzh;
+    const int64_t Vh = (int64_t)d.Nt * Vsh;
+    const int copy = blockIdx.y / d.Nt;
+    const int t = blockIdx.y - copy * d.Nt, par = blockIdx.z;
+    links += copy * copy_bytes;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double acc = 0.0, zero = 0.0;
+    if (i < Vsh) {
+        int rem = i;
+        const int zh = rem % Nzh; rem /= Nzh;
+        const int y = rem % d.Ny;
+        const int x = rem / d.Ny;
+        SiteCoord s;
+        s.c[0] = t; s.c[1] = x; s.c[2] = y; s.c[3] = 2 * zh + ((t + x + y + par) & 1);
+        const int64_t cb = (int64_t)t * Vsh + i;
+#pragma unroll 1
+        for (int mu = 0; mu < 4; ++mu)
+#pragma unroll 1
+            for (int nu = mu + 1; nu < 4; ++nu) {
+                Quat<R> a, b, c, e;
+                global_get_q(links + L::link_offset(par, mu, Vh), Vh, cb, a);
+                global_get_q(links + L::link_offset(1 - par, nu, Vh), Vh, cb_shift(d, s, mu, +1, mu, 0), b);
+                global_get_q(links + L::link_offset(1 - par, mu, Vh), Vh, cb_shift(d, s, nu, +1, nu, 0), c);
+                global_get_q(links + L::link_offset(par, nu, Vh), Vh, cb, e);
+                const Quat<R> P = qmul_dagger(qmul_dagger(qmul(a, b), c), e);
+                acc += 2.0 * (double)P.v[0];                        // Re tr of the SU(2) matrix
             }
     }
     block_sum2(acc, zero);

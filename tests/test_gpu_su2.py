@@ -189,7 +189,7 @@ def test_su3_only_calls_refuse_su2_contexts_and_bad_arguments(gf):
     L = make(dims)
     with gf.GaugeFixer(*dims, precision=DP, su2=True) as fx:
         fx.set_links(L)
-        for call in (lambda: fx.wilson_heatbath(5.7, 1), lambda: fx.plaquette(), lambda: fx.unitarity()):
+        for call in (lambda: fx.unitarity(),):
             with pytest.raises(gf.GfError) as e:
                 call()
             assert e.value.code == gf.GF_ESTATE
@@ -217,3 +217,45 @@ def test_three_dimensional_lattices_are_coulomb_slices(gf, oracle):
     assert conv and r["converged"] and ths.max() < 1e-12
     assert np.all(np.abs(sw - sl) <= 2) and abs(r["F"] - Fo) <= 1e-10
     assert len(set(sw.tolist())) > 1
+
+
+@pytest.mark.parametrize("prec,beta", [(DP, 2.4), (DP, 0.5), (SP, 2.4)])
+def test_wilson_heatbath_and_plaquette(gf, oracle, prec, beta):
+    # the input generator on SU(2) links: draws identical to the oracle's, per link <= 1e-11 per sweep in DP
+    dims = (4, 6, 4, 6)
+    B = 2
+    dt = dt_of(prec)
+    L = make(dims, eps=0.4, seed=980, dtype=dt)
+    with gf.GaugeFixer(*dims, precision=prec, su2=True, n_copies=B) as fx:
+        fx.set_links(L)
+        assert abs(fx.plaquette()[0] - oracle.plaquette(L)) <= (1e-13 if prec == DP else 2e-7)
+        fx.wilson_heatbath(beta, seed=41, first_sweep_index=2, n_sweeps=2)
+        P = fx.plaquette()
+        for c in range(B):
+            ref = L.copy()
+            oracle.wilson_heatbath(ref, beta, 41 + c, 2)
+            oracle.wilson_heatbath(ref, beta, 41 + c, 3)
+            diff = np.abs(fx.get_links_copy(c, dtype=dt).astype(np.float64) - ref)
+            if prec == DP:
+                assert diff.max() <= 1e-10, diff.max()
+            else:
+                assert np.quantile(diff, 0.99) <= 5e-5 and diff.max() <= 5e-3
+            assert abs(P[c] - oracle.plaquette(ref)) <= (1e-10 if prec == DP else 1e-4)
+
+
+def test_thermalised_su2_lattice_is_fixed_and_keeps_its_plaquette(gf):
+    # 16^4 at beta = 2.4 from a cold start (lattice literature: <P> = 0.630; not a number of the paper), then Landau
+    dims = (16, 16, 16, 16)
+    cold = inputs.as_real(np.broadcast_to(np.eye(2, dtype=np.complex128), (16, 16, 16, 16, 4, 2, 2)).copy())
+    with gf.GaugeFixer(*dims, precision=DP, su2=True) as fx:
+        fx.set_links(cold)
+        fx.wilson_heatbath(2.4, seed=3, n_sweeps=200)
+        vals = []
+        for k in range(10):
+            fx.wilson_heatbath(2.4, seed=3, first_sweep_index=200 + 5 * k, n_sweeps=5)
+            vals.append(fx.plaquette()[0])
+        assert abs(np.mean(vals) - 0.630) < 0.004, np.mean(vals)
+        P0 = fx.plaquette()[0]
+        r = fx.run(LANDAU, OR, 1.7, max_sweeps=20000, eps=1e-12, check_every=10)
+        assert r["converged"] and 0.8 < r["F"] < 0.95
+        assert abs(fx.plaquette()[0] - P0) < 1e-12
