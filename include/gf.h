@@ -264,7 +264,8 @@ int gf_plaquette(gf_ctx* ctx, double* plaq);
 /*
  * gf_unitarity — the unitarity measure of Eq. (33): avg[c] = (1/4V) sum_{mu,x} |1 - det U_mu(x)| and
  * max[c] = max_{mu,x} |1 - det U_mu(x)| for every copy c (n_copies entries each, either may be NULL), evaluated in
- * double from the stored links (recon = 12: with the rebuilt third row).  SU(3) contexts.  Synchronous.
+ * double from the stored links (recon = 12: with the rebuilt third row; SU(2): det U = |u|^2 of the stored quaternion).
+ * Synchronous.
  */
 int gf_unitarity(gf_ctx* ctx, double* avg, double* max);
 

@@ -222,4 +222,32 @@ __global__ void gauge_apply2_kernel(char* links, char* gtot, const char* hfield,
     }
 }
 
+// Eq. (33) for N_c = 2: det U = u0^2 + u1^2 + u2^2 + u3^2 for a matrix of the form of Eq. (15); same partials
+// as unitarity_kernel (aux_kernels.cuh)
+template <class R>
+__global__ void unitarity2_kernel(const char* base, int64_t Vh, int64_t copy_bytes, double* partial) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    double dev = 0.0;
+    if (i < 8 * Vh) {
+        Quat<R> q;
+        global_get_q(base + blockIdx.y * copy_bytes + (i / Vh) * Layout<R, 4>::LINK_BYTES * Vh, Vh, i % Vh, q);
+        const double a = q.v[0], b = q.v[1], c = q.v[2], e = q.v[3];
+        dev = fabs(1.0 - (a * a + b * b + c * c + e * e));
+    }
+    __shared__ double smax[32];
+    double mx = dev;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_down_sync(0xffffffffu, mx, o));
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    if (lane == 0) smax[w] = mx;
+    double zero = 0.0;
+    block_sum2(dev, zero);
+    if (threadIdx.x == 0) {
+        double m2 = 0.0;
+        for (int k = 0; k < nw; ++k) m2 = fmax(m2, smax[k]);
+        double* p = partial + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * 2;
+        p[0] = dev; p[1] = m2;
+    }
+}
+
 }  // namespace gf

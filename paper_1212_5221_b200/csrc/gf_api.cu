@@ -1191,7 +1191,6 @@ int gf_plaquette(gf_ctx* ctx, double* plaq) {
 int gf_unitarity(gf_ctx* ctx, double* avg, double* max) {
     if (!ctx) return GF_EINVAL;
     if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_unitarity: no links set");
-    if (ctx->nc != 3) return fail(ctx, GF_ESTATE, "gf_unitarity: SU(3) contexts only");
     const int nb = (int)((8 * ctx->Vh + 255) / 256);
     double* part = nullptr;
     double* out = nullptr;
@@ -1201,7 +1200,11 @@ int gf_unitarity(gf_ctx* ctx, double* avg, double* max) {
     if (e == cudaSuccess) {
         const dim3 g((unsigned)nb, (unsigned)ctx->B);
 #define UNITARITY(R, RECON, dummy) unitarity_kernel<R, RECON><<<g, 256, 0, ctx->stream>>>(ctx->links, ctx->Vh, link_store_bytes(ctx), part)
-        DISPATCH_RR(ctx, UNITARITY, 0);
+        if (ctx->nc == 2) {
+            if (ctx->real_bytes == 4) unitarity2_kernel<float><<<g, 256, 0, ctx->stream>>>(ctx->links, ctx->Vh, link_store_bytes(ctx), part);
+            else unitarity2_kernel<double><<<g, 256, 0, ctx->stream>>>(ctx->links, ctx->Vh, link_store_bytes(ctx), part);
+        } else
+            DISPATCH_RR(ctx, UNITARITY, 0);
 #undef UNITARITY
         e = cudaGetLastError();
     }

@@ -184,15 +184,17 @@ def test_large_lattice_tiled(gf, oracle, prec):
     assert F == pytest.approx(m["F"], rel=rel, abs=rel) and th == pytest.approx(m["theta"], rel=10 * rel)
 
 
-def test_su3_only_calls_refuse_su2_contexts_and_bad_arguments(gf):
+def test_unitarity_and_bad_arguments_on_su2_contexts(gf):
     dims = (4, 4, 4, 4)
     L = make(dims)
     with gf.GaugeFixer(*dims, precision=DP, su2=True) as fx:
         fx.set_links(L)
-        for call in (lambda: fx.unitarity(),):
-            with pytest.raises(gf.GfError) as e:
-                call()
-            assert e.value.code == gf.GF_ESTATE
+        avg, mx = fx.unitarity()                       # Eq. (33) with det U = |u|^2
+        assert mx[0] < 1e-15
+        fx.set_links(L * 1.001)
+        avg, mx = fx.unitarity()
+        assert abs(avg[0] - (1.001 ** 2 - 1)) < 1e-12 and abs(mx[0] - (1.001 ** 2 - 1)) < 1e-12
+        fx.set_links(L)
         for kw in (dict(check_every=0), dict(sa_steps=-1), dict(or_omega=2.5), dict(sa_steps=2, sa_T_lo=0.0)):
             with pytest.raises(gf.GfError) as e:
                 fx.fix(LANDAU, **kw)
