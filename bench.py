@@ -255,6 +255,8 @@ class Ranks:
 # ---- the CUDA path ----------------------------------------------------------------------------
 def run_ours(args):
     import torch
+    from paper_1212_5221_b200 import build as _build
+    _build.build()                          # in-tree libgf.so: a no-op when it is up to date (nvcc, sm_100a)
     from paper_1212_5221_b200 import gf     # fails loudly if libgf.so is missing
 
     local = int(os.environ.get("LOCAL_RANK", "0"))

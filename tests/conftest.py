@@ -17,3 +17,11 @@ def oracle():
     from oracle import gf_oracle
     gf_oracle.build()
     return gf_oracle
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _libgf_built():
+    """The in-tree libgf.so is a build artefact (git-ignored): make sure it exists and is up to date before any
+    test imports the binding (nvcc cross-compiles without a GPU; a no-op when nothing changed)."""
+    from paper_1212_5221_b200 import build
+    build.build()
