@@ -397,7 +397,7 @@ def run_ours(args):
                              "bytes_per_site_update": v["roofline"]["bytes_per_site_update"],
                              "kernel_share_of_step": v["kernel_share_of_step"]})
 
-    def bench_other(dims_o, gauge, prec, recon, copies, sweeps, label, su2=False):
+    def bench_other(dims_o, gauge, prec, recon, copies, sweeps, label, su2=False, track=False):
         """Side measurement (not the headline): `sweeps` OR sweeps of `copies` lattices of extent dims_o."""
         ox, oy, oz, ot = dims_o
         Vo = ox * oy * oz * ot
@@ -412,7 +412,7 @@ def run_ours(args):
         with torch.cuda.stream(stream):
             src = torch.from_numpy(src_tile).to(dev).repeat(*r_o, 1, 1, 1, 1).contiguous()
         with gf.GaugeFixer(ox, oy, oz, ot, precision=PREC_NAMES[prec], recon=18 if su2 else recon, n_copies=copies,
-                           cuda_stream=stream, su2=su2) as fx:
+                           cuda_stream=stream, su2=su2, track_transform=track) as fx:
             fx.set_links(src)
             del src
             fx.run_batch(gauge, OR, OMEGA, max_sweeps=10, eps=-1.0, check_every=10)
@@ -430,6 +430,8 @@ def run_ours(args):
             kern_ms, kern_n = gf.gf_kernel_time_ms(fx.ctx, reset=True)
             gf.gf_kernel_timing(fx.ctx, False)
         bpsu = bytes_per_site_update(prec, recon, nd)
+        if track:       # g(x) (18 reals, 4 for SU(2)) read and written once per site update
+            bpsu += 2 * (4 if su2 else 18) * (8 if prec == "dp" else 4)
         ach = bpsu * (copies * Vo // 2) / (kern_ms / kern_n * 1e-3) / 1e9
         eff = bpsu * copies * Vo * sweeps / (ms * 1e-3) / 1e9        # whole run incl. gaps, reductions, reprojection
         store = copies * Vo * 4 * recon * (8 if prec == "dp" else 4)
@@ -452,6 +454,8 @@ def run_ours(args):
             bench_other((16, 16, 16, 16), 0, "dp", 18, 1, 200, "Landau OR, 16^4, DP-18, one copy (configs[1])"),
             bench_other((16, 16, 16, 16), 0, "dp", 18, 64, 100, "Landau OR, 64 gauge copies of 16^4 per launch, DP-18"),
             bench_other((32, 32, 32, 32), 0, "sp", 12, 16, 100, "Landau OR, 16 gauge copies of 32^4 per launch, SP-12"),
+            bench_other((64, 64, 64, 256), 0, "sp", 12, 1, 50, "Landau OR, 64^3x256, SP-12, accumulating g(x) (a8)", track=True),
+            bench_other((64, 64, 64, 256), 2, "dp", 18, 1, 30, "MAG OR, 64^3x256, DP-18"),
             bench_other((64, 64, 64, 256), 0, "sp", 4, 1, 100, "SU(2) Landau OR, 64^3x256, SP (4 reals per link)", su2=True),
             bench_other((64, 64, 64, 256), 0, "dp", 4, 1, 100, "SU(2) Landau OR, 64^3x256, DP (4 reals per link)", su2=True),
             bench_other((64, 64, 64, 256), 2, "mp", 4, 1, 100, "SU(2) MAG OR, 64^3x256, MP", su2=True),
