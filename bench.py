@@ -68,6 +68,9 @@ def parse_args():
     ap.add_argument("--lattice", default="64,64,64,256", help="Nx,Ny,Nz,Nt")
     ap.add_argument("--precision", default="dp", choices=list(PREC_NAMES))
     ap.add_argument("--recon", type=int, default=18, choices=[12, 18])
+    ap.add_argument("--gauge", default="landau", choices=["landau", "coulomb", "mag"], help="side study: gauge of the headline line")
+    ap.add_argument("--algo", default="or", choices=["or", "sr", "sa", "micro"], help="side study: update rule of the headline line")
+    ap.add_argument("--param", type=float, default=OMEGA, help="omega | p | T of --algo")
     ap.add_argument("--group", default="su3", choices=["su3", "su2"],
                     help="gauge group of the headline line (su2: side study, GF_FLAG_SU2, 4 reals per link)")
     ap.add_argument("--sweeps-per-step", type=int, default=SWEEPS_PER_STEP)
@@ -295,8 +298,15 @@ def run_ours(args):
     stream.synchronize()
     del tile_dev
 
+    GAUGE = {"landau": 0, "coulomb": 1, "mag": 2}[args.gauge]
+    ALGO = {"or": 0, "sr": 1, "sa": 2, "micro": 3}[args.algo]
+    if (GAUGE, ALGO) != (LANDAU, OR):
+        args.no_variants, args.no_cpu_baseline, args.no_others = True, True, True
+
     def bench_one(prec: str, recon: int, steps: int, warmup: int, e2e: bool, sample_clocks: bool):
         reunit = 100 if prec != "dp" else 0
+        if ALGO != OR and recon == 12:
+            reunit = 16          # heatbath / microcanonical sweeps on 12-real storage
         out = {}
         with gf.GaugeFixer(Nx, Ny, Nz, Nt, precision=PREC_NAMES[prec], recon=18 if su2 else recon, cuda_stream=stream,
                            su2=su2) as fx:
@@ -305,7 +315,7 @@ def run_ours(args):
             fx.set_links(links_dev)
 
             def step():
-                return fx.run(LANDAU, OR, OMEGA, max_sweeps=S, eps=-1.0, check_every=S, reunit_every=reunit)
+                return fx.run(GAUGE, ALGO, args.param, seed=7, max_sweeps=S, eps=-1.0, check_every=S, reunit_every=reunit)
 
             for _ in range(warmup):
                 step()
@@ -328,7 +338,7 @@ def run_ours(args):
             launches = gf.gf_launch_count(fx.ctx, reset=True)
             if sampler:
                 out["clocks"] = sampler.stop()
-            bpsu = bytes_per_site_update(prec, recon)
+            bpsu = bytes_per_site_update(prec, recon, 3 if GAUGE == 1 else 4)
             per_launch_bytes = bpsu * (V // 2)
             achieved = per_launch_bytes / (kern_ms / kern_n * 1e-3) / 1e9
             out.update({
@@ -397,7 +407,7 @@ def run_ours(args):
                              "bytes_per_site_update": v["roofline"]["bytes_per_site_update"],
                              "kernel_share_of_step": v["kernel_share_of_step"]})
 
-    def bench_other(dims_o, gauge, prec, recon, copies, sweeps, label, su2=False, track=False):
+    def bench_other(dims_o, gauge, prec, recon, copies, sweeps, label, su2=False, track=False, algo=OR, param=OMEGA):
         """Side measurement (not the headline): `sweeps` OR sweeps of `copies` lattices of extent dims_o."""
         ox, oy, oz, ot = dims_o
         Vo = ox * oy * oz * ot
@@ -415,18 +425,20 @@ def run_ours(args):
                            cuda_stream=stream, su2=su2, track_transform=track) as fx:
             fx.set_links(src)
             del src
-            fx.run_batch(gauge, OR, OMEGA, max_sweeps=10, eps=-1.0, check_every=10)
+            # heatbath / microcanonical sweeps on 12-real storage need frequent reprojection
+            ru = 16 if (algo != OR and recon == 12) else 0
+            fx.run_batch(gauge, algo, param, seed=7, max_sweeps=10, eps=-1.0, check_every=10, reunit_every=ru)
             # pass 1: the run as a user makes it (no events between the launches: back-to-back half-sweeps with
             # programmatic dependent launch) -> value;  pass 2: events around every half-sweep -> roofline
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record(stream)
-            fx.run_batch(gauge, OR, OMEGA, max_sweeps=sweeps, eps=-1.0, check_every=sweeps)
+            fx.run_batch(gauge, algo, param, seed=7, max_sweeps=sweeps, eps=-1.0, check_every=sweeps, reunit_every=ru)
             e1.record(stream)
             stream.synchronize()
             ms = e0.elapsed_time(e1)
             gf.gf_kernel_timing(fx.ctx, True)
             gf.gf_kernel_time_ms(fx.ctx, reset=True)
-            fx.run_batch(gauge, OR, OMEGA, max_sweeps=sweeps, eps=-1.0, check_every=sweeps)
+            fx.run_batch(gauge, algo, param, seed=7, max_sweeps=sweeps, eps=-1.0, check_every=sweeps, reunit_every=ru)
             kern_ms, kern_n = gf.gf_kernel_time_ms(fx.ctx, reset=True)
             gf.gf_kernel_timing(fx.ctx, False)
         bpsu = bytes_per_site_update(prec, recon, nd)
@@ -456,6 +468,9 @@ def run_ours(args):
             bench_other((32, 32, 32, 32), 0, "sp", 12, 16, 100, "Landau OR, 16 gauge copies of 32^4 per launch, SP-12"),
             bench_other((64, 64, 64, 256), 0, "sp", 12, 1, 50, "Landau OR, 64^3x256, SP-12, accumulating g(x) (a8)", track=True),
             bench_other((64, 64, 64, 256), 2, "dp", 18, 1, 30, "MAG OR, 64^3x256, DP-18"),
+            bench_other((64, 64, 64, 256), 0, "sp", 12, 1, 30, "Landau simulated-annealing heatbath T=1 (Philox), 64^3x256, SP-12", algo=2, param=1.0),
+            bench_other((64, 64, 64, 256), 2, "dp", 18, 1, 20, "MAG simulated-annealing heatbath T=0.5 (Philox), 64^3x256, DP-18", algo=2, param=0.5),
+            bench_other((64, 64, 64, 256), 0, "sp", 12, 1, 30, "Landau stochastic relaxation p=0.5 (Philox), 64^3x256, SP-12", algo=1, param=0.5),
             bench_other((64, 64, 64, 256), 0, "sp", 4, 1, 100, "SU(2) Landau OR, 64^3x256, SP (4 reals per link)", su2=True),
             bench_other((64, 64, 64, 256), 0, "dp", 4, 1, 100, "SU(2) Landau OR, 64^3x256, DP (4 reals per link)", su2=True),
             bench_other((64, 64, 64, 256), 2, "mp", 4, 1, 100, "SU(2) MAG OR, 64^3x256, MP", su2=True),
@@ -477,7 +492,7 @@ def run_ours(args):
             "unit": "site-updates/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": DTYPE_NAMES[args.precision], "data": "synthetic",
-            "config": {"workload": f"{'SU(2) ' if su2 else ''}Landau OR omega=1.7, {lat_name} (BASELINE.json configs[4]), "
+            "config": {"workload": f"{'SU(2) ' if su2 else ''}{'Landau OR omega=1.7' if (GAUGE, ALGO, args.param) == (LANDAU, OR, OMEGA) else f'{args.gauge.capitalize()} {args.algo.upper()} param={args.param:g} (side study)'}, {lat_name} (BASELINE.json configs[4]), "
                                    f"{args.precision.upper()}-{args.recon}, one lattice per GPU",
                        "lattice": list(dims), "precision": args.precision, "recon": args.recon,
                        "step": f"{S} sweeps (= {2 * S} half-sweep kernels) + "

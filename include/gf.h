@@ -203,6 +203,11 @@ int gf_get_slice_sweeps(gf_ctx* ctx, int* sweeps);
  * T_k = T_hi - k (T_hi - T_lo)/(n_steps - 1), each followed by n_micro microcanonical sweeps; every
  * sweep consumes one sweep index starting at first_sweep_index.  *next_sweep_index (may be NULL)
  * receives the first unused index.  Asynchronous.
+ * On contexts with recon = 12 the links are reprojected onto SU(3) after every 16th sweep of the schedule (the
+ * rebuilt third row compounds the norm errors of the two stored rows under large rotations: |1 - det U| grows by
+ * about a third per heatbath or microcanonical sweep).  gf_fix does the same in its annealing and
+ * stochastic-relaxation stages.  Long gf_run loops of GF_SA / GF_MICRO / GF_SR sweeps on recon = 12 contexts
+ * should pass reunit_every <= 16 themselves.
  */
 int gf_anneal(gf_ctx* ctx, int gauge, double T_hi, double T_lo, int n_steps, int n_micro, uint64_t seed,
               uint32_t first_sweep_index, uint32_t* next_sweep_index);

@@ -119,3 +119,27 @@ def test_fig7_temperature_scan(gf):
         frac_below = (F_end - F_at) / (F_end - F_start)
         assert frac_below > 0.88, (gauge, frac_below)
         assert F_end > F_start + 0.3
+
+
+@pytest.mark.parametrize("prec", [SP, DP])
+def test_twelve_real_storage_survives_a_long_annealing_schedule(gf, prec):
+    # 12-real storage compounds the norm errors of its two stored rows under large rotations (|1 - det U| grows by
+    # about a third per heatbath / microcanonical sweep: without reprojection SP-12 is at 1e+7 after 60 sweeps);
+    # gf_anneal and gf_fix reproject every 16 sweeps on such contexts
+    dims = (8, 8, 8, 8)
+    dt = np.float64 if prec == DP else np.float32
+    L = inputs.as_real(inputs.make_config(*dims, 0.5, 33, 34), dt)
+    with gf.GaugeFixer(*dims, precision=prec, recon=12) as fx:
+        fx.set_links(L)
+        fx.anneal(0, 2.0, 0.05, 60, 3, seed=3)                 # 240 sweeps, T from 2 down
+        avg, mx = fx.unitarity()
+        assert mx[0] < (1e-3 if prec == SP else 1e-11), mx[0]
+        fx.set_links(L)
+        r = fx.fix(0, seed=3, sa_steps=40, sa_T_hi=1.0, sa_T_lo=0.01, sa_micro=3, sr_max_sweeps=60, sr_p=0.5,
+                   or_omega=1.7, or_max_sweeps=20000, eps=1e-12 if prec == DP else 1e-9, check_every=5, reunit_every=0 if prec == DP else 50)[0]
+        assert r["converged"] and np.isfinite(r["F"]) and r["F"] > 0.7
+        # and what happens without: raw sweeps, no reprojection
+        fx.set_links(L)
+        for s in range(40):
+            fx.sweep(0, gf.GF_MICRO, 0.0, seed=3, sweep_index=s)
+        assert fx.unitarity()[1][0] > 100 * (4e-6 if prec == SP else 1e-14)
