@@ -112,16 +112,21 @@ GF_DEV void rule_heatbath_landau(const double a[4], double T, uint64_t seed, uin
         g[0] = 1.0; g[1] = g[2] = g[3] = 0.0;
         return;
     }
-    const double norm = sqrt(n2);
-    const double alpha = norm / T;
-    const double h0 = a[0] / norm, h1 = -a[1] / norm, h2 = -a[2] / norm, h3 = -a[3] / norm;
+    // one reciprocal square root and one reciprocal instead of a square root and six divisions; pi-scaled
+    // trigonometric functions (exact argument reduction).  The oracle writes the same quantities with sqrt, / and
+    // cos(2 pi r): the values agree to an ulp or two, the accept decisions but for events of probability ~1e-16.
+    const double inv_norm = rsqrt(n2);
+    const double norm = n2 * inv_norm;
+    const double alpha = norm * (1.0 / T);
+    const double inv_alpha = T * inv_norm;
+    const double h0 = a[0] * inv_norm, h1 = -a[1] * inv_norm, h2 = -a[2] * inv_norm, h3 = -a[3] * inv_norm;
     double u0 = 1.0;
     if (alpha >= 2.0) {
         for (uint32_t trial = 0; trial < GF_HB_MAX_TRIALS; ++trial) {
             const u32x4 r = rng_draw(seed, site, sweep, sub, 1, trial);
             const double r1 = uniform01(r.x), r2 = uniform01(r.y), r3 = uniform01(r.z), r4 = uniform01(r.w);
-            const double cs = cos(GF_TWO_PI * r2);
-            const double delta = -(log(r1) + cs * cs * log(r3)) / alpha;
+            const double cs = cospi(2.0 * r2);
+            const double delta = -(log(r1) + cs * cs * log(r3)) * inv_alpha;
             u0 = 1.0 - delta;
             if (r4 * r4 <= 1.0 - 0.5 * delta) break;
         }
@@ -131,23 +136,24 @@ GF_DEV void rule_heatbath_landau(const double a[4], double T, uint64_t seed, uin
             const u32x4 r = rng_draw(seed, site, sweep, sub, 1, trial);
             const double r1 = uniform01(r.x), r2 = uniform01(r.y);
             const double x = em + (1.0 - em) * r1;
-            u0 = 1.0 + log(x) / alpha;
+            u0 = 1.0 + log(x) * inv_alpha;
             if (r2 * r2 <= 1.0 - u0 * u0) break;
         }
     }
     u0 = fmin(1.0, fmax(-1.0, u0));
     const u32x4 rd = rng_draw(seed, site, sweep, sub, 2, 0);
     const double ct = 2.0 * uniform01(rd.x) - 1.0;
-    const double phi = GF_TWO_PI * uniform01(rd.y);
+    double sphi, cphi;
+    sincospi(2.0 * uniform01(rd.y), &sphi, &cphi);
     const double st = sqrt(fmax(0.0, 1.0 - ct * ct));
     const double rad = sqrt(fmax(0.0, 1.0 - u0 * u0));
-    const double u1 = rad * st * cos(phi), u2 = rad * st * sin(phi), u3 = rad * ct;
+    const double u1 = rad * st * cphi, u2 = rad * st * sphi, u3 = rad * ct;
     // g = u * g_hat as 2x2 matrices of Eq. (22): (pq)_0 = p0 q0 - p.q, (pq)_vec = p0 q + q0 p - p x q
     const double q0 = u0 * h0 - u1 * h1 - u2 * h2 - u3 * h3;
     const double q1 = u0 * h1 + h0 * u1 - (u2 * h3 - u3 * h2);
     const double q2 = u0 * h2 + h0 * u2 - (u3 * h1 - u1 * h3);
     const double q3 = u0 * h3 + h0 * u3 - (u1 * h2 - u2 * h1);
-    const double rn = 1.0 / sqrt(q0 * q0 + q1 * q1 + q2 * q2 + q3 * q3);
+    const double rn = rsqrt(q0 * q0 + q1 * q1 + q2 * q2 + q3 * q3);
     g[0] = q0 * rn; g[1] = q1 * rn; g[2] = q2 * rn; g[3] = q3 * rn;
 }
 
@@ -161,10 +167,11 @@ GF_DEV void rule_heatbath_mag(double D, double E, double F, double T, uint64_t s
     }
     const u32x4 r = rng_draw(seed, site, sweep, sub, 1, 0);
     const double r1 = uniform01(r.x), r2 = uniform01(r.y);
-    double cg = 1.0 + (T / lam) * log(1.0 - r1 * (1.0 - exp(-2.0 * lam / T)));
+    const double inv_lam = 1.0 / lam;
+    double cg = 1.0 + (T * inv_lam) * log(1.0 - r1 * (1.0 - exp(-2.0 * lam / T)));
     cg = fmin(1.0, fmax(-1.0, cg));
     const double sg = sqrt(fmax(0.0, 1.0 - cg * cg));
-    const double X0 = E / lam, X1 = F / lam, X2 = D / lam;
+    const double X0 = E * inv_lam, X1 = F * inv_lam, X2 = D * inv_lam;
     double e10 = -X1, e11 = X0, e12 = 0.0;
     const double n1 = sqrt(e10 * e10 + e11 * e11);
     if (n1 < 1e-150) {
@@ -173,8 +180,8 @@ GF_DEV void rule_heatbath_mag(double D, double E, double F, double T, uint64_t s
         e10 /= n1; e11 /= n1;
     }
     const double e20 = X1 * e12 - X2 * e11, e21 = X2 * e10 - X0 * e12, e22 = X0 * e11 - X1 * e10;
-    const double az = GF_TWO_PI * r2;
-    const double ca = cos(az), sa = sin(az);
+    double sa, ca;
+    sincospi(2.0 * r2, &sa, &ca);
     const double p0 = cg * X0 + sg * (ca * e10 + sa * e20);
     const double p1 = cg * X1 + sg * (ca * e11 + sa * e21);
     const double p2 = cg * X2 + sg * (ca * e12 + sa * e22);
@@ -184,8 +191,9 @@ GF_DEV void rule_heatbath_mag(double D, double E, double F, double T, uint64_t s
         return;
     }
     const double g0 = sqrt(h);
-    const double g1 = p0 / (2.0 * g0), g2 = p1 / (2.0 * g0);
-    const double rn = 1.0 / sqrt(g0 * g0 + g1 * g1 + g2 * g2);
+    const double hg = 0.5 / g0;
+    const double g1 = p0 * hg, g2 = p1 * hg;
+    const double rn = rsqrt(g0 * g0 + g1 * g1 + g2 * g2);
     g[0] = g0 * rn; g[1] = g1 * rn; g[2] = g2 * rn; g[3] = 0.0;
 }
 
