@@ -716,7 +716,8 @@ void gfo_apply_subgroup_d(double* mat18, const double* g4, int i, int j, int whi
     store<double>(mat18, U);
 }
 
-// Random start on the gauge orbit (reading R27): h(x) Haar on SU(3) from two rows of
+// Random start on the gauge orbit (reading R27; how the paper drew its starts is not stated:
+// the Haar law is pinned by its moments, the Philox keying is "parity unpinned"): h(x) Haar on SU(3) from two rows of
 // complex standard normals, Box-Muller on the Philox uniforms of counter (site, 0, k | 3<<8, 0), k=0..2:
 // normals 4k..4k+3 = sqrt(-2 ln u0)(cos, sin)(2 pi u1), sqrt(-2 ln u2)(cos, sin)(2 pi u3); then the
 // Gram-Schmidt reprojection above.  h: [V][3][3][2] doubles in site order.

@@ -13,6 +13,8 @@
 //   the Landau heatbath rule of gf_oracle.cpp at temperature T = 3/beta — and U <- g~ U.
 // Order of a sweep: for mu = 0..3, for parity = even, odd: all links U_mu(x) with x of that parity (they
 // share no plaquette).  Random numbers: counter (site, 4*sweep_index + mu, sub | purpose << 8, trial).
+// The paper gives nothing to compare this generator with: "parity unpinned" against the paper (R30), pinned
+// by the mathematics below and oracle <-> GPU.
 // Pins (tests/test_oracle_wilson.py): plaquette against an independent NumPy evaluation; strong-coupling
 // <P> = beta/18 + beta^2/216; weak-coupling 1 - <P> -> 2/beta; beta -> infinity raises every local action
 // term monotonically; unitarity; SU(2)-subgroup single-link law (u0 density) through the pinned rule.
