@@ -7,7 +7,7 @@
  * CPU fallback: without a CUDA device gf_create fails with GF_ECUDA.
  *
  * Conventions common to all calls
- *   - Return value: 0 = GF_OK, 1 = GF_NOT_CONVERGED (gf_run only), < 0 = error.  No exception or
+ *   - Return value: 0 = GF_OK, 1 = GF_NOT_CONVERGED (gf_run, gf_run_batch, gf_fix), < 0 = error.  No exception or
  *     abort crosses the ABI.  gf_last_error(ctx) returns a ctx-owned, NUL-terminated description of
  *     the last error (valid until the next call on that ctx).
  *   - A context owns all of its device memory.  The caller owns every pointer it passes in; the
@@ -40,7 +40,7 @@ typedef struct gf_ctx gf_ctx; /* opaque */
 
 /* return codes */
 #define GF_OK 0
-#define GF_NOT_CONVERGED 1
+#define GF_NOT_CONVERGED 1 /* gf_run / gf_run_batch / gf_fix: max_sweeps reached before every unit had theta < eps */
 #define GF_EINVAL (-1) /* bad argument (odd extent, unknown gauge/algo, NULL pointer, ...) */
 #define GF_ENOMEM (-2) /* device or host allocation failed */
 #define GF_ECUDA (-3)  /* a CUDA runtime call or kernel launch failed; see gf_last_error */
