@@ -227,7 +227,7 @@ __global__ void measure_kernel(const char* links, Dims d, double* partial, int64
                     sum += 0.25 * (xr * xr + xi * xi);
                     if (a == b) tr += 0.5 * xi;   // (X/2i)_aa = Im-part
                 }
-            th_term = sum - tr * tr / 3.0;
+            th_term = fmax(0.0, sum - tr * tr / 3.0);
         }
     }
     block_sum2(f_term, th_term);

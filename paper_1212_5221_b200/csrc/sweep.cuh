@@ -222,7 +222,8 @@ GF_DEV A theta_term_landau(const Mat<A>& K) {
             sum += A(0.25) * (xr * xr + xi * xi);
             if (a == b) tr += A(0.5) * xi;
         }
-    return sum - tr * tr / A(3);
+    const A th = sum - tr * tr / A(3);   // = tr[Delta Delta^dag] >= 0; rounding can leave -1e-23 at a fixed point
+    return th > A(0) ? th : A(0);
 }
 template <class A>
 GF_DEV A f_term_landau(const Mat<A>& K) { return K.v[RE(0, 0)] + K.v[RE(1, 1)] + K.v[RE(2, 2)]; }
