@@ -206,8 +206,9 @@ int gf_get_slice_sweeps(gf_ctx* ctx, int* sweeps);
  * On contexts with recon = 12 the links are reprojected onto SU(3) after every 16th sweep of the schedule (the
  * rebuilt third row compounds the norm errors of the two stored rows under large rotations: |1 - det U| grows by
  * about a third per heatbath or microcanonical sweep).  gf_fix does the same in its annealing and
- * stochastic-relaxation stages.  Long gf_run loops of GF_SA / GF_MICRO / GF_SR sweeps on recon = 12 contexts
- * should pass reunit_every <= 16 themselves.
+ * stochastic-relaxation stages, and gf_run / gf_run_batch with GF_SA, GF_MICRO or GF_SR on such a context use
+ * reunit_every = 16 when asked for none or for a longer interval.  (Sequences of single gf_sweep calls are the
+ * caller's: call gf_reunitarize.)
  */
 int gf_anneal(gf_ctx* ctx, int gauge, double T_hi, double T_lo, int n_steps, int n_micro, uint64_t seed,
               uint32_t first_sweep_index, uint32_t* next_sweep_index);

@@ -709,6 +709,10 @@ int gf_coulomb_finalize(gf_ctx* ctx) {
 }
 
 // ---- run loops -----------------------------------------------------------------------------------
+// sweeps of heatbath / microcanonical / stochastic-relaxation type on 12-real contexts are reprojected at least this
+// often (see the comment above anneal_impl and DESIGN.md §7)
+static const int GF_RECON12_REUNIT = 16;
+
 static int sweep_gx(const gf_ctx* ctx) {
     const int Vsh = ctx->Nx * ctx->Ny * (ctx->Nz / 2);
     const int block = (ctx->nc == 2)           ? sweep_su2_block(Vsh, ctx->block_override)
@@ -759,6 +763,8 @@ static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t see
     if (max_sweeps < 0 || check_every < 1 || reunit_every < 0) return fail(ctx, GF_EINVAL, "gf_run: bad loop arguments");
     rc = pre_sweep(ctx, gauge);
     if (rc) return rc;
+    if (algo != GF_OR && ctx->recon == 12 && (reunit_every == 0 || reunit_every > GF_RECON12_REUNIT))
+        reunit_every = GF_RECON12_REUNIT;
     const bool fused = ctx->fused != 0;
     const bool coulomb = gauge == GF_COULOMB;
     const bool per_slice = coulomb && (ctx->flags & GF_FLAG_FREEZE_SLICES);
@@ -981,13 +987,12 @@ int gf_get_slice_sweeps(gf_ctx* ctx, int* sweeps) {
     return GF_OK;
 }
 
+// (GF_RECON12_REUNIT is defined above run_impl)
 // With 12-real storage the third row is rebuilt as (u x v)^* from stored rows that are never re-orthonormalised:
 // a rotation that mixes it back into the stored rows compounds their norm errors, and under the large rotations of
 // heatbath and microcanonical sweeps |1 - det U| grows by about a third per sweep (measured: 7e-6 -> 1e+7 in 60
 // sweeps in SP, 6e-14 -> 2e-7 in DP; overrelaxation near a maximum is benign).  Schedules made of such sweeps
 // therefore reproject at least this often on 12-real contexts.
-static const int GF_RECON12_REUNIT = 16;
-
 // the annealing schedule; reunit_every > 0 reprojects after every reunit_every-th sweep of the schedule
 static int anneal_impl(gf_ctx* ctx, int gauge, double T_hi, double T_lo, int n_steps, int n_micro, uint64_t seed,
                        uint32_t first_sweep_index, int reunit_every, uint32_t* next_sweep_index) {
@@ -1046,10 +1051,9 @@ int gf_fix(gf_ctx* ctx, const gf_fix_params* p, gf_result* out) {
         for (int sl = 0; sl < NS; ++sl) total[(size_t)sl] += (int)idx;
     }
     if (p->sr_max_sweeps > 0) {   // stage 2: stochastic relaxation until theta < eps, at most sr_max_sweeps
-        int sr_reunit = p->reunit_every;   // stochastic relaxation takes microcanonical steps: see GF_RECON12_REUNIT
-        if (ctx->recon == 12 && (sr_reunit == 0 || sr_reunit > GF_RECON12_REUNIT)) sr_reunit = GF_RECON12_REUNIT;
+        // (stochastic relaxation takes microcanonical steps: run_impl applies GF_RECON12_REUNIT on 12-real contexts)
         rc = run_impl(ctx, p->gauge, GF_SR, p->sr_p, p->seed, idx, p->sr_max_sweeps, p->eps, p->check_every,
-                      sr_reunit, nullptr, res.data(), nullptr, &all);
+                      p->reunit_every, nullptr, res.data(), nullptr, &all);
         if (rc) return rc;
         have_res = true;
         for (int sl = 0; sl < NS; ++sl) total[(size_t)sl] += ctx->slice_sweeps[(size_t)sl];
