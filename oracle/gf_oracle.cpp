@@ -18,7 +18,8 @@
 // Parity pins (tests/test_oracle_*.py): pure gauge -> F=1, theta->0; plaquette invariance;
 // unitarity/det; monotone F at omega=1; exact F-invariance of microcanonical sweeps;
 // one-site brute force of Step 1 (Landau and MAG); Coulomb slice == standalone 3-d problem;
-// heatbath histograms vs closed-form densities, T->0 limit; Philox known answers.
+// heatbath histograms vs closed-form densities, T->0 limit; Philox known answers; theta_MAG (both forms) vs
+// Eq. (12) evaluated with NumPy matrices on a rough field and vs the N_c = 2 value on embedded SU(2) links.
 // "parity unpinned" items (no value in the paper pins them; any fixed choice is a valid
 // algorithm): subgroup order (R6), MAG heatbath construction (R15), Philox keying (R19).
 // =====================================================================================

@@ -44,7 +44,9 @@ struct gf_ctx {
     size_t real_bytes;      // 4 | 8
     char* links;            // device link store
     char* gtot;             // tracked transform (18 reals/site) or nullptr
-    char* gapplied;         // part of gtot already applied to the temporal links (Coulomb) or nullptr
+    char* gapplied;         // snapshot of gtot taken when Coulomb sweeps start: the part already applied to the temporal links
+    bool gapp_valid;        // the pending finalisation uses R = gtot gapplied^dag (false: gtot was the identity, R = gtot)
+    std::vector<unsigned char> gtot_ident;   // per copy: gtot is still the identity set by reset_transform
     bool have_links;        // every copy has received links
     std::vector<unsigned char> copies_set;
     bool temporal_stale;    // Coulomb sweeps ran since the temporal links were last finalised
@@ -162,6 +164,8 @@ int gf_create_batch(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int n_copies, 
     ctx->real_bytes = (precision == GF_DP) ? 8 : 4;
     ctx->links = ctx->gtot = ctx->gapplied = nullptr;
     ctx->have_links = false; ctx->temporal_stale = false;
+    ctx->gapp_valid = false;
+    ctx->gtot_ident.assign((size_t)n_copies, 1);
     ctx->partial = nullptr; ctx->slice_dev = nullptr; ctx->slice_host = nullptr;
     ctx->red_part[0] = ctx->red_part[1] = nullptr; ctx->red_dev = nullptr; ctx->red_host = nullptr;
     ctx->fused = 1;
@@ -298,16 +302,15 @@ static int reset_transform(gf_ctx* ctx, int copy) {
         int rc = field_identity(ctx, ctx->gtot + copy * field_store_bytes(ctx));
         if (rc) return rc;
     }
-    if (ctx->gapplied) {
-        if (ctx->B == 1) {
-            CU(cudaStreamSynchronize(ctx->stream));
-            cudaFree(ctx->gapplied);
-            ctx->gapplied = nullptr;
-            ctx->device_bytes -= field_store_bytes(ctx);
-        } else {
-            int rc = field_identity(ctx, ctx->gapplied + copy * field_store_bytes(ctx));
-            if (rc) return rc;
-        }
+    ctx->gtot_ident[(size_t)copy] = 1;
+    // gapplied is a snapshot taken at the next start of Coulomb sweeps (coulomb_begin); nothing to reset here.
+    // A single lattice gives the memory back (a transform field is 1/4 of an 18-real link store).
+    if (ctx->gapplied && ctx->B == 1) {
+        CU(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->gapplied);
+        ctx->gapplied = nullptr;
+        ctx->gapp_valid = false;
+        ctx->device_bytes -= field_store_bytes(ctx);
     }
     if (ctx->B == 1) ctx->temporal_stale = false;
     return GF_OK;
@@ -526,13 +529,41 @@ static int launch_half(gf_ctx* ctx, int gauge, int algo, double param, uint64_t 
     return GF_OK;
 }
 
-static int pre_sweep(gf_ctx* ctx, int gauge) {
-    if (gauge == GF_COULOMB) {
-        if (ctx->gtot) ctx->temporal_stale = true;
-    } else if (ctx->temporal_stale) {
-        return gf_coulomb_finalize(ctx);
+// Coulomb sweeps are about to start on temporal links that are up to date: whatever g(x) has accumulated so far
+// (Landau / MAG sweeps, gf_random_gauge) has been applied to U_0 already, so the finalisation that follows must
+// apply only what the Coulomb sweeps add, R = g_now g_start^dag.  Snapshot g_start (nothing to do while every
+// copy's g is still the identity of gf_set_links).
+static int coulomb_begin(gf_ctx* ctx) {
+    bool all_ident = true;
+    for (unsigned char f : ctx->gtot_ident) all_ident = all_ident && f;
+    if (all_ident) {
+        ctx->gapp_valid = false;
+    } else {
+        if (!ctx->gapplied) {
+            CU(cudaMalloc((void**)&ctx->gapplied, (size_t)(ctx->B * field_store_bytes(ctx))));
+            ctx->device_bytes += ctx->B * field_store_bytes(ctx);
+        }
+        CU(cudaMemcpyAsync(ctx->gapplied, ctx->gtot, (size_t)(ctx->B * field_store_bytes(ctx)), cudaMemcpyDeviceToDevice,
+                           ctx->stream));
+        ctx->gapp_valid = true;
     }
+    ctx->temporal_stale = true;
     return GF_OK;
+}
+
+static void transform_changed(gf_ctx* ctx) {
+    if (ctx->gtot) ctx->gtot_ident.assign((size_t)ctx->B, 0);
+}
+
+static int pre_sweep(gf_ctx* ctx, int gauge) {
+    int rc = GF_OK;
+    if (gauge == GF_COULOMB) {
+        if (ctx->gtot && !ctx->temporal_stale) rc = coulomb_begin(ctx);
+    } else if (ctx->temporal_stale) {
+        rc = gf_coulomb_finalize(ctx);
+    }
+    transform_changed(ctx);
+    return rc;
 }
 
 int gf_half_sweep(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t sweep_index,
@@ -679,32 +710,27 @@ int gf_reunitarize(gf_ctx* ctx) {
 // ---- Coulomb finalisation ------------------------------------------------------------------------
 #define FINALIZE(R, RECON, dummy)                                                                           \
     coulomb_finalize_kernel<R, RECON><<<dim3((unsigned)((2 * ctx->Vh + 127) / 128), (unsigned)ctx->B), 128, 0, ctx->stream>>>( \
-        ctx->links, ctx->gtot, ctx->gapplied, dims_of(ctx), link_store_bytes(ctx), field_store_bytes(ctx))
+        ctx->links, ctx->gtot, gapp, dims_of(ctx), link_store_bytes(ctx), field_store_bytes(ctx))
 
 int gf_coulomb_finalize(gf_ctx* ctx) {
     if (!ctx) return GF_EINVAL;
     if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_coulomb_finalize: no links set");
     if (!ctx->gtot) return fail(ctx, GF_ESTATE, "gf_coulomb_finalize: context created without GF_FLAG_TRACK_TRANSFORM");
     if (!ctx->temporal_stale) return GF_OK;
+    const char* gapp = ctx->gapp_valid ? ctx->gapplied : nullptr;   // the g(x) the Coulomb sweeps started from
     if (ctx->nc == 2) {
         const dim3 g((unsigned)((2 * ctx->Vh + 127) / 128), (unsigned)ctx->B);
         if (ctx->real_bytes == 4)
-            coulomb_finalize2_kernel<float><<<g, 128, 0, ctx->stream>>>(ctx->links, ctx->gtot, ctx->gapplied, dims_of(ctx),
+            coulomb_finalize2_kernel<float><<<g, 128, 0, ctx->stream>>>(ctx->links, ctx->gtot, gapp, dims_of(ctx),
                                                                         link_store_bytes(ctx), field_store_bytes(ctx));
         else
-            coulomb_finalize2_kernel<double><<<g, 128, 0, ctx->stream>>>(ctx->links, ctx->gtot, ctx->gapplied, dims_of(ctx),
+            coulomb_finalize2_kernel<double><<<g, 128, 0, ctx->stream>>>(ctx->links, ctx->gtot, gapp, dims_of(ctx),
                                                                          link_store_bytes(ctx), field_store_bytes(ctx));
     } else
         DISPATCH_RR(ctx, FINALIZE, 0);
     CU(cudaGetLastError());
     ++ctx->launches;
-    if (!ctx->gapplied) {
-        CU(cudaMalloc((void**)&ctx->gapplied, (size_t)(ctx->B * field_store_bytes(ctx))));
-        ctx->device_bytes += ctx->B * field_store_bytes(ctx);
-    }
-    CU(cudaMemcpyAsync(ctx->gapplied, ctx->gtot, (size_t)(ctx->B * field_store_bytes(ctx)), cudaMemcpyDeviceToDevice,
-                       ctx->stream));
-    ctx->temporal_stale = false;
+    ctx->temporal_stale = false;   // the next start of Coulomb sweeps takes a new snapshot (coulomb_begin)
     return GF_OK;
 }
 
@@ -1123,10 +1149,8 @@ int gf_random_gauge(gf_ctx* ctx, uint64_t seed) {
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
     cudaFree(h);
     CU(e);
-    // the transform just applied counts as already applied to the temporal links
-    if (ctx->gapplied)
-        CU(cudaMemcpyAsync(ctx->gapplied, ctx->gtot, (size_t)(ctx->B * field_store_bytes(ctx)), cudaMemcpyDeviceToDevice,
-                           ctx->stream));
+    // h was applied to all four directions: Coulomb sweeps that follow snapshot g(x) = h g(x) as already applied
+    transform_changed(ctx);
     return GF_OK;
 }
 

@@ -310,6 +310,66 @@ def test_theta_zero_iff_stationary_mag(oracle):
     assert m["theta_literal"] <= 3 * m["theta"] + 1e-30
 
 
+def _x_mag(U, sigma):
+    """X(x) = sum_mu [ U_mu(x) sigma U_mu(x)^dag + U_mu(x-mu)^dag sigma U_mu(x-mu) ] of Eq. (12) at
+    every site, from the complex links U[t,x,y,z,mu,n,n]; sigma a diagonal matrix.  Returns [t,x,y,z,n,n]."""
+    X = 0
+    for mu in range(4):
+        W = U[..., mu, :, :]
+        Wd = np.roll(W, 1, axis=mu)                      # U_mu(x - mu)
+        X = X + W @ sigma @ H.dag(W) + H.dag(Wd) @ sigma @ Wd
+    return X
+
+
+def test_theta_mag_su3_from_eq12_matrices(oracle):
+    # Eqs. (12), (13), (16) (PAPER.md:109-131) in the reading R11: for the subgroup s = (i,j) sigma_3 is the 3x3
+    # matrix diag(+1 at i, -1 at j); X^s(x) is Eq. (12) with it, its (i,j) element the quantity whose modulus
+    # squared enters theta.  Stopping theta = sum_x sum_s |X^s_ij|^2 / (N_c V); the literal Eq. (16) puts the sum
+    # over s inside the modulus.  Everything below is NumPy matrix algebra on a rough random field: a wrong
+    # prefactor, a dropped subgroup, a dropped up/down term or a transposed link fails it.
+    dims = (4, 4, 4, 6)
+    U = small_config(36, dims=dims, eps=0.6)
+    V = int(np.prod(dims))
+    tot = 0.0
+    lit = 0
+    for (i, j) in ((0, 1), (0, 2), (1, 2)):
+        sig = np.zeros((3, 3))
+        sig[i, i], sig[j, j] = 1.0, -1.0
+        X = _x_mag(U, sig)
+        assert np.abs(X - H.dag(X)).max() < 1e-13 and np.abs(np.trace(X, axis1=-2, axis2=-1)).max() < 1e-13
+        tot += (np.abs(X[..., i, j]) ** 2).sum()
+        lit = lit + X[..., i, j]
+    m = oracle.measure(inputs.as_real(U), MAG)
+    assert m["theta"] > 1e-2                              # far from stationary: a non-trivial expected value
+    assert m["theta"] == pytest.approx(tot / (3 * V), rel=1e-13)
+    assert m["theta_literal"] == pytest.approx((np.abs(lit) ** 2).sum() / (3 * V), rel=1e-13)
+    # the per-slice values are the same sums restricted to a slice (V -> Nx Ny Nz)
+    th_t = 0
+    for (i, j) in ((0, 1), (0, 2), (1, 2)):
+        sig = np.zeros((3, 3))
+        sig[i, i], sig[j, j] = 1.0, -1.0
+        th_t = th_t + (np.abs(_x_mag(U, sig)[..., i, j]) ** 2).sum(axis=(1, 2, 3))
+    assert np.allclose(m["theta_slice"], th_t / (3 * V / U.shape[0]), rtol=1e-13, atol=0)
+
+
+def test_theta_mag_su3_reduces_to_su2_on_embedded_links(oracle):
+    # links that are SU(2) matrices in the (0,1) block of the 3x3 identity: the subgroups (0,2) and (1,2) see
+    # diagonal blocks (X^s_ij = 0) and the (0,1) subgroup sees the SU(2) problem, so the N_c = 3 value is the
+    # N_c = 2 oracle's theta (pinned by Eq. (12)/(13) in tests/test_oracle_su2.py) times 2/3; F of Eq. (11):
+    # 3 F_3 = 2 F_2 + 1 per link
+    dims = (4, 4, 4, 4)
+    u = inputs.make_config_su2(*dims, 0.5, 81, 82)
+    U = np.zeros(dims + (4, 3, 3), dtype=np.complex128)
+    U[..., :2, :2] = u
+    U[..., 2, 2] = 1.0
+    m3 = oracle.measure(inputs.as_real(U), MAG)
+    m2 = oracle.measure(inputs.as_real(u), MAG)
+    assert m2["theta"] > 1e-3
+    assert m3["theta"] == pytest.approx(2.0 * m2["theta"] / 3.0, rel=1e-13)
+    assert m3["theta_literal"] == pytest.approx(m3["theta"], rel=1e-13)
+    assert m3["F"] == pytest.approx((2.0 * m2["F"] + 1.0) / 3.0, rel=1e-13)
+
+
 # ------------------------------------------------------------------------------------------
 # Coulomb: time-slices are independent problems (PAPER.md:76, 376; DESIGN.md R21/R22)
 # ------------------------------------------------------------------------------------------
