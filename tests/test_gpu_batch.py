@@ -62,14 +62,69 @@ def test_batch_sweep_per_copy(gf, oracle, prec, recon, gauge, algo, param):
             got = fx.get_links_copy(c, dtype=dt)
             tol = TOL_SWEEP[prec] * (10 if algo == SA and prec == DP else 1)    # BASELINE: 1e-11 for annealing
             gg = fx.get_gauge_transform_copy(c, dtype=dt)
-            for diff in (np.abs(got.astype(np.float64) - ref), np.abs(gg.astype(np.float64) - g)):
-                if algo == SA and prec == SP:
-                    # float Step 1: where the local field is weak (|a| or lambda of Eq. (29) small) the heatbath
-                    # direction is ill conditioned and float rounding of the neighbourhood sums (different
-                    # association on the two paths) is amplified by 1/|a|; rare sites, bounded separately
-                    assert np.quantile(diff, 0.99) <= tol and diff.max() <= 40 * tol, c
-                else:
-                    assert diff.max() <= tol, c
+            dl, dg = np.abs(got.astype(np.float64) - ref), np.abs(gg.astype(np.float64) - g)
+            if algo == SA and prec == SP:
+                # float Step 1: where the local field is weak (|a| of Eq. (20), lambda or sqrt(E^2+F^2) of Eq. (29))
+                # the heatbath direction is ill conditioned and the float rounding of the neighbourhood sums
+                # (different association on the two paths) is amplified by its inverse.  The quantitative bound is
+                # tested half-sweep by half-sweep in test_sp_heatbath_half_sweep_within_conditioning_bound; here,
+                # after the two half-sweeps: 99 % of all reals within BASELINE.json's 5e-5, and every link above it was
+                # rotated by a weak-field site (conditioning number below 0.1, taken from the oracle) or by an odd site
+                # that gathered a link from one (the odd half-sweep passes the even sites' differences on).
+                from tests import conditioning
+                assert np.quantile(dl, 0.99) <= tol and np.quantile(dg, 0.99) <= tol, c
+                mid = Ls[c].copy()
+                oracle.sweep(mid, gauge, algo, param, seed + c, 7, parity_mask=1)
+                pre = (Ls[c].astype(np.float64), mid.astype(np.float64))
+                n4 = dl.shape[:4]
+                cond = {}
+                for t, x, y, z, mu in zip(*np.nonzero(dl.max(axis=(-1, -2, -3)) > tol)):
+                    a = (int(t), int(x), int(y), int(z))
+                    b = tuple((v + (k == mu)) % n for k, (v, n) in enumerate(zip(a, n4)))
+                    odd = a if sum(a) & 1 else b
+                    sites = {a, b}
+                    for k in range(4):
+                        for sgn in (-1, 1):
+                            sites.add(tuple((v + sgn * (kk == k)) % n for kk, (v, n) in enumerate(zip(odd, n4))))
+                    for e in sites:
+                        if e not in cond:
+                            cond[e] = conditioning.site_conditioning(oracle, pre[sum(e) & 1], e, gauge, param, seed + c, 7)
+                    assert min(cond[e] for e in sites) < 0.1, (c, a, int(mu), float(dl[t, x, y, z, mu].max()))
+            else:
+                assert dl.max() <= tol and dg.max() <= tol, c
+
+
+@pytest.mark.parametrize("recon", [12, 18])
+@pytest.mark.parametrize("gauge,T", [(LANDAU, 1.1), (MAG, 0.8), (MAG, 0.1)])
+def test_sp_heatbath_half_sweep_within_conditioning_bound(gf, oracle, recon, gauge, T):
+    # SP heatbath against the oracle, one half-sweep at a time from identical float links, every link and every g(x)
+    # held to C * 2^-23 * (1 + 2d / c(x)) with c(x) the weakest local field of the updating site (tests/conditioning.py;
+    # c from oracle.local_quaternion / local_mag_def).  The bound is below BASELINE.json's 5e-5 for all (Landau) or all but
+    # a few per cent (MAG) of the links, so this is the 5e-5 test with the ill-conditioned sites accounted for one by one.
+    from tests import conditioning
+    dims = (6, 4, 8, 6)
+    B = 2
+    Ls = copies(dims, B, dtype=np.float32)
+    seed = 4321
+    with gf.GaugeFixer(*dims, precision=SP, recon=recon, n_copies=B, track_transform=True) as fx:
+        for parity in (0, 1):
+            for c in range(B):
+                fx.set_links_copy(c, Ls[c])
+            fx.half_sweep(gauge, SA, T, seed, 7, parity)
+            for c in range(B):
+                ref = Ls[c].copy()
+                g = oracle.identity_transform(ref)
+                oracle.sweep(ref, gauge, SA, T, seed + c, 7, gtot=g, parity_mask=1 << parity)
+                bl, bg, cmin = conditioning.half_sweep_error_bound(oracle, Ls[c], gauge, T, seed + c, 7, parity)
+                dl = np.abs(fx.get_links_copy(c, dtype=np.float32).astype(np.float64) - ref).max(axis=(-1, -2, -3))
+                dg = np.abs(fx.get_gauge_transform_copy(c, dtype=np.float32).astype(np.float64) - g).max(axis=(-1, -2, -3))
+                assert np.all(dl <= bl), (c, parity, float((dl / bl).max()))
+                assert np.all(dg <= bg + 1e-30), (c, parity)
+                # the bound is not vacuous: below 5e-5 on every Landau link and on > 92 % of the MAG links (whose three
+                # conditioning numbers are small more often: lambda, sqrt(E^2+F^2) and g_0), typically 2e-6 .. 1e-5
+                frac, med = float(np.mean(bl <= 5e-5)), float(np.median(bl))
+                assert frac >= (0.999 if gauge == LANDAU else 0.92) and med <= 1.5e-5, (frac, med)
+                Ls[c] = ref          # the odd half-sweep starts from the oracle's links on both paths
 
 
 def test_batch_set_links_broadcasts_and_single_calls_refuse(gf, oracle):

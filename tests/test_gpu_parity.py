@@ -240,7 +240,14 @@ def test_config1_full_run(gf, oracle):
     assert conv and r["converged"]
     assert abs(r["F"] - F) <= 1e-10
     assert r["theta"] < 1e-12 and abs(r["theta"] - th) <= 0.1 * th
-    assert abs(r["sweeps"] - s) <= 2
+    # the stopping sweep is an integer decision taken on a floating-point theta (both sides in double): it must be the
+    # decision the oracle's own theta history dictates, up to the relative agreement of the two theta values (1e-3
+    # of eps here; the histories agree to 1e-4 below) — i.e. the same sweep unless theta crosses eps within that band
+    th_o = np.array([h[2] for h in hist])
+    n_g = r["sweeps"]
+    assert n_g <= len(th_o) and th_o[n_g - 1] < 1e-12 * (1 + 1e-3) and np.all(th_o[:n_g - 1] >= 1e-12 * (1 - 1e-3))
+    if not (abs(th_o[s - 1] / 1e-12 - 1) < 1e-3 or (s > 1 and abs(th_o[s - 2] / 1e-12 - 1) < 1e-3)):
+        assert n_g == s
     n = min(len(hist), len(r["history"]))
     np.testing.assert_allclose(r["history"][:n, 1], [h[1] for h in hist][:n], atol=1e-10)
     np.testing.assert_allclose(r["history"][:n - 5, 2], [h[2] for h in hist][:n - 5], rtol=1e-4)

@@ -71,10 +71,7 @@ def test_one_sweep_per_link(gf, oracle, prec, gauge, algo, param):
         gg = fx.get_gauge_transform(dtype=dt)
     tol = TOL[prec] * (10 if (algo == SA and prec == DP) else 1)
     for diff in (np.abs(got.astype(np.float64) - ref), np.abs(gg.astype(np.float64) - g)):
-        if algo == SA and prec == SP:      # ill-conditioned heatbath direction at weak local field (see test_gpu_batch)
-            assert np.quantile(diff, 0.99) <= tol and diff.max() <= 40 * tol
-        else:
-            assert diff.max() <= tol, diff.max()
+        assert diff.max() <= tol, diff.max()
 
 
 @pytest.mark.parametrize("prec", [DP, SP])
@@ -238,10 +235,7 @@ def test_wilson_heatbath_and_plaquette(gf, oracle, prec, beta):
             oracle.wilson_heatbath(ref, beta, 41 + c, 2)
             oracle.wilson_heatbath(ref, beta, 41 + c, 3)
             diff = np.abs(fx.get_links_copy(c, dtype=dt).astype(np.float64) - ref)
-            if prec == DP:
-                assert diff.max() <= 1e-10, diff.max()
-            else:
-                assert np.quantile(diff, 0.99) <= 5e-5 and diff.max() <= 5e-3
+            assert diff.max() <= (1e-10 if prec == DP else 5e-5), diff.max()
             assert abs(P[c] - oracle.plaquette(ref)) <= (1e-10 if prec == DP else 1e-4)
 
 
