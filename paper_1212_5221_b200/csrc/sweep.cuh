@@ -144,9 +144,11 @@ GF_DEV void global_get(const char* plane0, int64_t Vh, int64_t cb, Mat<R>& m) {
 }
 
 // ---- Step 1 for one subgroup (I,J), index S in the Cabibbo-Marinari order (0,1),(0,2),(1,2) ----
+// d: what hb_draws (below) prepared for this subgroup while the gather was in flight (heatbath only).  The heatbath
+// runs in the Step-1 type A: float on SP contexts, double on MP and DP contexts (step1.cuh).
 template <bool STOCH, class A>
 GF_DEV void choose_rule(const A a[4], A g[4], bool mag, A Dm, A Em, A Fm, const SweepArgs& args, uint64_t seed,
-                        uint32_t site, int sub) {
+                        uint32_t site, int sub, const HbDraw<A>& d) {
     if (!STOCH) {
         if (args.algo == ALGO_MICRO) rule_micro<A>(a, g);
         else rule_or<A>(a, (A)args.param, g);
@@ -156,35 +158,37 @@ GF_DEV void choose_rule(const A a[4], A g[4], bool mag, A Dm, A Em, A Fm, const 
             const double u = uniform01(rng_draw(seed, site, args.sweep_index, sub, 0, 0).x);
             if (u < args.param) rule_micro<A>(a, g);
             else rule_or<A>(a, A(1), g);
+        } else if (mag) {
+            hb_finish_mag<A>(Dm, Em, Fm, (A)args.param, d, g);
         } else {
-            double gd[4];
-            if (mag) {
-                rule_heatbath_mag((double)Dm, (double)Em, (double)Fm, args.param, seed, site, args.sweep_index,
-                                  sub, gd);
-            } else {
-                const double ad[4] = {(double)a[0], (double)a[1], (double)a[2], (double)a[3]};
-                rule_heatbath_landau(ad, args.param, seed, site, args.sweep_index, sub, gd);
-            }
-            g[0] = (A)gd[0]; g[1] = (A)gd[1]; g[2] = (A)gd[2]; g[3] = (A)gd[3];
+            hb_finish_landau<A>(a, (A)args.param, d, seed, site, args.sweep_index, sub, g);
         }
     }
 }
 
+// the link-independent part of the heatbath for subgroup `sub` (step1.cuh): Philox draws and what follows from them
+// alone.  The half-sweep kernels call it between issuing their loads and waiting for them.
+template <class A>
+GF_DEV void hb_draws(bool mag, uint64_t seed, uint32_t site, uint32_t sweep, int sub, HbDraw<A>& d) {
+    if (mag) hb_draws_mag<A>(seed, site, sweep, sub, d);
+    else hb_draws_landau<A>(seed, site, sweep, sub, d);
+}
+
 template <int I, int J, int S, bool STOCH, class A>
-GF_DEV void subgroup_landau(Mat<A>& K, Mat<A>& G, const SweepArgs& args, uint64_t seed, uint32_t site) {
+GF_DEV void subgroup_landau(Mat<A>& K, Mat<A>& G, const SweepArgs& args, uint64_t seed, uint32_t site, const HbDraw<A>& d) {
     // Fig. A.10 on K, signs per Eq. (15)
     A a[4], g[4];
     a[0] = K.v[RE(I, I)] + K.v[RE(J, J)];
     a[3] = K.v[IM(I, I)] - K.v[IM(J, J)];
     a[2] = K.v[RE(I, J)] - K.v[RE(J, I)];
     a[1] = K.v[IM(I, J)] + K.v[IM(J, I)];
-    choose_rule<STOCH, A>(a, g, false, A(0), A(0), A(0), args, seed, site, S);
+    choose_rule<STOCH, A>(a, g, false, A(0), A(0), A(0), args, seed, site, S, d);
     sub_left<I, J>(K, g);   // applying g at x maps K(x) -> g K(x)
     sub_left<I, J>(G, g);
 }
 
 template <int I, int J, int S, bool STOCH, class A>
-GF_DEV void subgroup_mag(Herm<A> (&M)[3], Mat<A>& G, const SweepArgs& args, uint64_t seed, uint32_t site) {
+GF_DEV void subgroup_mag(Herm<A> (&M)[3], Mat<A>& G, const SweepArgs& args, uint64_t seed, uint32_t site, const HbDraw<A>& d) {
     // f(g) = const + g^T [[D,E,F],[E,-D,0],[F,0,-D]] g  (Eqs. (25)-(28), SU(3) form)
     // (I,J) with I < J: off-diagonal element (I,J) of a Herm is o[2*OFF], o[2*OFF+1]
     constexpr int OFF = (I == 0) ? (J - 1) : 2;
@@ -195,7 +199,7 @@ GF_DEV void subgroup_mag(Herm<A> (&M)[3], Mat<A>& G, const SweepArgs& args, uint
     const A Fm = M[I].o[2 * OFF] - M[J].o[2 * OFF];
     const A lam = sqrt_t(Dm * Dm + Em * Em + Fm * Fm);   // Eq. (29)
     A a[4] = {Dm + lam, -Em, -Fm, A(0)}, g[4];
-    choose_rule<STOCH, A>(a, g, true, Dm, Em, Fm, args, seed, site, S);
+    choose_rule<STOCH, A>(a, g, true, Dm, Em, Fm, args, seed, site, S, d);
 #pragma unroll
     for (int k = 0; k < 3; ++k) {   // M_k -> g M_k g^dagger
         Mat<A> F;
@@ -341,6 +345,13 @@ sweep_kernel(const SweepArgs args) {
     }
     Mat<R> Gt;
     if (TRACK) global_get<R, 18>(gtot + Layout<R, 18>::site_offset(par, Vh), Vh, cb, Gt);
+    // stochastic rules: draws, logarithms and trigonometric functions of the three subgroups while the gather is in
+    // flight (a rolled loop and a local array: one copy of the code, nothing held in registers over pass 1)
+    HbDraw<A> pre[STOCH ? 3 : 1];
+    if (STOCH && args.algo == ALGO_SA) {
+#pragma unroll 1
+        for (int s = 0; s < 3; ++s) hb_draws<A>(GAUGE == GAUGE_MAG, seed, site, args.sweep_index, s, pre[s]);
+    }
     cp_async_wait_all();
 
     // ---- a3: neighbourhood summary, pass 1 over the links ----
@@ -372,13 +383,13 @@ sweep_kernel(const SweepArgs args) {
 
     // ---- a4/a5: Step 1 through the three SU(2) subgroups, G = g3 g2 g1 ----
     if (GAUGE == GAUGE_MAG) {
-        subgroup_mag<0, 1, 0, STOCH, A>(M, G, args, seed, site);
-        subgroup_mag<0, 2, 1, STOCH, A>(M, G, args, seed, site);
-        subgroup_mag<1, 2, 2, STOCH, A>(M, G, args, seed, site);
+        subgroup_mag<0, 1, 0, STOCH, A>(M, G, args, seed, site, pre[0]);
+        subgroup_mag<0, 2, 1, STOCH, A>(M, G, args, seed, site, pre[STOCH ? 1 : 0]);
+        subgroup_mag<1, 2, 2, STOCH, A>(M, G, args, seed, site, pre[STOCH ? 2 : 0]);
     } else {
-        subgroup_landau<0, 1, 0, STOCH, A>(K, G, args, seed, site);
-        subgroup_landau<0, 2, 1, STOCH, A>(K, G, args, seed, site);
-        subgroup_landau<1, 2, 2, STOCH, A>(K, G, args, seed, site);
+        subgroup_landau<0, 1, 0, STOCH, A>(K, G, args, seed, site, pre[0]);
+        subgroup_landau<0, 2, 1, STOCH, A>(K, G, args, seed, site, pre[STOCH ? 1 : 0]);
+        subgroup_landau<1, 2, 2, STOCH, A>(K, G, args, seed, site, pre[STOCH ? 2 : 0]);
     }
 
     // the summary now is that of the updated site (K -> G K, M_k -> G M_k G^dag): its F and theta terms

@@ -68,6 +68,8 @@ __global__ void __launch_bounds__(128, sizeof(R) == 8 ? 3 : 4) sweep_su2_kernel(
     }
     Quat<R> gt;
     if (TRACK) global_get_q(gtot + L::site_offset(par, Vh), Vh, cb, gt);
+    HbDraw<A> pre;   // heatbath: the link-independent part, while the loads are in flight
+    if (STOCH && args.algo == ALGO_SA) hb_draws<A>(GAUGE == GAUGE_MAG, seed, site, args.sweep_index, 0, pre);
 
     // a3: neighbourhood summary
     A a[4] = {A(0), A(0), A(0), A(0)};
@@ -86,7 +88,7 @@ __global__ void __launch_bounds__(128, sizeof(R) == 8 ? 3 : 4) sweep_su2_kernel(
 
     // a4/a5: Step 1
     A g[4];
-    choose_rule<STOCH, A>(a, g, GAUGE == GAUGE_MAG, Dm, Em, Fm, args, seed, site, 0);
+    choose_rule<STOCH, A>(a, g, GAUGE == GAUGE_MAG, Dm, Em, Fm, args, seed, site, 0, pre);
     Quat<R> gr;
 #pragma unroll
     for (int k = 0; k < 4; ++k) gr.v[k] = (R)g[k];

@@ -70,8 +70,11 @@ __global__ void __launch_bounds__(128, GF_HB_MIN_CTAS) wilson_heatbath_kernel(ch
     const int Nzh = d.Nz >> 1;
     const int Vsh = d.Nx * d.Ny * Nzh;
     const int64_t Vh = (int64_t)d.Nt * Vsh;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= Vsh) return;
+    // threads past the end of the slice redo the last site without storing: the heatbath's retries are evaluated by
+    // whole warps (step1.cuh, hb_retry)
+    const int i_raw = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool active = i_raw < Vsh;
+    const int i = active ? i_raw : Vsh - 1;
     const int copy = blockIdx.y / d.Nt;
     const int t = blockIdx.y - copy * d.Nt;
     char* links = links_all + copy * copy_bytes;
@@ -120,7 +123,7 @@ __global__ void __launch_bounds__(128, GF_HB_MIN_CTAS) wilson_heatbath_kernel(ch
     wilson_subgroup<0, 1, 0>(W, U, T, seed, site, sw);
     wilson_subgroup<0, 2, 1>(W, U, T, seed, site, sw);
     wilson_subgroup<1, 2, 2>(W, U, T, seed, site, sw);
-    global_put<R, RECON>(links + L::link_offset(parity, mu, Vh), Vh, cb, U);
+    if (active) global_put<R, RECON>(links + L::link_offset(parity, mu, Vh), Vh, cb, U);
 }
 
 // sum over the 6 plaquettes at x of Re tr U_P: grid (ceil(Vsh/block), ncopies*Nt, 2) like measure_kernel;
@@ -176,8 +179,9 @@ __global__ void __launch_bounds__(128) wilson_heatbath2_kernel(char* links_all, 
     const int Nzh = d.Nz >> 1;
     const int Vsh = d.Nx * d.Ny * Nzh;
     const int64_t Vh = (int64_t)d.Nt * Vsh;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= Vsh) return;
+    const int i_raw = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool active = i_raw < Vsh;     // whole warps stay (hb_retry)
+    const int i = active ? i_raw : Vsh - 1;
     const int copy = blockIdx.y / d.Nt;
     const int t = blockIdx.y - copy * d.Nt;
     char* links = links_all + copy * copy_bytes;
@@ -221,7 +225,7 @@ __global__ void __launch_bounds__(128) wilson_heatbath2_kernel(char* links_all, 
     Quat<R> g;
 #pragma unroll
     for (int k = 0; k < 4; ++k) g.v[k] = (R)gd[k];
-    global_put_q(links + L::link_offset(parity, mu, Vh), Vh, cb, qmul(g, U));
+    if (active) global_put_q(links + L::link_offset(parity, mu, Vh), Vh, cb, qmul(g, U));
 }
 
 template <class R>
