@@ -120,10 +120,11 @@ GF_DEV void rule_micro(const A a[4], A g[4]) {
 
 template <class S>
 struct HbDraw {
-    // Landau/Coulomb: v[0] = L = ln r1 + cos^2(2 pi r2) ln r3 and v[1] = r4^2 of Kennedy-Pendleton trial 0,
-    //                 v[2..4] = uniform direction (sin th cos ph, sin th sin ph, cos th), v[5] = |ln r1| + |ln r3|
+    // Landau/Coulomb: v[0] = L = ln r1 + cos^2(2 pi r2) ln r3, v[1] = r4^2, v[5] = |ln r1| + |ln r3| of Kennedy-Pendleton
+    //                 trial 0 and v[6], v[7], v[8] the same of trial 1 (most lanes that reject trial 0 accept trial 1: the
+    //                 warp-wide retry becomes rare); v[2..4] = uniform direction (sin th cos ph, sin th sin ph, cos th)
     // MAG:            v[0] = r1, v[1] = sin(2 pi r2), v[2] = cos(2 pi r2), v[3] = 1 - r1
-    S v[6];
+    S v[9];
 };
 
 // (w + 0.5) 2^-32 in S; the float version rounds w to 24 bits (relative error 2^-24)
@@ -133,6 +134,21 @@ template <> GF_DEV float uniform_s<float>(uint32_t w) { return __fmaf_rn((float)
 
 GF_DEV float log_s(float x) { return logf(x); }
 GF_DEV double log_s(double x) { return log(x); }
+// ln of a uniform in (0, 1].  float: the SFU's lg2 (2 ulp outside [1/2, 2], 2^-22 absolute inside: CUDA C Programming
+// Guide, __log2f) times ln 2 - as good as logf for this purpose at a tenth of the instructions
+GF_DEV float log_u(float x) { return __log2f(x) * 0.693147180559945309f; }
+GF_DEV double log_u(double x) { return log(x); }
+// cos^2(2 pi r) = 1/2 - 1/2 cos(2 pi c), c = frac(2 r) - 1/2 in [-1/2, 1/2); float: SFU cosine on [-pi, pi)
+// (absolute error 2^-21.41 there, __cosf)
+GF_DEV float cos2_2pi(float r) {
+    float y = r + r;
+    y = (y >= 1.0f) ? y - 1.0f : y;
+    return __fmaf_rn(-0.5f, __cosf(6.283185307179586f * (y - 0.5f)), 0.5f);
+}
+GF_DEV double cos2_2pi(double r) { const double c = cospi(2.0 * r); return c * c; }
+// (sin, cos)(2 pi r): pi-scaled functions (exact argument reduction)
+GF_DEV void sincos_2pi(float r, float* s, float* c) { sincospif(2.0f * r, s, c); }
+GF_DEV void sincos_2pi(double r, double* s, double* c) { sincospi(2.0 * r, s, c); }
 GF_DEV float exp_s(float x) { return expf(x); }
 GF_DEV double exp_s(double x) { return exp(x); }
 GF_DEV float cospi_s(float x) { return cospif(x); }
@@ -151,20 +167,22 @@ GF_DEV S sqrt_pos(S x) { return x > S(0) ? x * rsqrt_s(x) : S(0); }
 
 template <class S>
 GF_DEV void hb_draws_landau(uint64_t seed, uint32_t site, uint32_t sweep, int sub, HbDraw<S>& d) {
-    const u32x4 r = rng_draw(seed, site, sweep, sub, 1, 0);
     const u32x4 rd = rng_draw(seed, site, sweep, sub, 2, 0);
-    const S r1 = uniform_s<S>(r.x), r2 = uniform_s<S>(r.y), r3 = uniform_s<S>(r.z), r4 = uniform_s<S>(r.w);
-    const S cs = cospi_s(S(2) * r2);   // pi-scaled: exact argument reduction
-    const S l1 = log_s(r1), l3 = log_s(r3);
-    d.v[0] = l1 + cs * cs * l3;
-    d.v[1] = r4 * r4;
-    d.v[5] = -(l1 + l3);
+#pragma unroll
+    for (int t = 0; t < 2; ++t) {
+        const u32x4 r = rng_draw(seed, site, sweep, sub, 1, (uint32_t)t);
+        const S r1 = uniform_s<S>(r.x), r2 = uniform_s<S>(r.y), r3 = uniform_s<S>(r.z), r4 = uniform_s<S>(r.w);
+        const S l1 = log_u(r1), l3 = log_u(r3);
+        d.v[t ? 6 : 0] = l1 + cos2_2pi(r2) * l3;
+        d.v[t ? 7 : 1] = r4 * r4;
+        d.v[t ? 8 : 5] = -(l1 + l3);
+    }
     // cos th = 2 r5 - 1 = r5 - (1 - r5) and sin^2 th = 4 r5 (1 - r5), with 1 - r5 converted from the complemented
     // Philox word: no cancellation near the poles (in float 1 - cos^2 th would lose sin th there)
     const S r5 = uniform_s<S>(rd.x), r5c = uniform_s<S>(~rd.x);
     const S ct = r5 - r5c;
     S sphi, cphi;
-    sincospi_s(S(2) * uniform_s<S>(rd.y), &sphi, &cphi);
+    sincos_2pi(uniform_s<S>(rd.y), &sphi, &cphi);
     const S st = S(2) * sqrt_pos(r5 * r5c);
     d.v[2] = st * cphi;
     d.v[3] = st * sphi;
@@ -174,15 +192,15 @@ template <class S>
 GF_DEV void hb_draws_mag(uint64_t seed, uint32_t site, uint32_t sweep, int sub, HbDraw<S>& d) {
     const u32x4 r = rng_draw(seed, site, sweep, sub, 1, 0);
     d.v[0] = uniform_s<S>(r.x);
-    sincospi_s(S(2) * uniform_s<S>(r.y), &d.v[1], &d.v[2]);
+    sincos_2pi(uniform_s<S>(r.y), &d.v[1], &d.v[2]);
     d.v[3] = uniform_s<S>(~r.x);   // 1 - r1 = ((2^32 - 1 - w) + 0.5) 2^-32, to full relative precision
 }
 
 // Guard bands of the float decisions (first-order bounds of the rounding error of the decision variable, with a
-// factor >= 8 to spare).  Kennedy-Pendleton: v = 1 - delta/2 - r4^2, delta = -L/alpha; logf and cospif are good to
-// 1-2 ulp, the uniforms to 2^-24 relative: |error of L| <= 1.5e-6 (|ln r1| + |ln r3|) + 1.2e-7, so
-// |error of v| <= 1e-6 (|ln r1| + |ln r3|)/alpha + 5e-7.  Creutz: v = w (2 - w) - r2^2 with w in [0, 2] good to
-// 5e-7 relative: |error of v| <= 2.5e-6.
+// factor >= 8 to spare).  Kennedy-Pendleton: v = 1 - delta/2 - r4^2, delta = -L/alpha; the logarithms are good to
+// 3.6e-7 relative or 1.7e-7 absolute, cos^2 to 6e-7 (SFU 1.8e-7, argument 4 pi 2^-25), the uniforms to 2^-24
+// relative: |error of L| <= 1e-6 (|ln r1| + |ln r3|) + 4e-7, so |error of v| <= 0.5e-6 (|ln r1| + |ln r3|)/alpha
+// + 6e-7.  Creutz: v = w (2 - w) - r2^2 with w in [0, 2] good to 5e-7 relative: |error of v| <= 2.5e-6.
 #define GF_HB_BAND_KP 1e-5f
 #define GF_HB_BAND_CREUTZ 3e-5f
 
@@ -206,9 +224,8 @@ GF_DEV bool hb_trial(bool kp, float inv_alpha, float aux, const u32x4& r, float&
     float v, band;
     if (kp) {
         const float r1 = uniform_s<float>(r.x), r3 = uniform_s<float>(r.z), r4 = uniform_s<float>(r.w);
-        const float cs = cospif(2.0f * r2);
-        const float l1 = logf(r1), l3 = logf(r3);
-        w = -(l1 + cs * cs * l3) * inv_alpha;
+        const float l1 = log_u(r1), l3 = log_u(r3);
+        w = -(l1 + cos2_2pi(r2) * l3) * inv_alpha;
         v = 1.0f - 0.5f * w - r4 * r4;
         band = GF_HB_BAND_KP * (1.0f - (l1 + l3) * inv_alpha);
     } else {
@@ -298,17 +315,25 @@ GF_DEV void hb_finish_landau(const S a[4], S T, const HbDraw<S>& d, uint64_t see
     const S inv_alpha = T * inv_norm;
     const S h0 = a[0] * inv_norm, h1 = -a[1] * inv_norm, h2 = -a[2] * inv_norm, h3 = -a[3] * inv_norm;
     const bool kp = alpha >= S(2);
-    S w = -d.v[0] * inv_alpha;   // trial 0 of Kennedy-Pendleton from the precomputed draws (w = delta = 1 - u0)
-    const S v = S(1) - S(0.5) * w - d.v[1];
-    bool accept0 = kp && v >= S(0);
-    if (sizeof(S) == 4) accept0 = kp && v > (S)GF_HB_BAND_KP * (S(1) + d.v[5] * inv_alpha);   // inside the band: redone by hb_retry
-    const bool pending = !zero && !accept0;
+    // trials 0 and 1 of Kennedy-Pendleton from the precomputed draws (w = delta = 1 - u0, accepted iff
+    // v = 1 - delta/2 - r4^2 >= 0); in float a trial inside the guard band is left open and redone by hb_retry
+    const S w0 = -d.v[0] * inv_alpha, w1 = -d.v[6] * inv_alpha;
+    const S v0 = S(1) - S(0.5) * w0 - d.v[1], v1 = S(1) - S(0.5) * w1 - d.v[7];
+    bool acc0, rej0, acc1, rej1;
+    if (sizeof(S) == 4) {
+        const S b0 = (S)GF_HB_BAND_KP * (S(1) + d.v[5] * inv_alpha), b1 = (S)GF_HB_BAND_KP * (S(1) + d.v[8] * inv_alpha);
+        acc0 = v0 > b0; rej0 = v0 < -b0; acc1 = v1 > b1; rej1 = v1 < -b1;
+    } else {
+        acc0 = v0 >= S(0); rej0 = !acc0; acc1 = v1 >= S(0); rej1 = !acc1;
+    }
+    S w = acc0 ? w0 : w1;
+    const bool pending = !zero && !(kp && (acc0 || (rej0 && acc1)));
     if (__any_sync(GF_FULL_WARP, pending)) {
-        // trial 0 is still open for a Creutz lane and for a float lane inside the band (or rejected: the band is tiny)
-        const bool redo0 = !kp || (sizeof(S) == 4 && v >= -(S)GF_HB_BAND_KP * (S(1) + d.v[5] * inv_alpha));
+        // first trial that is still open: 0 for a Creutz lane
+        const uint32_t next = (!kp || !rej0) ? 0u : (!rej1 ? 1u : 2u);
         S aux = S(0);
         if (!kp) aux = (sizeof(S) == 4) ? (S)(-expm1f(-2.0f * (float)alpha)) : exp_s(S(-2) * alpha);
-        w = hb_retry<S>(pending, redo0 ? 0u : 1u, kp, inv_alpha, aux, seed, site, sweep, sub, w);
+        w = hb_retry<S>(pending, next, kp, inv_alpha, aux, seed, site, sweep, sub, w);
     }
     w = min_s(S(2), max_s(S(0), w));   // u0 in [-1, 1]
     const S u0 = S(1) - w;
