@@ -16,7 +16,8 @@
  *     the gauge group SU(3) or, with GF_FLAG_SU2, SU(2).
  *   - A context lives on the CUDA device that is current when it is created; the caller keeps that device
  *     current for every later call on the context.
- *   - One context per stream, not thread-safe.  Kernels are enqueued on the cudaStream_t given to
+ *   - One context per stream.  A context is not thread-safe, but different contexts may be driven from different
+ *     host threads at the same time (the library keeps no unguarded global state).  Kernels are enqueued on the cudaStream_t given to
  *     gf_create (NULL = the legacy default stream).  gf_set_links, gf_get_*, gf_measure*, gf_run*, gf_fix,
  *     gf_random_gauge, gf_plaquette and gf_unitarity synchronise that stream before returning; gf_sweep,
  *     gf_half_sweep, gf_anneal, gf_wilson_heatbath, gf_reunitarize and gf_coulomb_finalize only enqueue.
@@ -240,6 +241,62 @@ typedef struct {
 int gf_fix(gf_ctx* ctx, const gf_fix_params* params, gf_result* out);
 
 /*
+ * t-shards: one lattice split along t over several link stores (Sec. 5).
+ *
+ * The paper splits N_t over the devices; the only links a half-sweep touches outside its own part
+ * are the inactive-parity U_0 of the boundary slice, 1/12 of a slice.  gf_create_shard makes a
+ * context that holds the slices [t0, t0 + Nt_local) of an Nx*Ny*Nz*Nt_global lattice (t0 and both extents even; SU(3),
+ * one gauge copy).  Its half-sweep kernel reads and writes the down-t links of its first slice IN PLACE in the store
+ * of the shard below — a pointer on the same device, a peer mapping (gf_shard_attach: contexts of this process, peer
+ * access is enabled when they live on another device) or a CUDA IPC mapping (gf_shard_export / gf_shard_attach_ipc:
+ * other processes) — so there are no halo buffers and no exchange step (the seven steps of PAPER.md:454-463 collapse
+ * into the kernel's own loads and stores over NVLink).  Every link is still touched by exactly one thread per
+ * half-sweep.  The Philox counter uses the site index in the WHOLE lattice and the reductions are summed per global
+ * time-slice in slice order on every shard, so links, F, theta, histories, stopping decisions and random draws are
+ * those of the unsharded context, bit for bit.
+ *
+ * What is left between shards is ordering and 2*Nt_global numbers per check (gf_comm, supplied by the caller — the
+ * library links no communication library):
+ *   barrier(user)              stream-ordered barrier over all shards: whatever was enqueued before it on any shard's
+ *                              stream completes before anything enqueued after it on any shard's stream starts.  Called
+ *                              after every Landau/MAG half-sweep and reprojection, before a reduction, around the
+ *                              Coulomb finalisation and after gf_set_links; Coulomb sweeps need none.
+ *                              One stream shared by all shards of a device: a no-op.  One process per GPU: an
+ *                              all-reduce of one element enqueued on the context's stream (NCCL).
+ *   allreduce_sum(user, b, n)  in-place sum over all shards of the host array b[n] (every shard has filled its own
+ *                              slices and zeroed the rest, so the sum is exact); blocking.
+ * Every shard must make the same sequence of calls with the same arguments (they take identical decisions).
+ * On a shard: gf_set_links / gf_get_links / gf_get_gauge_transform move the shard's own slab
+ * [t0, t0 + Nt_local) (contiguous in StandardPattern: t is the slowest index); gf_measure returns the global F and
+ * theta, theta_slice has Nt_global entries; gf_run / gf_anneal / gf_fix / gf_sweep / gf_half_sweep / gf_reunitarize /
+ * gf_coulomb_finalize (which reads g(x + t_hat) of its last slice from the shard above) work as on a
+ * whole lattice; gf_get_slice_sweeps has Nt_global entries; gf_unitarity covers the shard's own links;
+ * gf_random_gauge, gf_wilson_heatbath and gf_plaquette return GF_ESTATE.  Sweeps and reductions return GF_ESTATE
+ * until the neighbours are attached.  A single shard spanning the lattice attaches to itself.
+ * Multi-device operation (peer / IPC mappings) is written and guarded but was not run on hardware in this build
+ * (one GPU available); the tests drive 2 and 4 shards on one device and compare with the unsharded context bit for bit.
+ */
+int gf_create_shard(gf_ctx** out, int Nx, int Ny, int Nz, int Nt_local, int t0, int Nt_global, int precision, int recon,
+                    unsigned flags, void* cuda_stream);
+/* below holds slice t0 - 1 as its last slice, above holds slice t0 + Nt_local as its first one (periodic in Nt_global) */
+int gf_shard_attach(gf_ctx* ctx, gf_ctx* below, gf_ctx* above);
+typedef struct {
+    unsigned char links[64], gtot[64], gapplied[64]; /* cudaIpcMemHandle_t of the stores */
+    int t0, Nt_local, has_transform;
+} gf_shard_handle;
+int gf_shard_export(gf_ctx* ctx, gf_shard_handle* handle);
+int gf_shard_attach_ipc(gf_ctx* ctx, const gf_shard_handle* below, const gf_shard_handle* above);
+typedef struct {
+    void (*barrier)(void* user);
+    void (*allreduce_sum)(void* user, double* buf, int n);
+    void* user;
+} gf_comm;
+/* comm == NULL: no communicator (all shards on one stream of one process need none for ordering, but still need
+ * allreduce_sum for reductions unless there is a single shard) */
+int gf_shard_set_comm(gf_ctx* ctx, const gf_comm* comm);
+int gf_shard_info(const gf_ctx* ctx, int* t0, int* Nt_local, int* Nt_global);
+
+/*
  * gf_random_gauge — a random start on the gauge orbit ("100 randomly chosen points on the
  * gauge orbit", 580): every copy c is gauge transformed, U_mu(x) <- h(x) U_mu(x) h(x+mu)^dagger (Eq. (1),
  * PAPER.md:25), with h(x) Haar distributed on SU(3): two rows of complex standard normals — Box-Muller on
@@ -315,6 +372,22 @@ int64_t gf_volume(const gf_ctx* ctx);
 
 const char* gf_last_error(const gf_ctx* ctx);
 const char* gf_version(void);
+
+/*
+ * Tuning hooks — NOT part of the contract (bench.py's side studies and two tests use them; results never depend on them
+ * beyond what is said here).
+ *   gf_debug_set_fused(ctx, 0)  gf_run measures with the stand-alone reduction kernels at every check instead of the
+ *                               partial sums fused into the half-sweeps; same decisions, same results.
+ *   gf_debug_set_pdl(ctx, 0)    half-sweeps are launched without programmatic dependent launch.
+ *   gf_debug_set_block(ctx, n)  CTA size of the half-sweep kernel: a multiple of 32 up to the default (0 = default);
+ *                               links are bit-identical for every n, fused partial sums differ in summation order.
+ *   gf_debug_set_persistent(ctx, 0)  gf_run / gf_anneal never use the persistent whole-run kernel for small lattices
+ *                               (DESIGN.md §6.9); same results bit for bit.
+ */
+int gf_debug_set_fused(gf_ctx* ctx, int fused);
+int gf_debug_set_pdl(gf_ctx* ctx, int pdl);
+int gf_debug_set_block(gf_ctx* ctx, int block);
+int gf_debug_set_persistent(gf_ctx* ctx, int persistent);
 
 #ifdef __cplusplus
 }

@@ -160,8 +160,16 @@ GF_DEV void block_sum2(double& a, double& b) {
     }
 }
 
+// t-shards: sh.links_dn is the store that holds the slice below this store's first one (its last
+// slice, Nt_dn - 1); not sharded: the store itself (periodic wrap).
+struct ShardDn {
+    const char* links_dn;
+    int64_t Vh_dn, copy_bytes_dn;
+    int Nt_dn;
+};
+
 template <class R, int RECON, int GAUGE>
-__global__ void measure_kernel(const char* links, Dims d, double* partial, int64_t copy_bytes) {
+__global__ void measure_kernel(const char* links, Dims d, double* partial, int64_t copy_bytes, ShardDn sh) {
     typedef Layout<R, RECON> L;
     constexpr int MU0 = (GAUGE == GAUGE_COULOMB) ? 1 : 0;
     const int Nzh = d.Nz >> 1;
@@ -202,7 +210,11 @@ __global__ void measure_kernel(const char* links, Dims d, double* partial, int64
                 f_term += (double)U.v[RE(0, 0)] + (double)U.v[RE(1, 1)] + (double)U.v[RE(2, 2)];
                 acc_plain(K, U);
             }
-            global_get<R, RECON>(links + L::link_offset(1 - par, mu, Vh), Vh, cbn[mu], U);
+            if (mu == 0 && t == 0)   // x - t_hat of the first slice: last slice of the store below
+                global_get<R, RECON>(sh.links_dn + copy * sh.copy_bytes_dn + L::link_offset(1 - par, 0, sh.Vh_dn), sh.Vh_dn,
+                                     (int64_t)(sh.Nt_dn - 1) * Vsh + i, U);
+            else
+                global_get<R, RECON>(links + L::link_offset(1 - par, mu, Vh), Vh, cbn[mu], U);
             if (GAUGE == GAUGE_MAG) { mag_acc_down<0>(M[0], U); mag_acc_down<1>(M[1], U); mag_acc_down<2>(M[2], U); }
             else acc_dagger(K, U);
         }
@@ -267,9 +279,17 @@ __global__ void red_reduce_kernel(const double* partial, int gx, double* out) {
 }
 
 // ---- Coulomb finalisation: U_0(x) <- R(x) U_0(x) R(x+t)^dag, R = g_tot g_applied^dag -----------
+// t-shards: g(x + t_hat) of the last slice is the first slice of the transform store above (gtot_up / gapp_up with
+// Vh_up sites per parity); not sharded: the store itself (periodic wrap).
+struct ShardUp {
+    const char* gtot_up;
+    const char* gapp_up;
+    int64_t Vh_up, copy_bytes_up;
+};
+
 template <class R, int RECON>
 __global__ void coulomb_finalize_kernel(char* links, const char* gtot, const char* gapp, Dims d,
-                                        int64_t copy_links_bytes, int64_t copy_field_bytes) {
+                                        int64_t copy_links_bytes, int64_t copy_field_bytes, ShardUp sh) {
     links += blockIdx.y * copy_links_bytes;   // blockIdx.y = gauge copy
     gtot += blockIdx.y * copy_field_bytes;
     if (gapp) gapp += blockIdx.y * copy_field_bytes;
@@ -281,15 +301,19 @@ __global__ void coulomb_finalize_kernel(char* links, const char* gtot, const cha
     const int par = (int)(i / Vh);
     const int cb = (int)(i % Vh);
     const int t = cb / Vsh;
-    const int cbf = cb + ((t == d.Nt - 1) ? -(d.Nt - 1) * Vsh : Vsh);   // x + t_hat, other parity
+    const bool top = t == d.Nt - 1;
+    const int64_t cbf = top ? cb - (int64_t)(d.Nt - 1) * Vsh : cb + Vsh;   // x + t_hat, other parity (top: slice 0 above)
+    const char* gt_f = top ? sh.gtot_up + blockIdx.y * sh.copy_bytes_up : gtot;
+    const char* ga_f = top ? (sh.gapp_up ? sh.gapp_up + blockIdx.y * sh.copy_bytes_up : nullptr) : gapp;
+    const int64_t Vh_f = top ? sh.Vh_up : Vh;
     Mat<R> U, Ga, Gb, T, O;
     global_get<R, 18>(gtot + Layout<R, 18>::site_offset(par, Vh), Vh, cb, Ga);
-    global_get<R, 18>(gtot + Layout<R, 18>::site_offset(1 - par, Vh), Vh, cbf, Gb);
+    global_get<R, 18>(gt_f + Layout<R, 18>::site_offset(1 - par, Vh_f), Vh_f, cbf, Gb);
     if (gapp) {
         Mat<R> P;
         global_get<R, 18>(gapp + Layout<R, 18>::site_offset(par, Vh), Vh, cb, P);
         mul_right_dagger<3>(Ga, P, T); Ga = T;
-        global_get<R, 18>(gapp + Layout<R, 18>::site_offset(1 - par, Vh), Vh, cbf, P);
+        global_get<R, 18>(ga_f + Layout<R, 18>::site_offset(1 - par, Vh_f), Vh_f, cbf, P);
         mul_right_dagger<3>(Gb, P, T); Gb = T;
     }
     char* p0 = links + Layout<R, RECON>::link_offset(par, 0, Vh);

@@ -72,11 +72,28 @@ struct gf_ctx {
     int64_t device_bytes;
     int block_override;     // 0 = default CTA size
     int pdl;                // half-sweeps launched with programmatic stream serialization (default 1)
+    int persistent;         // small lattices: whole runs in one cooperative launch where possible (default 1)
     // kernel timing (gf_kernel_timing)
     bool timing;
     std::vector<cudaEvent_t> ev;   // pairs (start, stop)
     size_t ev_used;
     int64_t launches;       // kernels enqueued by this context (gf_launch_count)
+    // t-sharding (gf_create_shard): this store holds the slices [t0, t0 + Nt) of a lattice of NtG
+    // slices.  Host-side reduction arrays and the run loop's bookkeeping are indexed by GLOBAL slice (NSG = B * NtG
+    // entries; a shard fills its own part, the comm's allreduce completes it); not sharded: NtG = Nt, t0 = 0.
+    bool sharded;
+    int NtG, t0, NSG;
+    int64_t VG;
+    char* links_dn;         // store holding slice t0 - 1 as its last slice (not sharded: links)
+    int64_t Vh_dn;
+    int Nt_dn;
+    char* gtot_up;          // transform stores holding slice t0 + Nt as their first slice (not sharded: gtot / gapplied)
+    char* gapp_up;
+    int64_t Vh_up;
+    bool attached;
+    bool have_comm;
+    gf_comm comm;
+    std::vector<void*> ipc_opened;   // mappings opened by gf_shard_attach_ipc
     char err[512];
 };
 
@@ -136,15 +153,33 @@ int gf_create(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int precision, int r
     return gf_create_batch(out, Nx, Ny, Nz, Nt, 1, precision, recon, flags, cuda_stream);
 }
 
+static int create_impl(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int n_copies, int precision, int recon,
+                       unsigned flags, void* cuda_stream, int t0, int NtG);
+
 int gf_create_batch(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int n_copies, int precision, int recon,
                     unsigned flags, void* cuda_stream) {
+    return create_impl(out, Nx, Ny, Nz, Nt, n_copies, precision, recon, flags, cuda_stream, 0, Nt);
+}
+
+int gf_create_shard(gf_ctx** out, int Nx, int Ny, int Nz, int Nt_local, int t0, int Nt_global, int precision, int recon,
+                    unsigned flags, void* cuda_stream) {
+    if (!out) return GF_EINVAL;
+    *out = nullptr;
+    // even first slice and even extents: the 4-d colouring of the store is the global one
+    if (t0 < 0 || (t0 & 1) || Nt_global < 2 || (Nt_global & 1) || Nt_local < 2 || t0 + Nt_local > Nt_global) return GF_EINVAL;
+    if (flags & GF_FLAG_SU2) return GF_EINVAL;   // SU(3) only
+    return create_impl(out, Nx, Ny, Nz, Nt_local, 1, precision, recon, flags, cuda_stream, t0, Nt_global);
+}
+
+static int create_impl(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int n_copies, int precision, int recon,
+                       unsigned flags, void* cuda_stream, int t0, int NtG) {
     if (!out) return GF_EINVAL;
     *out = nullptr;
     if (n_copies < 1 || (int64_t)n_copies * Nt > 65535) return GF_EINVAL;   // grid.y = n_copies * Nt
     const int n[4] = {Nx, Ny, Nz, Nt};
     for (int k = 0; k < 4; ++k)
         if (n[k] < 2 || (n[k] & 1)) return GF_EINVAL;
-    const double vol = (double)Nx * Ny * Nz * Nt;
+    const double vol = (double)Nx * Ny * Nz * NtG;
     if (vol >= 4294967296.0) return GF_EINVAL;
     if (precision != GF_SP && precision != GF_DP && precision != GF_MP) return GF_EINVAL;
     if (recon != 18 && recon != 12) return GF_EINVAL;
@@ -171,11 +206,19 @@ int gf_create_batch(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int n_copies, 
     ctx->fused = 1;
     ctx->skip_dev = nullptr; ctx->skip_host = nullptr; ctx->have_slice_sweeps = false;
     ctx->staging = nullptr; ctx->staging_bytes = 0;
-    ctx->device_bytes = 0; ctx->block_override = 0; ctx->pdl = 1;
+    ctx->device_bytes = 0; ctx->block_override = 0; ctx->pdl = 1; ctx->persistent = 1;
     ctx->timing = false; ctx->ev_used = 0; ctx->launches = 0;
     ctx->err[0] = 0;
+    ctx->sharded = (NtG != Nt);
+    ctx->NtG = NtG; ctx->t0 = t0; ctx->NSG = n_copies * NtG;
+    ctx->VG = (int64_t)Nx * Ny * Nz * NtG;
+    ctx->links_dn = nullptr; ctx->Vh_dn = ctx->Vh; ctx->Nt_dn = Nt;
+    ctx->gtot_up = ctx->gapp_up = nullptr; ctx->Vh_up = ctx->Vh;
+    ctx->attached = !ctx->sharded;
+    ctx->have_comm = false;
+    memset(&ctx->comm, 0, sizeof(ctx->comm));
 
-    const int B = n_copies, NS = n_copies * Nt;
+    const int B = n_copies, NS = n_copies * Nt, NSG = ctx->NSG;
     cudaError_t e = cudaMalloc((void**)&ctx->links, (size_t)(B * link_store_bytes(ctx)));
     if (e == cudaSuccess) ctx->device_bytes += B * link_store_bytes(ctx);
     if (e == cudaSuccess && (flags & GF_FLAG_TRACK_TRANSFORM)) {
@@ -188,12 +231,16 @@ int gf_create_batch(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int n_copies, 
     const size_t npart = (size_t)ctx->meas_gx * NS * 2;
     if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->partial, npart * 2 * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->slice_dev, (size_t)2 * NS * sizeof(double));
-    if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->slice_host, (size_t)2 * NS * sizeof(double));
+    if (e == cudaSuccess && ctx->sharded && ctx->gtot) {   // a shard's neighbours map it: allocated once, never moved
+        e = cudaMalloc((void**)&ctx->gapplied, (size_t)(B * field_store_bytes(ctx)));
+        if (e == cudaSuccess) ctx->device_bytes += B * field_store_bytes(ctx);
+    }
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->slice_host, (size_t)2 * NSG * sizeof(double));
     const size_t nred = (size_t)((Vsh + 31) / 32) * NS * 3;   // smallest CTA = 32 sites
     for (int k = 0; k < 2; ++k)
         if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->red_part[k], nred * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->red_dev, (size_t)6 * NS * sizeof(double));
-    if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->red_host, (size_t)6 * NS * sizeof(double));
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->red_host, (size_t)6 * NSG * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->skip_dev, (size_t)NS);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->skip_host, (size_t)NS);
     if (e != cudaSuccess) {
@@ -203,6 +250,10 @@ int gf_create_batch(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int n_copies, 
         return code;
     }
     ctx->device_bytes += (int64_t)(npart * 2 + 2 * NS + 2 * nred + 6 * NS) * sizeof(double);
+    if (!ctx->sharded) {   // the periodic wrap in t: the store is its own neighbour
+        ctx->links_dn = ctx->links;
+        ctx->gtot_up = ctx->gtot;
+    }
     *out = ctx;
     return GF_OK;
 }
@@ -210,6 +261,7 @@ int gf_create_batch(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int n_copies, 
 int gf_destroy(gf_ctx* ctx) {
     if (!ctx) return GF_OK;
     cudaStreamSynchronize(ctx->stream);
+    for (void* p : ctx->ipc_opened) cudaIpcCloseMemHandle(p);
     cudaFree(ctx->links);
     cudaFree(ctx->gtot);
     cudaFree(ctx->gapplied);
@@ -305,7 +357,7 @@ static int reset_transform(gf_ctx* ctx, int copy) {
     ctx->gtot_ident[(size_t)copy] = 1;
     // gapplied is a snapshot taken at the next start of Coulomb sweeps (coulomb_begin); nothing to reset here.
     // A single lattice gives the memory back (a transform field is 1/4 of an 18-real link store).
-    if (ctx->gapplied && ctx->B == 1) {
+    if (ctx->gapplied && ctx->B == 1 && !ctx->sharded) {
         CU(cudaStreamSynchronize(ctx->stream));
         cudaFree(ctx->gapplied);
         ctx->gapplied = nullptr;
@@ -326,6 +378,132 @@ static int single_only(gf_ctx* ctx, const char* who) {
 }
 
 int gf_num_copies(const gf_ctx* ctx) { return ctx ? ctx->B : 0; }
+
+// ---- t-shards: neighbours and the caller's communicator ---------------------------
+// stream-ordered barrier over all shards: everything enqueued so far on every shard's stream completes before
+// anything enqueued afterwards on any of them starts (the caller's callback; nothing to do for one store)
+static void shard_barrier(gf_ctx* ctx) {
+    if (ctx->have_comm && ctx->comm.barrier) ctx->comm.barrier(ctx->comm.user);
+}
+// complete a host array indexed by global slice: every shard has filled its own entries and zeroed the others
+static void shard_allreduce(gf_ctx* ctx, double* buf, int n) {
+    if (ctx->have_comm && ctx->comm.allreduce_sum) ctx->comm.allreduce_sum(ctx->comm.user, buf, n);
+}
+static int need_attached(gf_ctx* ctx, const char* who) {
+    if (!ctx->attached) return fail(ctx, GF_ESTATE, "%s: shard has no neighbours yet (gf_shard_attach)", who);
+    return GF_OK;
+}
+static int not_on_shards(gf_ctx* ctx, const char* who) {
+    if (ctx->sharded) return fail(ctx, GF_ESTATE, "%s: not available on a t-shard", who);
+    return GF_OK;
+}
+static ShardDn shard_dn(const gf_ctx* ctx) {
+    ShardDn sh;
+    sh.links_dn = ctx->links_dn; sh.Vh_dn = ctx->Vh_dn; sh.Nt_dn = ctx->Nt_dn;
+    sh.copy_bytes_dn = ctx->sharded ? 0 : (int64_t)8 * ctx->recon * ctx->real_bytes * ctx->Vh;
+    return sh;
+}
+
+int gf_shard_set_comm(gf_ctx* ctx, const gf_comm* comm) {
+    if (!ctx) return GF_EINVAL;
+    ctx->have_comm = comm != nullptr;
+    if (comm) ctx->comm = *comm;
+    return GF_OK;
+}
+
+int gf_shard_info(const gf_ctx* ctx, int* t0, int* Nt_local, int* Nt_global) {
+    if (!ctx) return GF_EINVAL;
+    if (t0) *t0 = ctx->t0;
+    if (Nt_local) *Nt_local = ctx->Nt;
+    if (Nt_global) *Nt_global = ctx->NtG;
+    return GF_OK;
+}
+
+// make a pointer of another device of this process usable from the current one
+static int enable_peer_for(gf_ctx* ctx, const void* ptr) {
+    cudaPointerAttributes at;
+    CU(cudaPointerGetAttributes(&at, ptr));
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    if (at.type == cudaMemoryTypeDevice && at.device != dev) {
+        int can = 0;
+        CU(cudaDeviceCanAccessPeer(&can, dev, at.device));
+        if (!can) return fail(ctx, GF_ECUDA, "gf_shard_attach: device %d cannot map device %d", dev, at.device);
+        cudaError_t e = cudaDeviceEnablePeerAccess(at.device, 0);
+        if (e == cudaErrorPeerAccessAlreadyEnabled) cudaGetLastError();
+        else CU(e);
+    }
+    return GF_OK;
+}
+
+static int check_neighbour(gf_ctx* ctx, const gf_ctx* nb, int want_t0, const char* what) {
+    if (!nb) return fail(ctx, GF_EINVAL, "gf_shard_attach: NULL %s", what);
+    if (nb->Nx != ctx->Nx || nb->Ny != ctx->Ny || nb->Nz != ctx->Nz || nb->NtG != ctx->NtG || nb->precision != ctx->precision ||
+        nb->recon != ctx->recon || nb->nc != ctx->nc || nb->B != ctx->B || (nb->gtot != nullptr) != (ctx->gtot != nullptr))
+        return fail(ctx, GF_EINVAL, "gf_shard_attach: the %s does not match this shard (extents, precision, recon, flags)", what);
+    if (nb->t0 != want_t0) return fail(ctx, GF_EINVAL, "gf_shard_attach: the %s starts at slice %d, expected %d", what, nb->t0, want_t0);
+    return GF_OK;
+}
+
+int gf_shard_attach(gf_ctx* ctx, gf_ctx* below, gf_ctx* above) {
+    if (!ctx) return GF_EINVAL;
+    // below holds slice t0 - 1 as its last one, above holds slice t0 + Nt as its first one (periodic in NtG)
+    int rc = check_neighbour(ctx, above, (ctx->t0 + ctx->Nt) % ctx->NtG, "shard above");
+    if (rc) return rc;
+    if (!below) return fail(ctx, GF_EINVAL, "gf_shard_attach: NULL shard below");
+    rc = check_neighbour(ctx, below, below->t0, "shard below");
+    if (rc) return rc;
+    if ((below->t0 + below->Nt) % ctx->NtG != ctx->t0)
+        return fail(ctx, GF_EINVAL, "gf_shard_attach: the shard below ends at slice %d, this one starts at %d", below->t0 + below->Nt, ctx->t0);
+    rc = enable_peer_for(ctx, below->links);
+    if (rc) return rc;
+    ctx->links_dn = below->links; ctx->Vh_dn = below->Vh; ctx->Nt_dn = below->Nt;
+    if (ctx->gtot) {
+        rc = enable_peer_for(ctx, above->gtot);
+        if (rc) return rc;
+        ctx->gtot_up = above->gtot; ctx->gapp_up = above->gapplied; ctx->Vh_up = above->Vh;
+    }
+    ctx->attached = true;
+    return GF_OK;
+}
+
+int gf_shard_export(gf_ctx* ctx, gf_shard_handle* h) {
+    if (!ctx || !h) return GF_EINVAL;
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "gf_shard_handle holds 64-byte CUDA IPC handles");
+    memset(h, 0, sizeof(*h));
+    CU(cudaIpcGetMemHandle((cudaIpcMemHandle_t*)h->links, ctx->links));
+    if (ctx->gtot) {
+        CU(cudaIpcGetMemHandle((cudaIpcMemHandle_t*)h->gtot, ctx->gtot));
+        if (ctx->gapplied) CU(cudaIpcGetMemHandle((cudaIpcMemHandle_t*)h->gapplied, ctx->gapplied));
+        h->has_transform = 1;
+    }
+    h->t0 = ctx->t0; h->Nt_local = ctx->Nt;
+    return GF_OK;
+}
+
+int gf_shard_attach_ipc(gf_ctx* ctx, const gf_shard_handle* below, const gf_shard_handle* above) {
+    if (!ctx || !below || !above) return GF_EINVAL;
+    if ((below->t0 + below->Nt_local) % ctx->NtG != ctx->t0 || above->t0 != (ctx->t0 + ctx->Nt) % ctx->NtG)
+        return fail(ctx, GF_EINVAL, "gf_shard_attach_ipc: neighbours do not adjoin slices [%d, %d)", ctx->t0, ctx->t0 + ctx->Nt);
+    if ((ctx->gtot != nullptr) != (above->has_transform != 0))
+        return fail(ctx, GF_EINVAL, "gf_shard_attach_ipc: GF_FLAG_TRACK_TRANSFORM differs between the shards");
+    const int64_t Vs2 = (int64_t)ctx->Nx * ctx->Ny * ctx->Nz / 2;
+    void* p = nullptr;
+    CU(cudaIpcOpenMemHandle(&p, *(const cudaIpcMemHandle_t*)below->links, cudaIpcMemLazyEnablePeerAccess));
+    ctx->ipc_opened.push_back(p);
+    ctx->links_dn = (char*)p; ctx->Nt_dn = below->Nt_local; ctx->Vh_dn = Vs2 * below->Nt_local;
+    if (ctx->gtot) {
+        CU(cudaIpcOpenMemHandle(&p, *(const cudaIpcMemHandle_t*)above->gtot, cudaIpcMemLazyEnablePeerAccess));
+        ctx->ipc_opened.push_back(p);
+        ctx->gtot_up = (char*)p;
+        CU(cudaIpcOpenMemHandle(&p, *(const cudaIpcMemHandle_t*)above->gapplied, cudaIpcMemLazyEnablePeerAccess));
+        ctx->ipc_opened.push_back(p);
+        ctx->gapp_up = (char*)p;
+        ctx->Vh_up = Vs2 * above->Nt_local;
+    }
+    ctx->attached = true;
+    return GF_OK;
+}
 
 int gf_set_links_copy(gf_ctx* ctx, int copy, const void* links, int elem_bytes, int is_device) {
     if (!ctx) return GF_EINVAL;
@@ -359,6 +537,7 @@ int gf_set_links_copy(gf_ctx* ctx, int copy, const void* links, int elem_bytes, 
     rc = reset_transform(ctx, copy);
     if (rc) return rc;
     CU(cudaStreamSynchronize(ctx->stream));
+    shard_barrier(ctx);
     ctx->copies_set[(size_t)copy] = 1;
     ctx->have_links = true;
     for (int c = 0; c < ctx->B; ++c) ctx->have_links = ctx->have_links && ctx->copies_set[(size_t)c];
@@ -471,6 +650,7 @@ int gf_get_gauge_transform(gf_ctx* ctx, void* g, int elem_bytes, int is_device) 
 static int check_sweep_args(gf_ctx* ctx, int gauge, int algo, double param) {
     if (!ctx) return GF_EINVAL;
     if (!ctx->have_links) return fail(ctx, GF_ESTATE, "no links set (call gf_set_links first)");
+    if (!ctx->attached) return fail(ctx, GF_ESTATE, "shard has no neighbours yet (gf_shard_attach)");
     if (gauge < GF_LANDAU || gauge > GF_MAG) return fail(ctx, GF_EINVAL, "unknown gauge %d", gauge);
     if (algo < GF_OR || algo > GF_MICRO) return fail(ctx, GF_EINVAL, "unknown algorithm %d", algo);
     if (algo == GF_OR && !(param >= 1.0 && param < 2.0)) return fail(ctx, GF_EINVAL, "omega = %g not in [1,2)", param);
@@ -493,6 +673,8 @@ static int launch_half(gf_ctx* ctx, int gauge, int algo, double param, uint64_t 
     a.rcp_nzh = fast_div_rcp(ctx->Nz / 2);
     a.rcp_ny = fast_div_rcp(ctx->Ny);
     a.pdl = ctx->pdl;
+    a.links_dn = ctx->links_dn; a.Vh_dn = ctx->Vh_dn; a.Nt_dn = ctx->Nt_dn; a.t_off = ctx->t0;
+    a.copy_links_bytes_dn = ctx->sharded ? 0 : link_store_bytes(ctx);
     const bool track = ctx->gtot != nullptr;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (ctx->timing) {
@@ -526,6 +708,9 @@ static int launch_half(gf_ctx* ctx, int gauge, int algo, double param, uint64_t 
     CU(e);
     ++ctx->launches;
     if (ctx->timing) CU(cudaEventRecord(e1, ctx->stream));
+    // t-shards: the next half-sweep of a neighbour touches the boundary links this one wrote;
+    // Coulomb sweeps touch spatial links only and need nothing
+    if (gauge != GF_COULOMB) shard_barrier(ctx);
     return GF_OK;
 }
 
@@ -592,11 +777,11 @@ int gf_sweep(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint
         dim3 grid((unsigned)ctx->meas_gx, (unsigned)ctx->NS, 2);                                           \
         const int64_t cb_ = link_store_bytes(ctx);                                                         \
         if ((gauge_) == GF_LANDAU)                                                                         \
-            measure_kernel<R, RECON, GAUGE_LANDAU><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_); \
+            measure_kernel<R, RECON, GAUGE_LANDAU><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_, shard_dn(ctx)); \
         else if ((gauge_) == GF_COULOMB)                                                                   \
-            measure_kernel<R, RECON, GAUGE_COULOMB><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_); \
+            measure_kernel<R, RECON, GAUGE_COULOMB><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_, shard_dn(ctx)); \
         else                                                                                               \
-            measure_kernel<R, RECON, GAUGE_MAG><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_); \
+            measure_kernel<R, RECON, GAUGE_MAG><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_, shard_dn(ctx)); \
     } while (0)
 
 // enqueue the reduction and the copy of the 2*Nt slice sums to pinned host memory
@@ -613,6 +798,7 @@ int gf_sweep(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint
     } while (0)
 
 static int enqueue_measure(gf_ctx* ctx, int gauge) {
+    shard_barrier(ctx);   // the first slice reads the neighbour's last one
     if (ctx->nc == 2) {
         if (ctx->real_bytes == 4) MEASURE2(float, gauge);
         else MEASURE2(double, gauge);
@@ -622,8 +808,23 @@ static int enqueue_measure(gf_ctx* ctx, int gauge) {
     slice_reduce_kernel<<<ctx->NS, 128, 0, ctx->stream>>>(ctx->partial, 2 * ctx->meas_gx, ctx->NS, ctx->slice_dev);
     CU(cudaGetLastError());
     ctx->launches += 2;
-    CU(cudaMemcpyAsync(ctx->slice_host, ctx->slice_dev, (size_t)2 * ctx->NS * sizeof(double), cudaMemcpyDeviceToHost,
-                       ctx->stream));
+    // slice_host = [F terms of the NSG global slices][theta terms of the NSG global slices]
+    if (ctx->sharded) {
+        memset(ctx->slice_host, 0, (size_t)2 * ctx->NSG * sizeof(double));
+        CU(cudaMemcpyAsync(ctx->slice_host + ctx->t0, ctx->slice_dev, (size_t)ctx->NS * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaMemcpyAsync(ctx->slice_host + ctx->NSG + ctx->t0, ctx->slice_dev + ctx->NS, (size_t)ctx->NS * sizeof(double),
+                           cudaMemcpyDeviceToHost, ctx->stream));
+    } else {
+        CU(cudaMemcpyAsync(ctx->slice_host, ctx->slice_dev, (size_t)2 * ctx->NS * sizeof(double), cudaMemcpyDeviceToHost,
+                           ctx->stream));
+    }
+    return GF_OK;
+}
+// wait for enqueue_measure's copies; t-shards: complete the global slice sums (every shard holds all of them and sums
+// them in slice order, so F, theta and every stopping decision are those of the unsharded lattice, bit for bit)
+static int finish_enqueued_measure(gf_ctx* ctx) {
+    CU(cudaStreamSynchronize(ctx->stream));
+    if (ctx->sharded) shard_allreduce(ctx, ctx->slice_host, 2 * ctx->NSG);
     return GF_OK;
 }
 
@@ -633,18 +834,18 @@ static void finish_measure(const gf_ctx* ctx, int gauge, int c, double* F, doubl
     const int nd = (gauge == GF_COULOMB) ? 3 : 4;
     const double ncd = (double)ctx->nc;   // N_c of Eqs. (4), (7), (11)
     const double Vs = (double)ctx->Nx * ctx->Ny * ctx->Nz;
-    const double* fs_ = ctx->slice_host + (size_t)c * ctx->Nt;
-    const double* th_ = ctx->slice_host + (size_t)ctx->NS + (size_t)c * ctx->Nt;
+    const double* fs_ = ctx->slice_host + (size_t)c * ctx->NtG;
+    const double* th_ = ctx->slice_host + (size_t)ctx->NSG + (size_t)c * ctx->NtG;
     double fs = 0.0, ths = 0.0, tmax = 0.0;
-    for (int t = 0; t < ctx->Nt; ++t) {
+    for (int t = 0; t < ctx->NtG; ++t) {
         fs += fs_[t];
         ths += th_[t];
         const double th_t = th_[t] / (ncd * Vs);
         if (theta_slice) theta_slice[t] = th_t;
         if (th_t > tmax) tmax = th_t;
     }
-    if (F) *F = fs / (ncd * nd * (double)ctx->V);
-    if (theta) *theta = ths / (ncd * (double)ctx->V);
+    if (F) *F = fs / (ncd * nd * (double)ctx->VG);
+    if (theta) *theta = ths / (ncd * (double)ctx->VG);
     if (theta_max) *theta_max = tmax;
 }
 
@@ -656,12 +857,15 @@ int gf_measure_batch(gf_ctx* ctx, int gauge, double* F, double* theta, double* t
         int rc = gf_coulomb_finalize(ctx);
         if (rc) return rc;
     }
-    int rc = enqueue_measure(ctx, gauge);
+    int rc = need_attached(ctx, "gf_measure");
     if (rc) return rc;
-    CU(cudaStreamSynchronize(ctx->stream));
+    rc = enqueue_measure(ctx, gauge);
+    if (rc) return rc;
+    rc = finish_enqueued_measure(ctx);
+    if (rc) return rc;
     for (int c = 0; c < ctx->B; ++c)
         finish_measure(ctx, gauge, c, F ? F + c : nullptr, theta ? theta + c : nullptr,
-                       theta_slice ? theta_slice + (size_t)c * ctx->Nt : nullptr, nullptr);
+                       theta_slice ? theta_slice + (size_t)c * ctx->NtG : nullptr, nullptr);
     return GF_OK;
 }
 
@@ -704,13 +908,14 @@ int gf_reunitarize(gf_ctx* ctx) {
         CU(cudaGetLastError());
         ++ctx->launches;
     }
+    shard_barrier(ctx);   // the neighbour above reads this store's last slice in its next half-sweep
     return GF_OK;
 }
 
 // ---- Coulomb finalisation ------------------------------------------------------------------------
 #define FINALIZE(R, RECON, dummy)                                                                           \
     coulomb_finalize_kernel<R, RECON><<<dim3((unsigned)((2 * ctx->Vh + 127) / 128), (unsigned)ctx->B), 128, 0, ctx->stream>>>( \
-        ctx->links, ctx->gtot, gapp, dims_of(ctx), link_store_bytes(ctx), field_store_bytes(ctx))
+        ctx->links, ctx->gtot, gapp, dims_of(ctx), link_store_bytes(ctx), field_store_bytes(ctx), up)
 
 int gf_coulomb_finalize(gf_ctx* ctx) {
     if (!ctx) return GF_EINVAL;
@@ -718,6 +923,16 @@ int gf_coulomb_finalize(gf_ctx* ctx) {
     if (!ctx->gtot) return fail(ctx, GF_ESTATE, "gf_coulomb_finalize: context created without GF_FLAG_TRACK_TRANSFORM");
     if (!ctx->temporal_stale) return GF_OK;
     const char* gapp = ctx->gapp_valid ? ctx->gapplied : nullptr;   // the g(x) the Coulomb sweeps started from
+    int rc_att = need_attached(ctx, "gf_coulomb_finalize");
+    if (rc_att) return rc_att;
+    // g(x + t_hat) of the last slice: the first slice of the store above (t-shards; every shard makes the same calls,
+    // so gapp_valid agrees between them), else this store (periodic wrap)
+    ShardUp up;
+    up.gtot_up = ctx->sharded ? ctx->gtot_up : ctx->gtot;
+    up.gapp_up = ctx->sharded ? (ctx->gapp_valid ? ctx->gapp_up : nullptr) : gapp;
+    up.Vh_up = ctx->sharded ? ctx->Vh_up : ctx->Vh;
+    up.copy_bytes_up = ctx->sharded ? 0 : field_store_bytes(ctx);
+    shard_barrier(ctx);   // the sweeps of the shard above are complete
     if (ctx->nc == 2) {
         const dim3 g((unsigned)((2 * ctx->Vh + 127) / 128), (unsigned)ctx->B);
         if (ctx->real_bytes == 4)
@@ -731,6 +946,7 @@ int gf_coulomb_finalize(gf_ctx* ctx) {
     CU(cudaGetLastError());
     ++ctx->launches;
     ctx->temporal_stale = false;   // the next start of Coulomb sweeps takes a new snapshot (coulomb_begin)
+    shard_barrier(ctx);            // the shard below reads g(x) of this store's first slice: not to be changed before it has
     return GF_OK;
 }
 
@@ -751,8 +967,7 @@ static int sweep_gx(const gf_ctx* ctx) {
 static int exact_measure(gf_ctx* ctx, int gauge) {
     int rc = enqueue_measure(ctx, gauge);
     if (rc) return rc;
-    CU(cudaStreamSynchronize(ctx->stream));
-    return GF_OK;
+    return finish_enqueued_measure(ctx);
 }
 
 /*
@@ -795,7 +1010,9 @@ static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t see
     const bool coulomb = gauge == GF_COULOMB;
     const bool per_slice = coulomb && (ctx->flags & GF_FLAG_FREEZE_SLICES);
     const int nd = coulomb ? 3 : 4;
-    const int Nt = ctx->Nt, B = ctx->B, NS = ctx->NS;
+    // host-side bookkeeping is per GLOBAL slice (t-shards: NSG = NtG slices of which this store holds [t0, t0 + Nt);
+    // otherwise NSG = NS = B * Nt); kernels and device arrays are per local slice
+    const int Nt = ctx->NtG, B = ctx->B, NS = ctx->NSG, NSloc = ctx->NS, goff = ctx->t0;
     const int nunits = per_slice ? NS : B, uspan = per_slice ? 1 : Nt;   // unit u = slices [u*uspan, (u+1)*uspan)
     const int gx = sweep_gx(ctx);
     const double Vs = (double)ctx->Nx * ctx->Ny * ctx->Nz;
@@ -811,7 +1028,10 @@ static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t see
     ctx->have_slice_sweeps = true;
     const bool use_skip = nunits > 1 || skip_slice;
     const unsigned char* skip = use_skip ? ctx->skip_dev : nullptr;
-    if (use_skip) memset(ctx->skip_host, 0, (size_t)NS);
+    if (use_skip) memset(ctx->skip_host, 0, (size_t)NSloc);
+    auto skip_set = [&](int sl) {   // global slice -> this store's flag array
+        if (sl - goff >= 0 && sl - goff < NSloc) ctx->skip_host[sl - goff] = 1;
+    };
 
     // stopping quantity of slices [lo, hi) from per-slice sums of theta terms val(s): Eq. (7) over the
     // slices' sites, or max_t theta_t for Coulomb
@@ -822,7 +1042,7 @@ static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t see
             tot += v;
             if (v / (ncd * Vs) > tmax) tmax = v / (ncd * Vs);
         }
-        return coulomb ? tmax : tot / (ncd * (double)ctx->V);
+        return coulomb ? tmax : tot / (ncd * (double)ctx->VG);
     };
     auto freeze_unit = [&](int u, int s_now) {
         unit_frozen[(size_t)u] = 1;
@@ -832,7 +1052,7 @@ static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t see
             fz_F[(size_t)sl] = ctx->slice_host[sl];
             fz_th[(size_t)sl] = ctx->slice_host[NS + sl];
             ctx->slice_sweeps[(size_t)sl] = s_now;
-            if (use_skip) ctx->skip_host[sl] = 1;
+            if (use_skip) skip_set(sl);
         }
     };
     // after an exact reduction (slice_host): stop every running unit whose exact stopping quantity is
@@ -845,11 +1065,11 @@ static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t see
             if (st < eps) { freeze_unit(u, s_now); changed = true; }
         }
         if (changed && use_skip)
-            CU(cudaMemcpyAsync(ctx->skip_dev, ctx->skip_host, (size_t)NS, cudaMemcpyHostToDevice, ctx->stream));
+            CU(cudaMemcpyAsync(ctx->skip_dev, ctx->skip_host, (size_t)NSloc, cudaMemcpyHostToDevice, ctx->stream));
         for (int c = 0; c < B; ++c) {
             double fs = 0.0;
             for (int sl = c * Nt; sl < (c + 1) * Nt; ++sl) fs += frozen[(size_t)sl] ? fz_F[(size_t)sl] : ctx->slice_host[sl];
-            Fc[(size_t)c] = fs / (ncd * nd * (double)ctx->V);
+            Fc[(size_t)c] = fs / (ncd * nd * (double)ctx->VG);
             stopc[(size_t)c] = stop_range(c * Nt, (c + 1) * Nt, [&](int sl) { return ctx->slice_host[NS + sl]; });
         }
         have_exact = true;
@@ -865,7 +1085,25 @@ static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t see
             if (all) freeze_unit(u, 0);
         }
     }
-    if (use_skip) CU(cudaMemcpyAsync(ctx->skip_dev, ctx->skip_host, (size_t)NS, cudaMemcpyHostToDevice, ctx->stream));
+    if (use_skip) CU(cudaMemcpyAsync(ctx->skip_dev, ctx->skip_host, (size_t)NSloc, cudaMemcpyHostToDevice, ctx->stream));
+
+    // fused partials of the even (and odd) half-sweep -> red_host = [NS][3] even, then [NS][3] odd, per global slice
+    auto fetch_red = [&](bool even, bool odd) -> int {
+        if (ctx->sharded) memset(ctx->red_host, 0, (size_t)6 * NS * sizeof(double));
+        for (int k = 0; k < 2; ++k) {
+            if (!(k ? odd : even)) continue;
+            red_reduce_kernel<<<NSloc, 128, 0, ctx->stream>>>(ctx->red_part[k], gx, ctx->red_dev + 3 * NSloc * k);
+            CU(cudaGetLastError());
+            ++ctx->launches;
+            CU(cudaMemcpyAsync(ctx->red_host + 3 * NS * k + 3 * goff, ctx->red_dev + 3 * NSloc * k, (size_t)3 * NSloc * sizeof(double),
+                               cudaMemcpyDeviceToHost, ctx->stream));
+        }
+        return GF_OK;
+    };
+    auto finish_red = [&]() -> int {   // after the copies of fetch_red have been waited for
+        if (ctx->sharded) shard_allreduce(ctx, ctx->red_host, 6 * NS);
+        return GF_OK;
+    };
 
     // history entry still waiting for the even sites' share of theta:
     //   stage 1 = the next even half-sweep must produce it, stage 2 = produced, reduced at the next check
@@ -898,31 +1136,27 @@ static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t see
         have_exact = false;
         if (!check_now) continue;
         if (!fused || reunit_now) {   // links were just reprojected: reduce what is stored now
-            if (pend_stage == 2) {
-                red_reduce_kernel<<<NS, 128, 0, ctx->stream>>>(ctx->red_part[0], gx, ctx->red_dev);
-                CU(cudaGetLastError());
-                ++ctx->launches;
-                CU(cudaMemcpyAsync(ctx->red_host, ctx->red_dev, (size_t)3 * NS * sizeof(double),
-                                   cudaMemcpyDeviceToHost, ctx->stream));
+            const bool had_pending = pend_stage == 2;
+            if (had_pending) {
+                rc = fetch_red(true, false);
+                if (rc) return rc;
             }
             rc = exact_measure(ctx, gauge);
             if (rc) return rc;
-            if (pend_stage == 2) complete_pending(ctx->red_host);
+            if (had_pending) {
+                rc = finish_red();
+                if (rc) return rc;
+                complete_pending(ctx->red_host);
+            }
             pend_stage = 0;
             rc = after_exact(s);
             if (rc) return rc;
         } else {
-            red_reduce_kernel<<<NS, 128, 0, ctx->stream>>>(ctx->red_part[1], gx, ctx->red_dev + 3 * NS);
-            CU(cudaGetLastError());
-            ++ctx->launches;
-            if (pend_stage == 2) {
-                red_reduce_kernel<<<NS, 128, 0, ctx->stream>>>(ctx->red_part[0], gx, ctx->red_dev);
-                CU(cudaGetLastError());
-                ++ctx->launches;
-            }
-            CU(cudaMemcpyAsync(ctx->red_host, ctx->red_dev, (size_t)6 * NS * sizeof(double), cudaMemcpyDeviceToHost,
-                               ctx->stream));
+            rc = fetch_red(pend_stage == 2, true);
+            if (rc) return rc;
             CU(cudaStreamSynchronize(ctx->stream));
+            rc = finish_red();
+            if (rc) return rc;
             const double* ev = ctx->red_host;            // [sl][3]: even half-sweep of this or an earlier sweep
             const double* od = ctx->red_host + 3 * NS;   // [sl][3]: odd half-sweep of sweep s
             if (pend_stage == 2) complete_pending(ev);
@@ -940,7 +1174,7 @@ static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t see
                 for (int c = 0; c < B; ++c) {
                     double fs = 0.0;
                     for (int sl = c * Nt; sl < (c + 1) * Nt; ++sl) fs += frozen[(size_t)sl] ? fz_F[(size_t)sl] : od[3 * sl];
-                    Fc[(size_t)c] = fs / (ncd * nd * (double)ctx->V);
+                    Fc[(size_t)c] = fs / (ncd * nd * (double)ctx->VG);
                     stopc[(size_t)c] = stop_range(c * Nt, (c + 1) * Nt, [&](int sl) { return od[3 * sl + 1]; });
                 }
                 for (int sl = 0; sl < NS; ++sl) pend_odd[(size_t)sl] = od[3 * sl + 1];
@@ -1009,7 +1243,7 @@ int gf_get_slice_sweeps(gf_ctx* ctx, int* sweeps) {
     if (!ctx) return GF_EINVAL;
     if (!sweeps) return fail(ctx, GF_EINVAL, "gf_get_slice_sweeps: NULL pointer");
     if (!ctx->have_slice_sweeps) return fail(ctx, GF_ESTATE, "gf_get_slice_sweeps: no gf_run yet");
-    for (int t = 0; t < ctx->NS; ++t) sweeps[t] = ctx->slice_sweeps[(size_t)t];
+    for (int t = 0; t < ctx->NSG; ++t) sweeps[t] = ctx->slice_sweeps[(size_t)t];
     return GF_OK;
 }
 
@@ -1064,7 +1298,7 @@ int gf_fix(gf_ctx* ctx, const gf_fix_params* p, gf_result* out) {
     if (!p) return fail(ctx, GF_EINVAL, "gf_fix: NULL parameters");
     if (p->sa_steps < 0 || p->sr_max_sweeps < 0 || p->or_max_sweeps < 0 || p->check_every < 1 || p->reunit_every < 0)
         return fail(ctx, GF_EINVAL, "gf_fix: bad stage lengths");
-    const int B = ctx->B, Nt = ctx->Nt, NS = ctx->NS;
+    const int B = ctx->B, Nt = ctx->NtG, NS = ctx->NSG;   // per global slice (run_impl)
     uint32_t idx = 0;
     int rc;
     std::vector<int> total((size_t)NS, 0);   // sweeps per slice, all stages
@@ -1116,6 +1350,7 @@ int gf_fix(gf_ctx* ctx, const gf_fix_params* p, gf_result* out) {
 int gf_random_gauge(gf_ctx* ctx, uint64_t seed) {
     if (!ctx) return GF_EINVAL;
     if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_random_gauge: no links set");
+    if (int rcs = not_on_shards(ctx, "gf_random_gauge")) return rcs;
     if (ctx->temporal_stale && ctx->gtot) {
         int rc = gf_coulomb_finalize(ctx);
         if (rc) return rc;
@@ -1163,6 +1398,7 @@ int gf_wilson_heatbath(gf_ctx* ctx, double beta, uint64_t seed, uint32_t first_s
     if (!ctx) return GF_EINVAL;
     if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_wilson_heatbath: no links set");
     if (!(beta > 0.0) || n_sweeps < 0) return fail(ctx, GF_EINVAL, "gf_wilson_heatbath: beta = %g, n_sweeps = %d", beta, n_sweeps);
+    if (int rcs = not_on_shards(ctx, "gf_wilson_heatbath")) return rcs;
     if (ctx->temporal_stale && ctx->gtot) {
         int rc = gf_coulomb_finalize(ctx);
         if (rc) return rc;
@@ -1200,6 +1436,7 @@ int gf_plaquette(gf_ctx* ctx, double* plaq) {
     if (!ctx) return GF_EINVAL;
     if (!plaq) return fail(ctx, GF_EINVAL, "gf_plaquette: NULL pointer");
     if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_plaquette: no links set");
+    if (int rcs = not_on_shards(ctx, "gf_plaquette")) return rcs;
     if (ctx->temporal_stale && ctx->gtot) {
         int rc = gf_coulomb_finalize(ctx);
         if (rc) return rc;
@@ -1292,24 +1529,31 @@ int gf_launch_count(gf_ctx* ctx, int64_t* launches, int reset) {
     return GF_OK;
 }
 
-// tuning hook (not declared in gf.h): 0 = gf_run measures after every check with the measure kernels
+// tuning hook (gf.h "Tuning hooks"): 0 = gf_run measures after every check with the measure kernels
 int gf_debug_set_fused(gf_ctx* ctx, int fused) {
     if (!ctx) return GF_EINVAL;
     ctx->fused = fused != 0;
     return GF_OK;
 }
 
-// tuning hook (not declared in gf.h): 0 = half-sweeps launched without programmatic dependent launch
+// tuning hook (gf.h "Tuning hooks"): 0 = half-sweeps launched without programmatic dependent launch
 int gf_debug_set_pdl(gf_ctx* ctx, int pdl) {
     if (!ctx) return GF_EINVAL;
     ctx->pdl = pdl != 0;
     return GF_OK;
 }
 
-// tuning hook (not declared in gf.h): CTA size of the half-sweep kernel, 0 = default
+// tuning hook (gf.h "Tuning hooks"): CTA size of the half-sweep kernel, 0 = default
 int gf_debug_set_block(gf_ctx* ctx, int block) {
     if (!ctx || block < 0 || (block & 31)) return GF_EINVAL;
     ctx->block_override = block;
+    return GF_OK;
+}
+
+// tuning hook (gf.h "Tuning hooks"): 0 = never use the persistent whole-run kernel
+int gf_debug_set_persistent(gf_ctx* ctx, int persistent) {
+    if (!ctx) return GF_EINVAL;
+    ctx->persistent = persistent != 0;
     return GF_OK;
 }
 

@@ -45,6 +45,14 @@ struct SweepArgs {
     int64_t copy_links_bytes, copy_gtot_bytes;
     uint32_t rcp_nzh, rcp_ny;   // floor(2^32 / (Nz/2)), floor(2^32 / Ny): site decode without integer division
     int pdl;                    // launch with programmatic stream serialization (host side only)
+    // t-sharding: this store holds the time-slices [t_off, t_off + Nt) of a
+    // lattice split over several link stores.  The only links a half-sweep touches outside its own store are
+    // U_0(x - t_hat) of its first slice: they are the last slice (Nt_dn - 1) of the store links_dn (Vh_dn sites per
+    // parity), which the kernel reads and writes in place (the same device, a peer mapping or an IPC mapping).
+    // Not sharded: links_dn = links, Vh_dn = Vh, Nt_dn = Nt, t_off = 0 (the periodic wrap in t).
+    char* links_dn;
+    int64_t Vh_dn, copy_links_bytes_dn;
+    int Nt_dn, t_off;
 };
 
 // Programmatic dependent launch (sm_90+): a half-sweep lets the next kernel in the stream be scheduled as soon as
@@ -300,12 +308,17 @@ sweep_kernel(const SweepArgs args) {
     const int par = (GAUGE == GAUGE_COULOMB) ? ((args.parity + t) & 1) : args.parity;
     const int r = (t + x + y + par) & 1;   // z = 2 zh + r
     const int z = 2 * zh + r;
-    const uint32_t site = (uint32_t)(((t * args.Nx + x) * args.Ny + y) * args.Nz + z);
+    // Philox site index: lexicographic in the whole lattice (t_off = first slice of this store; an even number,
+    // so the colouring above is the global one)
+    const uint32_t site = (uint32_t)((((uint32_t)(t + args.t_off) * (uint32_t)args.Nx + (uint32_t)x) * (uint32_t)args.Ny +
+                                      (uint32_t)y) * (uint32_t)args.Nz + (uint32_t)z);
 
     // checkerboard index of x - mu (lives in the other parity's arrays)
     const int sy = Nzh, sx = Nzh * args.Ny;
     const int64_t st = Vsh;
-    const int64_t cbn0 = cb + (t ? -st : (int64_t)(args.Nt - 1) * st);
+    // x - t_hat of the first slice: the last slice of the store links_dn (block-uniform)
+    const int64_t Vh_t = t ? Vh : args.Vh_dn;
+    const int64_t cbn0 = t ? cb - st : (int64_t)(args.Nt_dn - 1) * st + i_s;
     const int64_t cbn1 = cb + (x ? -sx : (args.Nx - 1) * sx);
     const int64_t cbn2 = cb + (y ? -sy : (args.Ny - 1) * sy);
     const int64_t cbn3 = r ? cb : (zh ? cb - 1 : cb + Nzh - 1);
@@ -320,6 +333,7 @@ sweep_kernel(const SweepArgs args) {
     const int64_t lstride = (int64_t)L::LINK_BYTES * Vh;
     char* const up0 = links + L::link_offset(par, MU0, Vh);        // U_mu(x): own parity
     char* const dn0 = links + L::link_offset(1 - par, MU0, Vh);    // U_mu(x - mu): other parity
+    char* const dnt = (t ? links : args.links_dn + copy * args.copy_links_bytes_dn) + L::link_offset(1 - par, 0, Vh_t);   // U_0(x - t_hat)
     pdl_wait();   // nothing of the previous kernel's output is read above this line
     {
         const char* pu = up0;
@@ -328,10 +342,11 @@ sweep_kernel(const SweepArgs args) {
         for (int m = 0; m < ND; ++m, pu += lstride, pd += lstride) {
             const int mu = MU0 + m;
             const int64_t cdn = (mu == 0) ? cbn0 : (mu == 1) ? cbn1 : (mu == 2) ? cbn2 : cbn3;
+            const int64_t plane_d = (mu == 0) ? 16 * Vh_t : plane;
             const char* qu = pu + cb * 16;
-            const char* qd = pd + cdn * 16;
+            const char* qd = ((mu == 0) ? dnt : pd) + cdn * 16;
 #pragma unroll
-            for (int c = 0; c < L::NV16; ++c, qu += plane, qd += plane) {
+            for (int c = 0; c < L::NV16; ++c, qu += plane, qd += plane_d) {
                 cp_async16(sbase + (uint32_t)(((2 * m) * L::NV16 + c) * NTHR * 16), qu);
                 cp_async16(sbase + (uint32_t)(((2 * m + 1) * L::NV16 + c) * NTHR * 16), qd);
             }
@@ -418,7 +433,7 @@ sweep_kernel(const SweepArgs args) {
             if (active) global_put<R, RECON>(pu, Vh, cb, O);
             smem_get<R, RECON, NTHR>(smem, NL, 2 * m + 1, U);
             mul_right_dagger<NR>(U, Gr, O);
-            if (active) global_put<R, RECON>(pd, Vh, cdn, O);
+            if (active) global_put<R, RECON>((mu == 0) ? dnt : pd, (mu == 0) ? Vh_t : Vh, cdn, O);
         }
     }
 

@@ -2,6 +2,8 @@
 // half-sweep kernels.  Included by sweep_<prec><recon>.cu, one translation unit per family so the
 // families compile in parallel.
 #pragma once
+#include <atomic>
+
 #include "sweep.cuh"
 
 namespace gf {
@@ -14,17 +16,19 @@ static cudaError_t launch_one(const SweepArgs& args, int block, cudaStream_t str
     block = sweep_block<R>(Vsh, block);
     // the slice stride is the maximal CTA size whatever the block (sweep.cuh, smem_get)
     const size_t smem = (size_t)SweepLaunch<R, A>::MAX_BLOCK * 2 * ND * Layout<R, RECON>::LINK_BYTES;
-    // function attributes are per device: remember what was set for this instantiation on each device
-    static size_t smem_set[64] = {0};
+    // function attributes are per device: remember what was set for this instantiation on each device.  Contexts may
+    // be driven from several host threads (one thread per context, gf.h): the cache is atomic, and setting the same
+    // attribute twice is harmless.
+    static std::atomic<size_t> smem_set[64];
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
-    if (dev < 0 || dev >= 64 || smem > smem_set[dev]) {
+    if (dev < 0 || dev >= 64 || smem > smem_set[dev].load(std::memory_order_acquire)) {
         e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
         if (e != cudaSuccess) return e;
-        if (dev >= 0 && dev < 64) smem_set[dev] = smem;
+        if (dev >= 0 && dev < 64) smem_set[dev].store(smem, std::memory_order_release);
     }
     const dim3 grid((unsigned)((Vsh + block - 1) / block), (unsigned)(args.ncopies * args.Nt));
     return launch_with_pdl(kern, grid, dim3((unsigned)block), smem, stream, args);

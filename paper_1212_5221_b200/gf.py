@@ -33,7 +33,9 @@ GF_FLAG_SU2 = 4
 EXPORTS = ["gf_create", "gf_num_colors", "gf_create_batch", "gf_num_copies", "gf_set_links_copy", "gf_get_links_copy",
            "gf_get_gauge_transform_copy", "gf_measure_batch", "gf_run_batch", "gf_fix", "gf_random_gauge", "gf_wilson_heatbath", "gf_plaquette", "gf_unitarity", "gf_destroy", "gf_set_links", "gf_get_links", "gf_get_gauge_transform", "gf_sweep",
            "gf_half_sweep", "gf_measure", "gf_run", "gf_get_slice_sweeps", "gf_anneal", "gf_reunitarize", "gf_coulomb_finalize",
-           "gf_sync", "gf_kernel_timing", "gf_kernel_time_ms", "gf_launch_count", "gf_device_bytes", "gf_volume", "gf_last_error", "gf_version"]
+           "gf_sync", "gf_kernel_timing", "gf_kernel_time_ms", "gf_launch_count", "gf_device_bytes", "gf_volume", "gf_last_error", "gf_version",
+           "gf_create_shard", "gf_shard_attach", "gf_shard_export", "gf_shard_attach_ipc", "gf_shard_set_comm", "gf_shard_info",
+           "gf_debug_set_fused", "gf_debug_set_pdl", "gf_debug_set_block", "gf_debug_set_persistent"]
 
 
 class gf_result(ctypes.Structure):
@@ -48,7 +50,26 @@ class gf_fix_params(ctypes.Structure):
                 ("reunit_every", ctypes.c_int)]
 
 
+class gf_shard_handle(ctypes.Structure):
+    _fields_ = [("links", ctypes.c_ubyte * 64), ("gtot", ctypes.c_ubyte * 64), ("gapplied", ctypes.c_ubyte * 64),
+                ("t0", ctypes.c_int), ("Nt_local", ctypes.c_int), ("has_transform", ctypes.c_int)]
+
+
+GF_BARRIER_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p)
+GF_ALLREDUCE_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.c_int)
+
+
+class gf_comm(ctypes.Structure):
+    _fields_ = [("barrier", GF_BARRIER_FN), ("allreduce_sum", GF_ALLREDUCE_FN), ("user", ctypes.c_void_p)]
+
+
 _vp, _ci, _cd, _u64, _u32 = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_uint64, ctypes.c_uint32
+_lib.gf_create_shard.argtypes = [ctypes.POINTER(_vp), _ci, _ci, _ci, _ci, _ci, _ci, _ci, _ci, ctypes.c_uint, _vp]
+_lib.gf_shard_attach.argtypes = [_vp, _vp, _vp]
+_lib.gf_shard_export.argtypes = [_vp, ctypes.POINTER(gf_shard_handle)]
+_lib.gf_shard_attach_ipc.argtypes = [_vp, ctypes.POINTER(gf_shard_handle), ctypes.POINTER(gf_shard_handle)]
+_lib.gf_shard_set_comm.argtypes = [_vp, ctypes.POINTER(gf_comm)]
+_lib.gf_shard_info.argtypes = [_vp, ctypes.POINTER(_ci), ctypes.POINTER(_ci), ctypes.POINTER(_ci)]
 _lib.gf_create_batch.argtypes = [ctypes.POINTER(_vp), _ci, _ci, _ci, _ci, _ci, _ci, _ci, ctypes.c_uint, _vp]
 _lib.gf_num_copies.argtypes = [_vp]
 _lib.gf_num_colors.argtypes = [_vp]
@@ -89,6 +110,7 @@ _lib.gf_version.restype = ctypes.c_char_p
 _lib.gf_debug_set_block.argtypes = [_vp, _ci]
 _lib.gf_debug_set_fused.argtypes = [_vp, _ci]
 _lib.gf_debug_set_pdl.argtypes = [_vp, _ci]
+_lib.gf_debug_set_persistent.argtypes = [_vp, _ci]
 
 
 class GfError(RuntimeError):
@@ -153,6 +175,41 @@ def gf_create_batch(Nx, Ny, Nz, Nt, n_copies, precision, recon=18, flags=0, cuda
                               _vp(_stream_handle(cuda_stream)))
     _check(None, rc)
     return h
+
+
+def gf_create_shard(Nx, Ny, Nz, Nt_local, t0, Nt_global, precision, recon=18, flags=0, cuda_stream=None):
+    """-> context holding the time-slices [t0, t0 + Nt_local) of an Nx*Ny*Nz*Nt_global lattice (gf.h, "t-shards")."""
+    h = _vp()
+    rc = _lib.gf_create_shard(ctypes.byref(h), Nx, Ny, Nz, Nt_local, t0, Nt_global, precision, recon, flags,
+                              _vp(_stream_handle(cuda_stream)))
+    _check(None, rc)
+    return h
+
+
+def gf_shard_attach(ctx, below, above):
+    return _check(ctx, _lib.gf_shard_attach(ctx, below, above))
+
+
+def gf_shard_export(ctx) -> gf_shard_handle:
+    h = gf_shard_handle()
+    _check(ctx, _lib.gf_shard_export(ctx, ctypes.byref(h)))
+    return h
+
+
+def gf_shard_attach_ipc(ctx, below: gf_shard_handle, above: gf_shard_handle):
+    return _check(ctx, _lib.gf_shard_attach_ipc(ctx, ctypes.byref(below), ctypes.byref(above)))
+
+
+def gf_shard_set_comm(ctx, comm):
+    """comm: a gf_comm (the caller keeps it, and the callables it was built from, alive) or None."""
+    return _check(ctx, _lib.gf_shard_set_comm(ctx, ctypes.byref(comm) if comm is not None else None))
+
+
+def gf_shard_info(ctx):
+    """-> (t0, Nt_local, Nt_global)"""
+    a, b, c = _ci(), _ci(), _ci()
+    _check(ctx, _lib.gf_shard_info(ctx, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)))
+    return a.value, b.value, c.value
 
 
 def gf_num_copies(ctx):
@@ -370,6 +427,10 @@ def gf_debug_set_pdl(ctx, pdl):
     return _check(ctx, _lib.gf_debug_set_pdl(ctx, 1 if pdl else 0))
 
 
+def gf_debug_set_persistent(ctx, persistent):
+    return _check(ctx, _lib.gf_debug_set_persistent(ctx, 1 if persistent else 0))
+
+
 def gf_debug_set_block(ctx, block):
     return _check(ctx, _lib.gf_debug_set_block(ctx, block))
 
@@ -378,13 +439,29 @@ class GaugeFixer:
     """Context manager around one gf_ctx.  Methods forward to the C entry points of the same name."""
 
     def __init__(self, Nx, Ny, Nz, Nt, precision=GF_DP, recon=18, track_transform=False, cuda_stream=None,
-                 freeze_slices=False, n_copies=1, su2=False):
+                 freeze_slices=False, n_copies=1, su2=False, shard=None):
+        """shard = (t0, Nt_global): the context holds the slices [t0, t0 + Nt) of an Nx*Ny*Nz*Nt_global lattice
+        (gf_create_shard); buffers of set_links / get_links / get_gauge_transform then are the shard's own slab."""
         self.dims = (Nx, Ny, Nz, Nt)
         self.precision, self.recon, self.n_copies = precision, recon, n_copies
         self.nc = 2 if su2 else 3
         flags = ((GF_FLAG_TRACK_TRANSFORM if track_transform else 0) | (GF_FLAG_FREEZE_SLICES if freeze_slices else 0)
                  | (GF_FLAG_SU2 if su2 else 0))
-        self.ctx = gf_create_batch(Nx, Ny, Nz, Nt, n_copies, precision, recon, flags, cuda_stream)
+        self.Nt_global = Nt
+        self._comm = None
+        if shard is None:
+            self.ctx = gf_create_batch(Nx, Ny, Nz, Nt, n_copies, precision, recon, flags, cuda_stream)
+        else:
+            t0, self.Nt_global = shard
+            self.ctx = gf_create_shard(Nx, Ny, Nz, Nt, t0, self.Nt_global, precision, recon, flags, cuda_stream)
+
+    def attach(self, below, above):
+        """below / above: the GaugeFixer shards (of this process) that hold the slices below and above this one."""
+        return gf_shard_attach(self.ctx, below.ctx, above.ctx)
+
+    def set_comm(self, comm):
+        self._comm = comm          # keeps the callbacks alive
+        return gf_shard_set_comm(self.ctx, comm)
 
     def close(self):
         if self.ctx is not None:
@@ -430,13 +507,13 @@ class GaugeFixer:
         return gf_half_sweep(self.ctx, gauge, algo, param, seed, sweep_index, parity)
 
     def measure(self, gauge, slices=False):
-        return gf_measure(self.ctx, gauge, self.dims[3] if slices else None)
+        return gf_measure(self.ctx, gauge, self.Nt_global if slices else None)
 
     def run(self, gauge, algo, param, **kw):
         return gf_run(self.ctx, gauge, algo, param, **kw)
 
     def slice_sweeps(self):
-        return gf_get_slice_sweeps(self.ctx, self.dims[3])
+        return gf_get_slice_sweeps(self.ctx, self.Nt_global)
 
     def anneal(self, gauge, T_hi, T_lo, n_steps, n_micro, seed, first_sweep_index=0):
         return gf_anneal(self.ctx, gauge, T_hi, T_lo, n_steps, n_micro, seed, first_sweep_index)

@@ -1,0 +1,223 @@
+"""t-shards (include/gf.h "t-shards"; Sec. 5) on ONE device.
+
+The lattice is split along t over 2 and 4 link stores (gf_create_shard); every shard is driven by its own host thread
+through the C ABI, all on one CUDA stream, with the thread communicator of paper_1212_5221_b200/shards.py supplying
+the barrier and the sum of the per-slice reduction arrays.  The first slice of a shard reads and writes the down-t links
+of the shard below in place, the Philox counter uses the site index in the whole lattice and the reductions are summed
+per global slice in slice order, so everything — links, g(x), F, theta, histories, sweep counts, annealing draws — must
+equal the unsharded context BIT FOR BIT (integer-exact bar; the unsharded context is held to the oracle elsewhere, and
+once here).  Several devices / processes (peer and IPC mappings) use the same kernels and were not run on hardware.
+"""
+import threading
+
+import numpy as np
+import pytest
+
+from paper_1212_5221_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+LANDAU, COULOMB, MAG = 0, 1, 2
+OR, SR, SA, MICRO = 0, 1, 2, 3
+SP, DP, MP = 0, 1, 2
+
+
+@pytest.fixture(scope="module")
+def gf():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1212_5221_b200 import gf as _gf
+    return _gf
+
+
+def config(dims, prec, eps=0.5, seed=301):
+    Nx, Ny, Nz, Nt = dims
+    dt = np.float64 if prec == DP else np.float32
+    return inputs.as_real(inputs.make_config(Nx, Ny, Nz, Nt, eps, seed, seed + 1), dt)
+
+
+def run_unsharded(gf, dims, L, body, **kw):
+    with gf.GaugeFixer(*dims, **kw) as fx:
+        fx.set_links(L)
+        return body(fx)
+
+
+def run_sharded(gf, dims, L, n_shards, body, **kw):
+    """body(fx) on every shard in its own thread; -> list of what body returned, in shard order.  The shards get
+    their slabs of L; get_links of a shard returns its slab."""
+    import torch
+    from paper_1212_5221_b200 import shards
+    Nx, Ny, Nz, Nt = dims
+    parts = shards.partition_t(Nt, n_shards)
+    stream = torch.cuda.Stream()
+    fxs = [gf.GaugeFixer(Nx, Ny, Nz, n, cuda_stream=stream, shard=(t0, Nt), **kw) for t0, n in parts]
+    comms = shards.ThreadComm.group(n_shards)
+    out, err = [None] * n_shards, [None] * n_shards
+    try:
+        for k, fx in enumerate(fxs):
+            fx.attach(fxs[(k - 1) % n_shards], fxs[(k + 1) % n_shards])
+            fx.set_comm(comms[k].comm)
+
+        def work(k):
+            try:
+                t0, n = parts[k]
+                fxs[k].set_links(np.ascontiguousarray(L[t0:t0 + n]))
+                out[k] = body(fxs[k])
+            except BaseException as e:   # noqa: BLE001 - reported by the main thread
+                err[k] = e
+                comms[k].shared.barrier.abort()
+
+        th = [threading.Thread(target=work, args=(k,)) for k in range(n_shards)]
+        for t in th:
+            t.start()
+        for t in th:
+            t.join()
+        for e in err:
+            if e is not None and not isinstance(e, threading.BrokenBarrierError):
+                raise e
+        for e in err:
+            if e is not None:
+                raise e
+    finally:
+        for fx in fxs:
+            fx.close()
+    return out
+
+
+def join_t(slabs):
+    return np.concatenate(slabs, axis=0)
+
+
+@pytest.mark.parametrize("n_shards", [2, 4])
+@pytest.mark.parametrize("prec,recon", [(DP, 18), (SP, 12)])
+def test_landau_or_run_bit_for_bit(gf, n_shards, prec, recon):
+    dims = (8, 8, 8, 16)
+    L = config(dims, prec)
+    dt = L.dtype
+    eps = 1e-12 if prec == DP else 1e-9
+    kw = dict(precision=prec, recon=recon, track_transform=True)
+
+    def body(fx):
+        r = fx.run(LANDAU, OR, 1.7, max_sweeps=60, eps=eps, check_every=3, reunit_every=20 if prec == SP else 0, history=True)
+        F, th, ts = fx.measure(LANDAU, slices=True)
+        return r, (F, th, ts), fx.get_links(dtype=dt), fx.get_gauge_transform(dtype=dt), fx.slice_sweeps()
+
+    ref = run_unsharded(gf, dims, L, body, **kw)
+    got = run_sharded(gf, dims, L, n_shards, body, **kw)
+    assert ref[0]["sweeps"] > 6
+    for g in got:       # every shard reports the global run
+        assert g[0]["sweeps"] == ref[0]["sweeps"] and g[0]["F"] == ref[0]["F"] and g[0]["theta"] == ref[0]["theta"]
+        assert np.array_equal(g[0]["history"], ref[0]["history"])
+        assert g[1][0] == ref[1][0] and g[1][1] == ref[1][1] and np.array_equal(g[1][2], ref[1][2])
+        assert np.array_equal(g[4], ref[4])
+    assert np.array_equal(join_t([g[2] for g in got]), ref[2])
+    assert np.array_equal(join_t([g[3] for g in got]), ref[3])
+
+
+def test_sharded_sweep_matches_oracle(gf, oracle):
+    # once against the oracle directly: one Landau OR sweep and one MAG heatbath sweep on 4 shards, DP per-link bars
+    dims = (6, 4, 8, 8)
+    L = config(dims, DP, seed=311)
+    for gauge, algo, param, tol in ((LANDAU, OR, 1.7, 1e-12), (MAG, SA, 0.8, 1e-11)):
+        ref = L.copy()
+        oracle.sweep(ref, gauge, algo, param, 77, 5)
+        got = run_sharded(gf, dims, L, 4, lambda fx: (fx.sweep(gauge, algo, param, seed=77, sweep_index=5), fx.get_links())[1],
+                          precision=DP)
+        assert np.abs(join_t(got) - ref).max() <= tol
+
+
+@pytest.mark.parametrize("n_shards", [2, 4])
+def test_mag_anneal_then_or_bit_for_bit(gf, n_shards):
+    # simulated annealing draws are keyed by the site index in the whole lattice
+    dims = (8, 8, 8, 16)
+    L = config(dims, DP, seed=321)
+    kw = dict(precision=DP, recon=18)
+
+    def body(fx):
+        nxt = fx.anneal(MAG, 1.2, 0.05, 6, 2, seed=99)
+        r = fx.run(MAG, OR, 1.7, seed=99, first_sweep_index=nxt, max_sweeps=40, eps=1e-10, check_every=4, history=True)
+        return nxt, r, fx.get_links()
+
+    ref = run_unsharded(gf, dims, L, body, **kw)
+    got = run_sharded(gf, dims, L, n_shards, body, **kw)
+    for g in got:
+        assert g[0] == ref[0] == 18
+        assert g[1]["sweeps"] == ref[1]["sweeps"] and g[1]["F"] == ref[1]["F"] and g[1]["theta"] == ref[1]["theta"]
+        assert np.array_equal(g[1]["history"], ref[1]["history"])
+    assert np.array_equal(join_t([g[2] for g in got]), ref[2])
+
+
+@pytest.mark.parametrize("n_shards", [2, 4])
+@pytest.mark.parametrize("freeze", [False, True])
+def test_coulomb_with_finalisation_bit_for_bit(gf, n_shards, freeze):
+    # Coulomb sweeps need nothing from the neighbours; the finalisation of the temporal links of a
+    # shard's last slice reads g(x + t_hat) from the shard above.  First a Landau sweep, so that the finalisation has to
+    # apply the increment only (g(x) snapshot at the start of the Coulomb sweeps, on every shard).
+    dims = (8, 8, 8, 16)
+    L = config(dims, DP, seed=331)
+    kw = dict(precision=DP, recon=18, track_transform=True, freeze_slices=freeze)
+
+    def body(fx):
+        fx.sweep(LANDAU, OR, 1.5)
+        r = fx.run(COULOMB, OR, 1.7, max_sweeps=400, eps=1e-11, check_every=5)
+        return r, fx.get_links(), fx.get_gauge_transform(), fx.slice_sweeps()
+
+    ref = run_unsharded(gf, dims, L, body, **kw)
+    got = run_sharded(gf, dims, L, n_shards, body, **kw)
+    assert ref[0]["converged"]
+    for g in got:
+        assert g[0]["sweeps"] == ref[0]["sweeps"] and g[0]["F"] == ref[0]["F"] and g[0]["theta"] == ref[0]["theta"]
+        assert np.array_equal(g[3], ref[3])
+    links, gt = join_t([g[1] for g in got]), join_t([g[2] for g in got])
+    assert np.array_equal(links, ref[1]) and np.array_equal(gt, ref[2])
+    # Eq. (1): the links returned are the input transformed by the g(x) returned, temporal links included
+    want = inputs.gauge_transform(inputs.as_complex(L), inputs.as_complex(gt))
+    assert np.abs(want - inputs.as_complex(links)).max() < 1e-12
+
+
+def test_full_size_slab_32x32x32x64_sp12(gf):
+    # the launch configuration of bench.py --shard-t on a 32^3 x 64 lattice, SP-12, 2 shards: 12 sweeps with a check
+    dims = (32, 32, 32, 64)
+    tile = config((16, 16, 16, 16), DP, seed=341)
+    L = np.ascontiguousarray(inputs.tile_lattice(tile, (4, 2, 2, 2, 1)).astype(np.float32))
+    kw = dict(precision=SP, recon=12)
+
+    def body(fx):
+        r = fx.run(LANDAU, OR, 1.7, max_sweeps=12, eps=-1.0, check_every=6, history=True)
+        return r, fx.get_links(dtype=np.float32)
+
+    ref = run_unsharded(gf, dims, L, body, **kw)
+    got = run_sharded(gf, dims, L, 2, body, **kw)
+    for g in got:
+        assert np.array_equal(g[0]["history"], ref[0]["history"])
+    assert np.array_equal(join_t([g[1] for g in got]), ref[1])
+
+
+def test_shard_argument_checks(gf):
+    with pytest.raises(gf.GfError):
+        gf.gf_create_shard(8, 8, 8, 4, 3, 16, DP)          # odd first slice
+    with pytest.raises(gf.GfError):
+        gf.gf_create_shard(8, 8, 8, 8, 12, 16, DP)         # past the end
+    with pytest.raises(gf.GfError):
+        gf.gf_create_shard(8, 8, 8, 8, 0, 16, DP, flags=gf.GF_FLAG_SU2)
+    a = gf.GaugeFixer(4, 4, 4, 4, shard=(0, 8))
+    b = gf.GaugeFixer(4, 4, 4, 4, shard=(4, 8))
+    try:
+        assert gf.gf_shard_info(b.ctx) == (4, 4, 8)
+        a.set_links(np.zeros(a.shape))
+        with pytest.raises(gf.GfError) as e:
+            a.sweep(LANDAU, OR, 1.7)                        # no neighbours yet
+        assert e.value.code == gf.GF_ESTATE
+        with pytest.raises(gf.GfError):
+            a.attach(a, b)                                  # a is not the shard below a
+        a.attach(b, b)
+        b.attach(a, a)
+        with pytest.raises(gf.GfError) as e:
+            a.random_gauge(1)
+        assert e.value.code == gf.GF_ESTATE
+        h = gf.gf_shard_export(a.ctx)
+        assert (h.t0, h.Nt_local, h.has_transform) == (0, 4, 0) and any(h.links)
+    finally:
+        a.close()
+        b.close()
