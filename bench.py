@@ -79,6 +79,9 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-others", action="store_true", help="skip the 32^3x64 and batched-copies side measurements")
     ap.add_argument("--block", type=int, default=0, help="CTA size override of the half-sweep kernel (tuning)")
+    ap.add_argument("--shard-t", action="store_true",
+                    help="N > 1: ONE lattice split along t over the N GPUs (t-shards, DESIGN.md §10; strong scaling) "
+                         "instead of N independent replicas")
     return ap.parse_args()
 
 
@@ -253,6 +256,101 @@ class Ranks:
     def close(self):
         if self.dist:
             self.dist.destroy_process_group()
+
+
+# ---- t-shards: one lattice over N GPUs (strong scaling) ---------------------------
+def run_sharded(args):
+    """`--shard-t`: rank k holds the k-th slab of time-slices of ONE lattice; the half-sweep kernel of a rank reads and
+    writes the boundary links in its neighbour's store in place through a CUDA IPC mapping (NVLink), torch.distributed
+    (NCCL) carries only the stream-ordered barrier after each half-sweep and the sum of 2 Nt slice sums per check."""
+    import torch
+    from paper_1212_5221_b200 import build as _build
+    _build.build()
+    from paper_1212_5221_b200 import gf, shards
+
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    ranks = Ranks("nccl", dev)
+    world, rank = ranks.world, ranks.rank
+    dims = tuple(int(x) for x in args.lattice.split(","))
+    Nx, Ny, Nz, Nt = dims
+    V, S = Nx * Ny * Nz * Nt, args.sweeps_per_step
+    peak, peak_src = peaks()
+    tile = make_tile()
+    stream = torch.cuda.Stream(device=dev)
+    prec, recon = args.precision, args.recon
+    reunit = 100 if prec != "dp" else 0
+
+    class _Dist:      # the part of torch.distributed the shard helpers use, also for a single rank
+        def __init__(self, d):
+            self.d = d
+
+        def get_world_size(self):
+            return world
+
+        def get_rank(self):
+            return rank
+
+        def __getattr__(self, n):
+            return getattr(self.d, n)
+
+    fx, comm, (t0, nloc) = shards.make_rank_shard(_Dist(ranks.dist), dev, stream, Nx, Ny, Nz, Nt,
+                                                   precision=PREC_NAMES[prec], recon=recon)
+    reps = reps_for((Nx, Ny, Nz, nloc))
+    with torch.cuda.stream(stream):
+        slab = torch.from_numpy(tile).to(dev).repeat(*reps, 1, 1, 1, 1).contiguous()
+    stream.synchronize()
+    fx.set_links(slab)
+    del slab
+
+    def step():
+        return fx.run(LANDAU, OR, OMEGA, seed=7, max_sweeps=S, eps=-1.0, check_every=S, reunit_every=reunit)
+
+    for _ in range(args.warmup):
+        step()
+    sampler = ClockSampler(local)
+    ranks.barrier(); torch.cuda.synchronize()
+    sampler.start()
+    gf.gf_launch_count(fx.ctx, reset=True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        r = step()
+    e1.record(stream)
+    ranks.barrier(); torch.cuda.synchronize()
+    ms = ranks.max_over_ranks(e0.elapsed_time(e1))
+    launches = gf.gf_launch_count(fx.ctx, reset=True)
+    clocks = sampler.stop()
+    bpsu = bytes_per_site_update(prec, recon)
+    # every rank streams its own slab once per half-sweep: aggregate algorithmic bytes over the slowest rank's time
+    achieved = bpsu * V * S * args.steps / (ms * 1e-3) / 1e9 / world
+    if rank == 0:
+        line = {
+            "metric": "site-updates/s (Landau OR sweep incl. F/theta reductions)", "value": V * S * args.steps / (ms * 1e-3),
+            "unit": "site-updates/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": DTYPE_NAMES[prec], "data": "synthetic",
+            "config": {"workload": f"Landau OR omega=1.7, {'x'.join(map(str, dims))} (BASELINE.json configs[4]), "
+                                   f"{prec.upper()}-{recon}, ONE lattice split along t over {world} GPU(s)",
+                       "lattice": list(dims), "precision": prec, "recon": recon,
+                       "parallelism": f"t-shards x{world}: {Nt // world} slices per GPU, boundary links read and written in "
+                                      "place in the neighbour's store (CUDA IPC mapping over NVLink), NCCL for the barrier "
+                                      "per half-sweep and the slice sums per check",
+                       "l2": "every slab >> 126 MB L2: streams from HBM"},
+            "paper_gflops": V * S * args.steps / (ms * 1e-3) * 2274 / 1e9,
+            "gpu_launches": launches, "F": r["F"], "theta": r["theta"],
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "kernel": "gf::sweep_kernel (one half-sweep, per GPU, whole step incl. barriers)",
+                         "peak_source": peak_src, "bytes_per_site_update": bpsu},
+            "clocks": clocks, "e2e": None, "cpu_baseline": None,
+            "comm_calls": comm.calls if comm else {"barrier": 0, "allreduce": 0},
+        }
+        print(json.dumps(line), flush=True)
+    fx.close()
+    ranks.close()
 
 
 # ---- the CUDA path ----------------------------------------------------------------------------
@@ -454,6 +552,58 @@ def run_ours(args):
                 "bytes_per_site_update": bpsu, "link_store_bytes": store,
                 "resident_in": "L2 (126 MB): not an HBM measurement" if store < 100e6 else "HBM"}
 
+    def bench_shards_one_device(dims_o, prec, recon, n_shards, sweeps, label):
+        """Side measurement: ONE lattice as n_shards t-shards on this device, all on one stream, every shard driven by its
+        own host thread (thread communicator).  Shows what the in-place boundary access and the per-half-sweep ordering
+        cost against the unsharded run of the same lattice (the multi-GPU path itself needs several GPUs)."""
+        import threading
+        from paper_1212_5221_b200 import shards
+        ox, oy, oz, ot = dims_o
+        Vo = ox * oy * oz * ot
+        parts = shards.partition_t(ot, n_shards)
+        fxs = [gf.GaugeFixer(ox, oy, oz, n, precision=PREC_NAMES[prec], recon=recon, cuda_stream=stream, shard=(t0, ot))
+               for t0, n in parts]
+        comms = shards.ThreadComm.group(n_shards)
+        res = {}
+        try:
+            for k, fx in enumerate(fxs):
+                fx.attach(fxs[(k - 1) % n_shards], fxs[(k + 1) % n_shards])
+                fx.set_comm(comms[k].comm)
+
+            def work(k):
+                t0, n = parts[k]
+                with torch.cuda.stream(stream):
+                    src = torch.from_numpy(tile).to(dev).repeat(n // TILE[3], ox // TILE[0], oy // TILE[1], oz // TILE[2], 1, 1, 1, 1).contiguous()
+                stream.synchronize()
+                fxs[k].set_links(src)
+                del src
+                fxs[k].run(LANDAU, OR, OMEGA, seed=7, max_sweeps=4, eps=-1.0, check_every=4)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                comms[k].shared.barrier.wait()
+                if k == 0:
+                    e0.record(stream)
+                r = fxs[k].run(LANDAU, OR, OMEGA, seed=7, max_sweeps=sweeps, eps=-1.0, check_every=sweeps)
+                comms[k].shared.barrier.wait()
+                if k == 0:
+                    e1.record(stream)
+                    stream.synchronize()
+                    res["ms"], res["F"] = e0.elapsed_time(e1), r["F"]
+
+            th = [threading.Thread(target=work, args=(k,)) for k in range(n_shards)]
+            for t in th:
+                t.start()
+            for t in th:
+                t.join()
+        finally:
+            for fx in fxs:
+                fx.close()
+        bpsu = bytes_per_site_update(prec, recon)
+        eff = bpsu * Vo * sweeps / (res["ms"] * 1e-3) / 1e9
+        return {"workload": label, "gauge_group": "SU(3)", "lattice": list(dims_o), "copies": 1, "shards": n_shards,
+                "precision": prec, "recon": recon, "sweeps": sweeps, "value": Vo * sweeps / (res["ms"] * 1e-3),
+                "unit": "site-updates/s", "whole_run_gbs": eff, "whole_run_frac": eff / peak, "bytes_per_site_update": bpsu,
+                "F": res["F"], "resident_in": "HBM"}
+
     others = []
     if rank == 0 and world == 1 and not args.no_others:
         del links_dev
@@ -474,6 +624,8 @@ def run_ours(args):
             bench_other((64, 64, 64, 256), 0, "sp", 4, 1, 100, "SU(2) Landau OR, 64^3x256, SP (4 reals per link)", su2=True),
             bench_other((64, 64, 64, 256), 0, "dp", 4, 1, 100, "SU(2) Landau OR, 64^3x256, DP (4 reals per link)", su2=True),
             bench_other((64, 64, 64, 256), 2, "mp", 4, 1, 100, "SU(2) MAG OR, 64^3x256, MP", su2=True),
+            bench_shards_one_device((64, 64, 64, 256), "sp", 12, 4, 50,
+                                    "Landau OR, 64^3x256, SP-12, ONE lattice as 4 t-shards on one device (one stream)"),
         ]
 
     cpu = None
@@ -516,6 +668,8 @@ def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.shard_t:
+        run_sharded(args)
     else:
         run_ours(args)
 

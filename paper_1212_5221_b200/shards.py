@@ -111,3 +111,29 @@ class TorchDistComm:
         else:
             self.dist.all_reduce(t)
         a[:] = t.numpy()
+
+
+def exchange_handles(dist, handle: "gf.gf_shard_handle"):
+    """All-gather the exported stores of the shards (one per rank, rank k = k-th slab) and return the handles of the
+    shards below and above this rank's (periodic).  Marshalling only: the handles are opaque bytes."""
+    world, rank = dist.get_world_size(), dist.get_rank()
+    blobs = [None] * world
+    dist.all_gather_object(blobs, bytes(handle))
+    hs = [gf.gf_shard_handle.from_buffer_copy(b) for b in blobs]
+    return hs[(rank - 1) % world], hs[(rank + 1) % world]
+
+
+def make_rank_shard(dist, device, stream, Nx, Ny, Nz, Nt_global, **kw):
+    """One process per GPU: this rank's shard of the lattice, attached to its neighbours' stores through CUDA IPC
+    mappings (NVLink peer access) and wired to torch.distributed.  -> (GaugeFixer, TorchDistComm, (t0, Nt_local))."""
+    world, rank = dist.get_world_size(), dist.get_rank()
+    t0, n = partition_t(Nt_global, world)[rank]
+    fx = gf.GaugeFixer(Nx, Ny, Nz, n, cuda_stream=stream, shard=(t0, Nt_global), **kw)
+    if world == 1:
+        fx.attach(fx, fx)
+        return fx, None, (t0, n)
+    below, above = exchange_handles(dist, gf.gf_shard_export(fx.ctx))
+    gf.gf_shard_attach_ipc(fx.ctx, below, above)
+    comm = TorchDistComm(dist, device=device, stream=stream)
+    fx.set_comm(comm.comm)
+    return fx, comm, (t0, n)
