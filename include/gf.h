@@ -67,6 +67,7 @@ typedef struct gf_ctx gf_ctx; /* opaque */
 #define GF_FLAG_TRACK_TRANSFORM 1u /* accumulate g(x) so that gf_get_gauge_transform / Coulomb finalisation work */
 #define GF_FLAG_SU2 4u /* gauge group SU(2) instead of SU(3) (Eqs. (8), (12)-(15), (20)-(29)); see "SU(2)" below */
 #define GF_FLAG_FREEZE_SLICES 2u   /* gf_run(Coulomb): stop sweeping a time-slice once its own theta_t < eps */
+#define GF_FLAG_LAGGED_STOP 8u     /* gf_run: take the stopping decision half a sweep late at no cost; see gf_run */
 
 /*
  * gf_create — allocate a context for an Nx*Ny*Nz*Nt periodic lattice (BASELINE.json north_star:
@@ -170,6 +171,17 @@ typedef struct {
  * 3 * (max_sweeps / check_every + 1) doubles, filled with (sweep, F, theta) per check.
  * For Coulomb with a tracked transform the temporal links are finalised before returning
  * (PAPER.md:448).  Returns GF_OK if converged, GF_NOT_CONVERGED otherwise.  Synchronous.
+ *
+ * Cost of a check: the odd half-sweep of a check sweep s leaves F(s) and the odd sites' share of theta(s), a lower
+ * bound of theta(s), at no extra traffic; only a check at which that bound is below eps runs the stand-alone
+ * reduction (one read of every link twice, about one half-sweep), so every stopping decision is the one a reduction
+ * after every check would take (Alg. 1).  With GF_FLAG_LAGGED_STOP (single lattice, not with
+ * GF_FLAG_FREEZE_SLICES) that reduction is not run either: the even sites' share of theta(s) is what the even
+ * half-sweep of sweep s + 1 sees before it updates, so theta(s) is known, exactly and at no cost, half a sweep later.
+ * If theta(s) < eps the run stops THERE: out->sweeps = s, and the links returned have received the even half-sweep of
+ * sweep s + 1 on top of Alg. 1's s sweeps (out->F, out->theta are those of the links returned; GF_OK).  A check at
+ * max_sweeps is decided by the stand-alone reduction as without the flag.  The oracle's run loop mirrors this reading
+ * (oracle/gf_oracle.py, lagged_stop).
  */
 int gf_run(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint32_t first_sweep_index,
            int max_sweeps, double eps, int check_every, int reunit_every, gf_result* out, double* hist);
@@ -381,13 +393,10 @@ const char* gf_version(void);
  *   gf_debug_set_pdl(ctx, 0)    half-sweeps are launched without programmatic dependent launch.
  *   gf_debug_set_block(ctx, n)  CTA size of the half-sweep kernel: a multiple of 32 up to the default (0 = default);
  *                               links are bit-identical for every n, fused partial sums differ in summation order.
- *   gf_debug_set_persistent(ctx, 0)  gf_run / gf_anneal never use the persistent whole-run kernel for small lattices
- *                               (DESIGN.md §6.9); same results bit for bit.
  */
 int gf_debug_set_fused(gf_ctx* ctx, int fused);
 int gf_debug_set_pdl(gf_ctx* ctx, int pdl);
 int gf_debug_set_block(gf_ctx* ctx, int block);
-int gf_debug_set_persistent(gf_ctx* ctx, int persistent);
 
 #ifdef __cplusplus
 }

@@ -218,10 +218,13 @@ def stop_value(m: dict, gauge: int) -> float:
 
 def run(links: np.ndarray, gauge: int, algo: int, param: float, seed: int = 0, max_sweeps: int = 1000,
         eps: float = 1e-12, check_every: int = 1, reunit_every: int = 0, mixed: bool = False,
-        gtot: np.ndarray | None = None, first_sweep_index: int = 0):
+        gtot: np.ndarray | None = None, first_sweep_index: int = 0, lagged_stop: bool = False):
     """Alg. 1's outer loop: sweep until theta < eps (checked every `check_every` sweeps) or
     max_sweeps; reproject every `reunit_every` sweeps.  Returns
-    (sweeps, F, theta, history[(sweep, F, theta)], converged)."""
+    (sweeps, F, theta, history[(sweep, F, theta)], converged).
+    lagged_stop (the reading of include/gf.h GF_FLAG_LAGGED_STOP, not Alg. 1's): a run that converges at a check
+    before max_sweeps applies the even half-sweep of the next sweep before it returns; F, theta returned are those
+    of the links returned, the history entry that of the check."""
     hist = []
     m = None
     s = 0
@@ -239,6 +242,9 @@ def run(links: np.ndarray, gauge: int, algo: int, param: float, seed: int = 0, m
             hist.append((s, m["F"], th))
             if th < eps:
                 conv = True
+                if lagged_stop and s < max_sweeps:
+                    sweep(links, gauge, algo, param, seed, first_sweep_index + s, mixed, gtot, parity_mask=1)
+                    m = measure(links, gauge)
                 break
     if m is None:
         m = measure(links, gauge)

@@ -72,7 +72,6 @@ struct gf_ctx {
     int64_t device_bytes;
     int block_override;     // 0 = default CTA size
     int pdl;                // half-sweeps launched with programmatic stream serialization (default 1)
-    int persistent;         // small lattices: whole runs in one cooperative launch where possible (default 1)
     // kernel timing (gf_kernel_timing)
     bool timing;
     std::vector<cudaEvent_t> ev;   // pairs (start, stop)
@@ -206,7 +205,7 @@ static int create_impl(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int n_copie
     ctx->fused = 1;
     ctx->skip_dev = nullptr; ctx->skip_host = nullptr; ctx->have_slice_sweeps = false;
     ctx->staging = nullptr; ctx->staging_bytes = 0;
-    ctx->device_bytes = 0; ctx->block_override = 0; ctx->pdl = 1; ctx->persistent = 1;
+    ctx->device_bytes = 0; ctx->block_override = 0; ctx->pdl = 1;
     ctx->timing = false; ctx->ev_used = 0; ctx->launches = 0;
     ctx->err[0] = 0;
     ctx->sharded = (NtG != Nt);
@@ -1116,6 +1115,14 @@ static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t see
                     stop_range(c * Nt, (c + 1) * Nt, [&](int sl) { return pend_odd[(size_t)sl] + ev[3 * sl + 2]; });
         pend_stage = 0;
     };
+    // GF_FLAG_LAGGED_STOP (one unit): a check whose lower bound theta_odd(s) falls below eps is not decided by the
+    // stand-alone reduction but half a sweep later, from the even sites' share that the even half-sweep of sweep s + 1
+    // sees before it updates: exact and free; if theta(s) < eps the run stops there (gf.h)
+    const bool lagged = fused && (ctx->flags & GF_FLAG_LAGGED_STOP) && nunits == 1 && !skip_slice;
+    bool lag_decide = false, lag_stopped = false;
+    // float Step 1 (GF_SP): the fused terms are formed from float sums and carry their rounding noise (~1e-12 in
+    // theta); the exact reduction is called for a little earlier so that the bound stays one
+    const double trig = eps + ((ctx->precision == GF_SP && eps > 0.0) ? (2e-12 > 1e-2 * eps ? 2e-12 : 1e-2 * eps) : 0.0);
     int s = 0, nh = 0, last_entry_sweep = -1;
     while (s < max_sweeps && n_frozen < nunits) {
         const bool check_now = ((s + 1) % check_every == 0) || (s + 1 == max_sweeps);
@@ -1124,6 +1131,18 @@ static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t see
         rc = launch_half(ctx, gauge, algo, param, seed, idx, 0, red_even ? ctx->red_part[0] : nullptr, skip);
         if (rc) return rc;
         if (red_even) pend_stage = 2;
+        if (lag_decide) {   // the decision of the check at sweep s, now that theta_even(s) is known
+            rc = fetch_red(true, false);
+            if (rc) return rc;
+            CU(cudaStreamSynchronize(ctx->stream));
+            rc = finish_red();
+            if (rc) return rc;
+            const double* ev0 = ctx->red_host;
+            const double th_s = stop_range(0, NS, [&](int sl) { return pend_odd[(size_t)sl] + ev0[3 * sl + 2]; });
+            complete_pending(ev0);
+            lag_decide = false;
+            if (th_s < eps) { lag_stopped = true; break; }
+        }
         const bool reunit_now = reunit_every && (s + 1) % reunit_every == 0;
         rc = launch_half(ctx, gauge, algo, param, seed, idx, 1,
                          (fused && check_now && !reunit_now) ? ctx->red_part[1] : nullptr, skip);
@@ -1164,7 +1183,11 @@ static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t see
             bool need_exact = false;
             for (int u = 0; u < nunits && !need_exact; ++u)
                 need_exact = !unit_frozen[(size_t)u] &&
-                             stop_range(u * uspan, (u + 1) * uspan, [&](int sl) { return od[3 * sl + 1]; }) < eps;
+                             stop_range(u * uspan, (u + 1) * uspan, [&](int sl) { return od[3 * sl + 1]; }) < trig;
+            if (need_exact && lagged && s < max_sweeps) {
+                lag_decide = true;
+                need_exact = false;
+            }
             if (need_exact) {
                 rc = exact_measure(ctx, gauge);
                 if (rc) return rc;
@@ -1195,12 +1218,13 @@ static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t see
         if (rc) return rc;
         rc = after_exact(s);
         if (rc) return rc;
-        if (hist && nh > 0 && last_entry_sweep == s)
+        if (hist && nh > 0 && last_entry_sweep == s && !lag_stopped)   // (lagged stop: the entry stays that of the check)
             for (int c = 0; c < B; ++c) {
                 double* h = hist + 3 * ((size_t)(nh - 1) * B + c);
                 h[1] = Fc[(size_t)c]; h[2] = stopc[(size_t)c];
             }
     }
+    if (lag_stopped && !unit_frozen[0]) freeze_unit(0, s);   // converged by theta(s); the links are half a sweep further
     for (int sl = 0; sl < NS; ++sl)
         if (!frozen[(size_t)sl]) ctx->slice_sweeps[(size_t)sl] = s;
     ctx->slice_frozen = frozen;
@@ -1547,13 +1571,6 @@ int gf_debug_set_pdl(gf_ctx* ctx, int pdl) {
 int gf_debug_set_block(gf_ctx* ctx, int block) {
     if (!ctx || block < 0 || (block & 31)) return GF_EINVAL;
     ctx->block_override = block;
-    return GF_OK;
-}
-
-// tuning hook (gf.h "Tuning hooks"): 0 = never use the persistent whole-run kernel
-int gf_debug_set_persistent(gf_ctx* ctx, int persistent) {
-    if (!ctx) return GF_EINVAL;
-    ctx->persistent = persistent != 0;
     return GF_OK;
 }
 

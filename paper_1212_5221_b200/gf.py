@@ -29,13 +29,14 @@ GF_OR, GF_SR, GF_SA, GF_MICRO = 0, 1, 2, 3
 GF_FLAG_TRACK_TRANSFORM = 1
 GF_FLAG_FREEZE_SLICES = 2
 GF_FLAG_SU2 = 4
+GF_FLAG_LAGGED_STOP = 8
 
 EXPORTS = ["gf_create", "gf_num_colors", "gf_create_batch", "gf_num_copies", "gf_set_links_copy", "gf_get_links_copy",
            "gf_get_gauge_transform_copy", "gf_measure_batch", "gf_run_batch", "gf_fix", "gf_random_gauge", "gf_wilson_heatbath", "gf_plaquette", "gf_unitarity", "gf_destroy", "gf_set_links", "gf_get_links", "gf_get_gauge_transform", "gf_sweep",
            "gf_half_sweep", "gf_measure", "gf_run", "gf_get_slice_sweeps", "gf_anneal", "gf_reunitarize", "gf_coulomb_finalize",
            "gf_sync", "gf_kernel_timing", "gf_kernel_time_ms", "gf_launch_count", "gf_device_bytes", "gf_volume", "gf_last_error", "gf_version",
            "gf_create_shard", "gf_shard_attach", "gf_shard_export", "gf_shard_attach_ipc", "gf_shard_set_comm", "gf_shard_info",
-           "gf_debug_set_fused", "gf_debug_set_pdl", "gf_debug_set_block", "gf_debug_set_persistent"]
+           "gf_debug_set_fused", "gf_debug_set_pdl", "gf_debug_set_block"]
 
 
 class gf_result(ctypes.Structure):
@@ -110,7 +111,6 @@ _lib.gf_version.restype = ctypes.c_char_p
 _lib.gf_debug_set_block.argtypes = [_vp, _ci]
 _lib.gf_debug_set_fused.argtypes = [_vp, _ci]
 _lib.gf_debug_set_pdl.argtypes = [_vp, _ci]
-_lib.gf_debug_set_persistent.argtypes = [_vp, _ci]
 
 
 class GfError(RuntimeError):
@@ -427,10 +427,6 @@ def gf_debug_set_pdl(ctx, pdl):
     return _check(ctx, _lib.gf_debug_set_pdl(ctx, 1 if pdl else 0))
 
 
-def gf_debug_set_persistent(ctx, persistent):
-    return _check(ctx, _lib.gf_debug_set_persistent(ctx, 1 if persistent else 0))
-
-
 def gf_debug_set_block(ctx, block):
     return _check(ctx, _lib.gf_debug_set_block(ctx, block))
 
@@ -439,14 +435,14 @@ class GaugeFixer:
     """Context manager around one gf_ctx.  Methods forward to the C entry points of the same name."""
 
     def __init__(self, Nx, Ny, Nz, Nt, precision=GF_DP, recon=18, track_transform=False, cuda_stream=None,
-                 freeze_slices=False, n_copies=1, su2=False, shard=None):
+                 freeze_slices=False, n_copies=1, su2=False, shard=None, lagged_stop=False):
         """shard = (t0, Nt_global): the context holds the slices [t0, t0 + Nt) of an Nx*Ny*Nz*Nt_global lattice
         (gf_create_shard); buffers of set_links / get_links / get_gauge_transform then are the shard's own slab."""
         self.dims = (Nx, Ny, Nz, Nt)
         self.precision, self.recon, self.n_copies = precision, recon, n_copies
         self.nc = 2 if su2 else 3
         flags = ((GF_FLAG_TRACK_TRANSFORM if track_transform else 0) | (GF_FLAG_FREEZE_SLICES if freeze_slices else 0)
-                 | (GF_FLAG_SU2 if su2 else 0))
+                 | (GF_FLAG_SU2 if su2 else 0) | (GF_FLAG_LAGGED_STOP if lagged_stop else 0))
         self.Nt_global = Nt
         self._comm = None
         if shard is None:

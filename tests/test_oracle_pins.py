@@ -604,3 +604,23 @@ def test_invalid_extents_rejected(oracle):
     L = np.zeros((3, 4, 4, 4, 4, 3, 3, 2))
     with pytest.raises(ValueError):
         oracle.sweep(L, LANDAU, OR, 1.7)
+
+
+def test_lagged_stop_reading_is_the_plain_run_plus_one_even_half_sweep(oracle):
+    # include/gf.h GF_FLAG_LAGGED_STOP: same checks, same stopping sweep, same history; the links returned have received
+    # the even half-sweep of the next sweep (a gauge transformation: plaquettes unchanged, Eq. (1))
+    from paper_1212_5221_b200 import inputs
+    L0 = inputs.as_real(inputs.make_config(4, 4, 4, 4, 0.4, 91, 92))
+    a, b = L0.copy(), L0.copy()
+    sa, Fa, tha, ha, ca = oracle.run(a, oracle.LANDAU, oracle.OR, 1.7, max_sweeps=500, eps=1e-10, check_every=3)
+    sb, Fb, thb, hb, cb = oracle.run(b, oracle.LANDAU, oracle.OR, 1.7, max_sweeps=500, eps=1e-10, check_every=3, lagged_stop=True)
+    assert ca and cb and sa == sb and ha == hb
+    oracle.sweep(a, oracle.LANDAU, oracle.OR, 1.7, 0, sa, parity_mask=1)
+    assert np.array_equal(a, b)
+    m = oracle.measure(b, oracle.LANDAU)
+    assert Fb == m["F"] and thb == m["theta"] and Fb >= Fa - 1e-15
+    # a run that exhausts max_sweeps is not touched
+    c, d = L0.copy(), L0.copy()
+    assert oracle.run(c, oracle.LANDAU, oracle.OR, 1.7, max_sweeps=6, eps=1e-10)[:3] == \
+        oracle.run(d, oracle.LANDAU, oracle.OR, 1.7, max_sweeps=6, eps=1e-10, lagged_stop=True)[:3]
+    assert np.array_equal(c, d)
