@@ -47,14 +47,21 @@ PREC_NAMES = {"sp": 0, "dp": 1, "mp": 2}
 DTYPE_NAMES = {"sp": "f32", "dp": "f64", "mp": "f32 (Step 1 in f64)"}
 
 # dram__bytes_read.sum + dram__bytes_write.sum per half-sweep launch from the `ncu --set full`
-# captures summarised under profiles/ (bytes; key = (precision, recon, "NxxNyxNzxNt")).
-NCU_TRAFFIC = {}
+# captures summarised under profiles/ (bytes; key = (workload, precision, recon, "NxxNyxNzxNt"), workload = "or" for
+# the overrelaxation kernels).  The file names the commit whose kernels were captured: it has to be regenerated when a
+# kernel changes, and the bench line says which capture it quotes.
+NCU_TRAFFIC, NCU_TRAFFIC_COMMIT = {}, None
 try:
     with open(os.path.join(ROOT, "profiles", "traffic.csv")) as _fh:
         for _line in _fh:
+            if _line.startswith("# captured_at_commit:"):
+                NCU_TRAFFIC_COMMIT = _line.split(":", 1)[1].strip()
             _f = _line.strip().split(",")
-            if len(_f) >= 4 and _f[0] in PREC_NAMES:
-                NCU_TRAFFIC[(_f[0], int(_f[1]), _f[2])] = float(_f[3])
+            if len(_f) >= 4 and not _line.startswith("#"):
+                _wl = _f[8] if len(_f) > 8 else "or"
+                _prec = _f[0].split("_")[-1]
+                if _prec in PREC_NAMES:
+                    NCU_TRAFFIC[("or" if _wl.startswith("or") else _wl, _prec, int(_f[1]), _f[2])] = float(_f[3])
 except OSError:
     pass
 
@@ -400,6 +407,7 @@ def run_ours(args):
     ALGO = {"or": 0, "sr": 1, "sa": 2, "micro": 3}[args.algo]
     if (GAUGE, ALGO) != (LANDAU, OR):
         args.no_variants, args.no_cpu_baseline, args.no_others = True, True, True
+    TRAFFIC_KEY = "or" if ALGO == OR and GAUGE == LANDAU else ("sa_mag" if (GAUGE, ALGO) == (2, 2) else ("sa" if (GAUGE, ALGO) == (0, 2) else "none"))
 
     def bench_one(prec: str, recon: int, steps: int, warmup: int, e2e: bool, sample_clocks: bool):
         reunit = 100 if prec != "dp" else 0
@@ -447,7 +455,8 @@ def run_ours(args):
                 "kernel_share_of_step": kern_ms / ms,
                 "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                              "frac": achieved / peak, "frac_of_8TBps_nominal": achieved / 8000.0,
-                             "traffic": NCU_TRAFFIC.get((prec, recon, lat_name)),
+                             "traffic": NCU_TRAFFIC.get((TRAFFIC_KEY, prec, recon, lat_name)),
+                             "traffic_source": f"profiles/traffic.csv, ncu --set full capture of the kernels of commit {NCU_TRAFFIC_COMMIT}",
                              "kernel": "gf::sweep_su2_kernel (one half-sweep)" if su2 else "gf::sweep_kernel (one half-sweep)",
                              "peak_source": peak_src,
                              "algorithmic_bytes_per_launch": per_launch_bytes,
