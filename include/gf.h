@@ -156,6 +156,15 @@ int gf_half_sweep(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed,
 int gf_measure(gf_ctx* ctx, int gauge, double* F, double* theta, double* theta_slice);
 /* the same for every copy: F[n_copies], theta[n_copies], theta_slice NULL or [n_copies][Nt] */
 int gf_measure_batch(gf_ctx* ctx, int gauge, double* F, double* theta, double* theta_slice);
+/*
+ * gf_measure_mag_eq16 — the maximally Abelian precision as Eq. (16) prints it for SU(3),
+ * theta_eq16[c] = 1/(N_c V) sum_x |X_12 + Y_12 + Z_12|^2 for every copy c, the sum over the three SU(2) subgroups INSIDE
+ * the modulus.  gf_measure / gf_run use sum_x sum_s |X^s_12|^2 / (N_c V) instead (R11): a norm, zero exactly
+ * at a stationary point, whereas the printed form can vanish away from one; theta_eq16 <= 3 theta, and the two differ by
+ * the cross terms.  eps thresholds and MAG theta values quoted from the paper (Table 4, Fig. 7) refer to the printed
+ * form: compare them with this call.  SU(3) contexts only (GF_ESTATE otherwise).  Synchronous.
+ */
+int gf_measure_mag_eq16(gf_ctx* ctx, double* theta_eq16);
 
 typedef struct {
     int sweeps;   /* sweeps performed */

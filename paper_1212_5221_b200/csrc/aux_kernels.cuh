@@ -169,7 +169,7 @@ struct ShardDn {
 };
 
 template <class R, int RECON, int GAUGE>
-__global__ void measure_kernel(const char* links, Dims d, double* partial, int64_t copy_bytes, ShardDn sh) {
+__global__ void measure_kernel(const char* links, Dims d, double* partial, int64_t copy_bytes, ShardDn sh, int mag_eq16) {
     typedef Layout<R, RECON> L;
     constexpr int MU0 = (GAUGE == GAUGE_COULOMB) ? 1 : 0;
     const int Nzh = d.Nz >> 1;
@@ -220,13 +220,18 @@ __global__ void measure_kernel(const char* links, Dims d, double* partial, int64
         }
         if (GAUGE == GAUGE_MAG) {
             // theta: sum over the three subgroups of |X^s_12|^2 = E_s^2 + F_s^2 (R11)
+            // mag_eq16: Eq. (16) as printed, |X_12 + Y_12 + Z_12|^2 with the sum over the subgroups
+            // INSIDE the modulus: not a norm (it can vanish away from a maximum), reported for comparison with the paper
             const int SI[3] = {0, 0, 1}, SJ[3] = {1, 2, 2};
+            double Es = 0.0, Fs = 0.0;
 #pragma unroll
             for (int s = 0; s < 3; ++s) {
                 const double E = M[SI[s]].o[2 * s + 1] - M[SJ[s]].o[2 * s + 1];
                 const double F = M[SI[s]].o[2 * s] - M[SJ[s]].o[2 * s];
                 th_term += E * E + F * F;
+                Es += E; Fs += F;
             }
+            if (mag_eq16) th_term = Es * Es + Fs * Fs;
         } else {
             // Delta = traceless[(K - K^dag)/2i] (Eqs. (6)); tr[Delta Delta^dag] (Eq. (7))
             double sum = 0.0, tr = 0.0;

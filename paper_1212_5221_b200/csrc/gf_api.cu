@@ -776,11 +776,11 @@ int gf_sweep(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint
         dim3 grid((unsigned)ctx->meas_gx, (unsigned)ctx->NS, 2);                                           \
         const int64_t cb_ = link_store_bytes(ctx);                                                         \
         if ((gauge_) == GF_LANDAU)                                                                         \
-            measure_kernel<R, RECON, GAUGE_LANDAU><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_, shard_dn(ctx)); \
+            measure_kernel<R, RECON, GAUGE_LANDAU><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_, shard_dn(ctx), eq16_); \
         else if ((gauge_) == GF_COULOMB)                                                                   \
-            measure_kernel<R, RECON, GAUGE_COULOMB><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_, shard_dn(ctx)); \
+            measure_kernel<R, RECON, GAUGE_COULOMB><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_, shard_dn(ctx), eq16_); \
         else                                                                                               \
-            measure_kernel<R, RECON, GAUGE_MAG><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_, shard_dn(ctx)); \
+            measure_kernel<R, RECON, GAUGE_MAG><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_, shard_dn(ctx), eq16_); \
     } while (0)
 
 // enqueue the reduction and the copy of the 2*Nt slice sums to pinned host memory
@@ -796,7 +796,7 @@ int gf_sweep(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint
             measure2_kernel<R, GAUGE_MAG><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_); \
     } while (0)
 
-static int enqueue_measure(gf_ctx* ctx, int gauge) {
+static int enqueue_measure(gf_ctx* ctx, int gauge, int eq16_ = 0) {
     shard_barrier(ctx);   // the first slice reads the neighbour's last one
     if (ctx->nc == 2) {
         if (ctx->real_bytes == 4) MEASURE2(float, gauge);
@@ -865,6 +865,25 @@ int gf_measure_batch(gf_ctx* ctx, int gauge, double* F, double* theta, double* t
     for (int c = 0; c < ctx->B; ++c)
         finish_measure(ctx, gauge, c, F ? F + c : nullptr, theta ? theta + c : nullptr,
                        theta_slice ? theta_slice + (size_t)c * ctx->NtG : nullptr, nullptr);
+    return GF_OK;
+}
+
+int gf_measure_mag_eq16(gf_ctx* ctx, double* theta_eq16) {
+    if (!ctx) return GF_EINVAL;
+    if (!theta_eq16) return fail(ctx, GF_EINVAL, "gf_measure_mag_eq16: NULL pointer");
+    if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_measure_mag_eq16: no links set");
+    if (ctx->nc != 3) return fail(ctx, GF_ESTATE, "gf_measure_mag_eq16: N_c = 2 has one subgroup, gf_measure's theta is Eq. (13)");
+    int rc = need_attached(ctx, "gf_measure_mag_eq16");
+    if (rc) return rc;
+    if (ctx->temporal_stale) {
+        rc = gf_coulomb_finalize(ctx);
+        if (rc) return rc;
+    }
+    rc = enqueue_measure(ctx, GF_MAG, 1);
+    if (rc) return rc;
+    rc = finish_enqueued_measure(ctx);
+    if (rc) return rc;
+    for (int c = 0; c < ctx->B; ++c) finish_measure(ctx, GF_MAG, c, nullptr, theta_eq16 + c, nullptr, nullptr);
     return GF_OK;
 }
 

@@ -280,6 +280,7 @@ sweep_kernel(const SweepArgs args) {
     constexpr int MU0 = (GAUGE == GAUGE_COULOMB) ? 1 : 0;
     constexpr int ND = 4 - MU0;
     constexpr int NL = 2 * ND;
+    static_assert(SweepLaunch<R, A>::MAX_BLOCK <= 128, "red_s below holds the partial sums of at most four warps");
     extern __shared__ __align__(16) unsigned char smem[];
 
     // grid = (ceil(Vsh / block), ncopies*Nt): blockIdx.y is (gauge copy, time-slice), so a CTA never

@@ -24,6 +24,7 @@ __global__ void __launch_bounds__(128, sizeof(R) == 8 ? 3 : 4) sweep_su2_kernel(
     typedef Layout<R, 4> L;
     constexpr int MU0 = (GAUGE == GAUGE_COULOMB) ? 1 : 0;
     constexpr int ND = 4 - MU0;
+    // (CTAs of at most 128 threads: red_s below holds the partial sums of four warps; sweep_su2_block)
     pdl_launch_dependents();
     const int Nzh = args.Nz >> 1;
     const int Vsh = args.Nx * args.Ny * Nzh;
@@ -46,7 +47,8 @@ __global__ void __launch_bounds__(128, sizeof(R) == 8 ? 3 : 4) sweep_su2_kernel(
     const int par = (GAUGE == GAUGE_COULOMB) ? ((args.parity + t) & 1) : args.parity;
     const int r = (t + x + y + par) & 1;
     const int z = 2 * zh + r;
-    const uint32_t site = (uint32_t)(((t * args.Nx + x) * args.Ny + y) * args.Nz + z);
+    const uint32_t site = (uint32_t)((((uint32_t)t * (uint32_t)args.Nx + (uint32_t)x) * (uint32_t)args.Ny + (uint32_t)y) *
+                                     (uint32_t)args.Nz + (uint32_t)z);   // unsigned: V may exceed 2^31
     const int sy = Nzh, sx = Nzh * args.Ny;
     const int64_t st = Vsh;
     int64_t cbn[4];

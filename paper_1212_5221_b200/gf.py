@@ -32,7 +32,7 @@ GF_FLAG_SU2 = 4
 GF_FLAG_LAGGED_STOP = 8
 
 EXPORTS = ["gf_create", "gf_num_colors", "gf_create_batch", "gf_num_copies", "gf_set_links_copy", "gf_get_links_copy",
-           "gf_get_gauge_transform_copy", "gf_measure_batch", "gf_run_batch", "gf_fix", "gf_random_gauge", "gf_wilson_heatbath", "gf_plaquette", "gf_unitarity", "gf_destroy", "gf_set_links", "gf_get_links", "gf_get_gauge_transform", "gf_sweep",
+           "gf_get_gauge_transform_copy", "gf_measure_batch", "gf_measure_mag_eq16", "gf_run_batch", "gf_fix", "gf_random_gauge", "gf_wilson_heatbath", "gf_plaquette", "gf_unitarity", "gf_destroy", "gf_set_links", "gf_get_links", "gf_get_gauge_transform", "gf_sweep",
            "gf_half_sweep", "gf_measure", "gf_run", "gf_get_slice_sweeps", "gf_anneal", "gf_reunitarize", "gf_coulomb_finalize",
            "gf_sync", "gf_kernel_timing", "gf_kernel_time_ms", "gf_launch_count", "gf_device_bytes", "gf_volume", "gf_last_error", "gf_version",
            "gf_create_shard", "gf_shard_attach", "gf_shard_export", "gf_shard_attach_ipc", "gf_shard_set_comm", "gf_shard_info",
@@ -78,6 +78,7 @@ _lib.gf_set_links_copy.argtypes = [_vp, _ci, _vp, _ci, _ci]
 _lib.gf_get_links_copy.argtypes = [_vp, _ci, _vp, _ci, _ci]
 _lib.gf_get_gauge_transform_copy.argtypes = [_vp, _ci, _vp, _ci, _ci]
 _lib.gf_measure_batch.argtypes = [_vp, _ci, _vp, _vp, _vp]
+_lib.gf_measure_mag_eq16.argtypes = [_vp, _vp]
 _lib.gf_run_batch.argtypes = [_vp, _ci, _ci, _cd, _u64, _u32, _ci, _cd, _ci, _ci, _vp, _vp]
 _lib.gf_fix.argtypes = [_vp, ctypes.POINTER(gf_fix_params), _vp]
 _lib.gf_random_gauge.argtypes = [_vp, _u64]
@@ -277,6 +278,13 @@ def gf_measure_batch(ctx, gauge, Nt=None):
     _check(ctx, _lib.gf_measure_batch(ctx, gauge, _vp(F.ctypes.data), _vp(th.ctypes.data),
                                       _vp(ts.ctypes.data) if Nt else None))
     return (F, th, ts) if Nt else (F, th)
+
+
+def gf_measure_mag_eq16(ctx):
+    """-> theta[n_copies] of Eq. (16) as printed (sum over the subgroups inside the modulus); gf.h."""
+    th = np.zeros(gf_num_copies(ctx))
+    _check(ctx, _lib.gf_measure_mag_eq16(ctx, _vp(th.ctypes.data)))
+    return th
 
 
 def gf_run_batch(ctx, gauge, algo, param, seed=0, first_sweep_index=0, max_sweeps=1000, eps=1e-12, check_every=1,
@@ -538,6 +546,9 @@ class GaugeFixer:
             out = np.empty(self.shape[:4] + self.shape[-3:], dtype=dtype)
         gf_get_gauge_transform_copy(self.ctx, copy, out)
         return out
+
+    def measure_mag_eq16(self):
+        return gf_measure_mag_eq16(self.ctx)
 
     def measure_batch(self, gauge, slices=False):
         return gf_measure_batch(self.ctx, gauge, self.dims[3] if slices else None)

@@ -192,6 +192,32 @@ def test_measure_matches_oracle(gf, oracle, prec, recon, gauge):
     assert (F, th) == (F2, th2)          # fixed summation order: bit-reproducible
 
 
+@pytest.mark.parametrize("prec,recon", [(DP, 18), (DP, 12), (SP, 12)])
+def test_mag_theta_as_printed_in_eq16_matches_oracle(gf, oracle, prec, recon):
+    # Eq. (16) as printed (sum over the subgroups inside the modulus) next to the stopping theta of R11;
+    # the oracle's value is pinned to Eq. (12) evaluated with NumPy matrices (tests/test_oracle_pins.py)
+    dims = (6, 4, 10, 6)
+    dt = oracle_dtype(prec)
+    Ls = [inputs.as_real(make(dims, seed=340 + c), dt) for c in range(2)]
+    for L in Ls:
+        oracle.sweep(L, MAG, OR, 1.7)
+    with gf.GaugeFixer(*dims, precision=prec, recon=recon, n_copies=2) as fx:
+        for c, L in enumerate(Ls):
+            fx.set_links_copy(c, L)
+        lit = fx.measure_mag_eq16()
+        F, th = fx.measure_batch(MAG)
+    rel = 1e-12 if prec == DP else 2e-5
+    for c, L in enumerate(Ls):
+        m = oracle.measure(L, MAG)
+        assert lit[c] == pytest.approx(m["theta_literal"], rel=rel) and th[c] == pytest.approx(m["theta"], rel=rel)
+        assert 0 < lit[c] <= 3 * th[c] and abs(lit[c] - th[c]) > 1e-3 * th[c]      # the two really differ
+    with gf.GaugeFixer(4, 4, 4, 4, su2=True) as fx2:
+        fx2.set_links(np.zeros(fx2.shape))
+        with pytest.raises(gf.GfError) as e:
+            fx2.measure_mag_eq16()
+        assert e.value.code == gf.GF_ESTATE
+
+
 @pytest.mark.parametrize("prec,recon", [(DP, 18), (SP, 18), (SP, 12)])
 def test_reunitarize_matches_oracle(gf, oracle, prec, recon):
     dims = (4, 4, 4, 6)
