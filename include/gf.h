@@ -338,6 +338,9 @@ int gf_random_gauge(gf_ctx* ctx, uint64_t seed);
  * (Kennedy-Pendleton / Creutz sampler of GF_SA at T = 3/beta).  Philox counter (site, 4 * sweep + mu,
  * sub | purpose << 8, trial), key seed + copy, sweeps first_sweep_index .. first_sweep_index + n_sweeps - 1.
  * The result is a new configuration, so a tracked transform restarts at the identity.  Asynchronous.
+ * On contexts with recon = 12 the links are reprojected onto SU(3) after every 16th sweep of the call (as in gf_anneal),
+ * on other float contexts after every 100th.  On SP contexts the heatbath arithmetic is float with
+ * guard-banded accept decisions, as in GF_SA sweeps.
  * On SU(2) contexts the same with the single subgroup and the weight exp((beta/2) Re tr[U A]) (T = 2/beta).
  * gf_plaquette: plaq[n_copies] receives <Re tr U_P> / N_c over the 6 V plaquettes (gauge invariant under
  * Eq. (1): it does not change under any sweep of this library).  Synchronous.

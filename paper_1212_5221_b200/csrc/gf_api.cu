@@ -1462,6 +1462,13 @@ int gf_wilson_heatbath(gf_ctx* ctx, double beta, uint64_t seed, uint32_t first_s
                     DISPATCH_RR(ctx, WILSON_HB, mu, par, first_sweep_index + (uint32_t)k);
                 CU(cudaGetLastError());
                 ++ctx->launches;
+                if (mu == 3 && par == 1 && ((ctx->recon == 12 && (k + 1) % GF_RECON12_REUNIT == 0) ||
+                                            (ctx->recon != 12 && ctx->real_bytes == 4 && (k + 1) % 100 == 0))) {
+                    // 12-real storage under heatbath rotations: reproject as the annealing schedules do;
+                    // float links otherwise: every 100 sweeps
+                    int rc = gf_reunitarize(ctx);
+                    if (rc) return rc;
+                }
             }
     // a new configuration, not a gauge transform of the old one: the accumulated g(x) restarts
     for (int c = 0; c < ctx->B && ctx->gtot; ++c) {

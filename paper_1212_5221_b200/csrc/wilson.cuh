@@ -46,15 +46,17 @@ GF_DEV int64_t cb_shift(const Dims& d, const SiteCoord& s, int mu, int dmu, int 
     return ((((int64_t)c[0] * d.Nx + c[1]) * d.Ny + c[2]) * d.Nz + c[3]) >> 1;
 }
 
+// the heatbath runs in the storage type, as in the half-sweep kernel (step1.cuh: float with guard-banded decisions on
+// SP contexts, double on DP contexts)
 template <int I, int J, int S, class R>
-GF_DEV void wilson_subgroup(Mat<R>& W, Mat<R>& U, double T, uint64_t seed, uint32_t site, uint32_t sweep) {
-    double a[4], gd[4];
-    a[0] = (double)W.v[RE(I, I)] + (double)W.v[RE(J, J)];
-    a[3] = (double)W.v[IM(I, I)] - (double)W.v[IM(J, J)];
-    a[2] = (double)W.v[RE(I, J)] - (double)W.v[RE(J, I)];
-    a[1] = (double)W.v[IM(I, J)] + (double)W.v[IM(J, I)];
-    rule_heatbath_landau(a, T, seed, site, sweep, S, gd);
-    const R g[4] = {(R)gd[0], (R)gd[1], (R)gd[2], (R)gd[3]};
+GF_DEV void wilson_subgroup(Mat<R>& W, Mat<R>& U, double T, uint64_t seed, uint32_t site, uint32_t sweep,
+                            const HbDraw<R>& pre) {
+    R a[4], g[4];
+    a[0] = W.v[RE(I, I)] + W.v[RE(J, J)];
+    a[3] = W.v[IM(I, I)] - W.v[IM(J, J)];
+    a[2] = W.v[RE(I, J)] - W.v[RE(J, I)];
+    a[1] = W.v[IM(I, J)] + W.v[IM(J, I)];
+    hb_finish_landau<R>(a, (R)T, pre, seed, site, sweep, S, g);
     sub_left<I, J>(W, g);
     sub_left<I, J>(U, g);
 }
@@ -89,8 +91,15 @@ __global__ void __launch_bounds__(128, GF_HB_MIN_CTAS) wilson_heatbath_kernel(ch
     const uint32_t site = (uint32_t)(((t * d.Nx + x) * d.Ny + y) * d.Nz + s.c[3]);
     const int q = 1 - parity;   // parity of the sites one step away
 
+    const double T = 3.0 / beta;
+    const uint64_t seed = seed0 + (uint64_t)copy;
+    const uint32_t sw = 4u * sweep_index + (uint32_t)mu;
     Mat<R> U, A;
     global_get<R, RECON>(links + L::link_offset(parity, mu, Vh), Vh, cb, U);
+    // the link-independent part of the three heatbath draws (step1.cuh) while the first loads are in flight
+    HbDraw<R> pre[3];
+#pragma unroll 1
+    for (int k = 0; k < 3; ++k) hb_draws_landau<R>(seed, site, sw, k, pre[k]);
     set_zero(A);
     const int64_t cb_mu = cb_shift(d, s, mu, +1, mu, 0);
 #pragma unroll 1
@@ -117,12 +126,9 @@ __global__ void __launch_bounds__(128, GF_HB_MIN_CTAS) wilson_heatbath_kernel(ch
     }
     Mat<R> W;
     mul_left<3>(U, A, W);
-    const double T = 3.0 / beta;
-    const uint64_t seed = seed0 + (uint64_t)copy;
-    const uint32_t sw = 4u * sweep_index + (uint32_t)mu;
-    wilson_subgroup<0, 1, 0>(W, U, T, seed, site, sw);
-    wilson_subgroup<0, 2, 1>(W, U, T, seed, site, sw);
-    wilson_subgroup<1, 2, 2>(W, U, T, seed, site, sw);
+    wilson_subgroup<0, 1, 0>(W, U, T, seed, site, sw, pre[0]);
+    wilson_subgroup<0, 2, 1>(W, U, T, seed, site, sw, pre[1]);
+    wilson_subgroup<1, 2, 2>(W, U, T, seed, site, sw, pre[2]);
     if (active) global_put<R, RECON>(links + L::link_offset(parity, mu, Vh), Vh, cb, U);
 }
 
@@ -196,6 +202,8 @@ __global__ void __launch_bounds__(128) wilson_heatbath2_kernel(char* links_all, 
     const int q = 1 - parity;
     Quat<R> U, a, b, c;
     global_get_q(links + L::link_offset(parity, mu, Vh), Vh, cb, U);
+    HbDraw<R> pre;   // the link-independent part of the heatbath draw while the loads are in flight
+    hb_draws_landau<R>(seed0 + (uint64_t)copy, site, 4u * sweep_index + (uint32_t)mu, 0, pre);
     R A[4] = {R(0), R(0), R(0), R(0)};
     const int64_t cb_mu = cb_shift(d, s, mu, +1, mu, 0);
 #pragma unroll 1
@@ -219,12 +227,9 @@ __global__ void __launch_bounds__(128) wilson_heatbath2_kernel(char* links_all, 
 #pragma unroll
     for (int k = 0; k < 4; ++k) Aq.v[k] = A[k];
     const Quat<R> W = qmul(U, Aq);                                   // the product is bilinear: A need not be unit
-    const double aw[4] = {2.0 * (double)W.v[0], 2.0 * (double)W.v[1], 2.0 * (double)W.v[2], 2.0 * (double)W.v[3]};
-    double gd[4];
-    rule_heatbath_landau(aw, 2.0 / beta, seed0 + (uint64_t)copy, site, 4u * sweep_index + (uint32_t)mu, 0, gd);
+    const R aw[4] = {R(2) * W.v[0], R(2) * W.v[1], R(2) * W.v[2], R(2) * W.v[3]};
     Quat<R> g;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) g.v[k] = (R)gd[k];
+    hb_finish_landau<R>(aw, (R)(2.0 / beta), pre, seed0 + (uint64_t)copy, site, 4u * sweep_index + (uint32_t)mu, 0, g.v);
     if (active) global_put_q(links + L::link_offset(parity, mu, Vh), Vh, cb, qmul(g, U));
 }
 
