@@ -137,7 +137,7 @@ __global__ void reunit_kernel(char* base, int64_t Vh, int nslots, int64_t copy_b
 }
 
 // ---- F and theta ---------------------------------------------------------------------------
-// grid = (ceil(Vsh / block), ncopies*Nt, 2): one thread per site of parity blockIdx.z in (gauge copy,
+// grid = (2 * ceil(Vsh / block), ncopies*Nt): one thread per site of parity blockIdx.x & 1 in (gauge copy,
 // time-slice) blockIdx.y.  Each block writes one (F-term, theta-term) pair; slice_reduce_kernel sums them in a
 // fixed order, so results are bit-reproducible.  All arithmetic in double (BASELINE.json).
 GF_DEV double warp_sum(double v) {
@@ -176,9 +176,13 @@ __global__ void measure_kernel(const char* links, Dims d, double* partial, int64
     const int Vsh = d.Nx * d.Ny * Nzh;
     const int64_t Vh = (int64_t)d.Nt * Vsh;
     const int copy = blockIdx.y / d.Nt;
-    const int t = blockIdx.y - copy * d.Nt, par = blockIdx.z;
+    // both parities of a tile in neighbouring CTAs (blockIdx.x = 2 tile + parity): a link is read once as the up link
+    // of its origin and once as the down link of its end point, and the second read then is an L2 hit unless the two
+    // sites are a whole time-slice apart
+    const int t = blockIdx.y - copy * d.Nt, par = (int)(blockIdx.x & 1u);
+    const int bx = (int)(blockIdx.x >> 1), gx = (int)(gridDim.x >> 1);
     links += copy * copy_bytes;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = bx * blockDim.x + threadIdx.x;
     double f_term = 0.0, th_term = 0.0;
     if (i < Vsh) {
         const int cb = t * Vsh + i;
@@ -249,7 +253,7 @@ __global__ void measure_kernel(const char* links, Dims d, double* partial, int64
     }
     block_sum2(f_term, th_term);
     if (threadIdx.x == 0) {
-        const int64_t b = ((int64_t)(blockIdx.y * 2 + par)) * gridDim.x + blockIdx.x;
+        const int64_t b = ((int64_t)(blockIdx.y * 2 + par)) * gx + bx;
         partial[2 * b] = f_term;
         partial[2 * b + 1] = th_term;
     }

@@ -88,9 +88,13 @@ __global__ void measure2_kernel(const char* links, Dims d, double* partial, int6
     const int Vsh = d.Nx * d.Ny * Nzh;
     const int64_t Vh = (int64_t)d.Nt * Vsh;
     const int copy = blockIdx.y / d.Nt;
-    const int t = blockIdx.y - copy * d.Nt, par = blockIdx.z;
+    // both parities of a tile in neighbouring CTAs (blockIdx.x = 2 tile + parity): a link is read once as the up link
+    // of its origin and once as the down link of its end point, and the second read then is an L2 hit unless the two
+    // sites are a whole time-slice apart
+    const int t = blockIdx.y - copy * d.Nt, par = (int)(blockIdx.x & 1u);
+    const int bx = (int)(blockIdx.x >> 1), gx = (int)(gridDim.x >> 1);
     links += copy * copy_bytes;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = bx * blockDim.x + threadIdx.x;
     double f_term = 0.0, th_term = 0.0;
     if (i < Vsh) {
         const int64_t cb = (int64_t)t * Vsh + i;
@@ -123,7 +127,7 @@ __global__ void measure2_kernel(const char* links, Dims d, double* partial, int6
     }
     block_sum2(f_term, th_term);
     if (threadIdx.x == 0) {
-        const int64_t b = ((int64_t)(blockIdx.y * 2 + par)) * gridDim.x + blockIdx.x;
+        const int64_t b = ((int64_t)(blockIdx.y * 2 + par)) * gx + bx;
         partial[2 * b] = f_term;
         partial[2 * b + 1] = th_term;
     }

@@ -773,7 +773,7 @@ int gf_sweep(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint
 // ---- reductions --------------------------------------------------------------------------------
 #define MEASURE(R, RECON, gauge_)                                                                          \
     do {                                                                                                   \
-        dim3 grid((unsigned)ctx->meas_gx, (unsigned)ctx->NS, 2);                                           \
+        dim3 grid((unsigned)(2 * ctx->meas_gx), (unsigned)ctx->NS);                                        \
         const int64_t cb_ = link_store_bytes(ctx);                                                         \
         if ((gauge_) == GF_LANDAU)                                                                         \
             measure_kernel<R, RECON, GAUGE_LANDAU><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_, shard_dn(ctx), eq16_); \
@@ -786,7 +786,7 @@ int gf_sweep(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, uint
 // enqueue the reduction and the copy of the 2*Nt slice sums to pinned host memory
 #define MEASURE2(R, gauge_)                                                                                \
     do {                                                                                                   \
-        dim3 grid((unsigned)ctx->meas_gx, (unsigned)ctx->NS, 2);                                           \
+        dim3 grid((unsigned)(2 * ctx->meas_gx), (unsigned)ctx->NS);                                        \
         const int64_t cb_ = link_store_bytes(ctx);                                                         \
         if ((gauge_) == GF_LANDAU)                                                                         \
             measure2_kernel<R, GAUGE_LANDAU><<<grid, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, cb_); \
