@@ -294,8 +294,9 @@ int gf_fix(gf_ctx* ctx, const gf_fix_params* params, gf_result* out);
  * whole lattice; gf_get_slice_sweeps has Nt_global entries; gf_unitarity covers the shard's own links;
  * gf_random_gauge, gf_wilson_heatbath and gf_plaquette return GF_ESTATE.  Sweeps and reductions return GF_ESTATE
  * until the neighbours are attached.  A single shard spanning the lattice attaches to itself.
- * Multi-device operation (peer / IPC mappings) is written and guarded but was not run on hardware in this build
- * (one GPU available); the tests drive 2 and 4 shards on one device and compare with the unsharded context bit for bit.
+ * The tests drive 2 and 4 shards on one device — threads of one process, and two processes with IPC-mapped stores —
+ * and compare with the unsharded context bit for bit; mappings of ANOTHER device's memory were not run in this build
+ * (one GPU available).
  */
 int gf_create_shard(gf_ctx** out, int Nx, int Ny, int Nz, int Nt_local, int t0, int Nt_global, int precision, int recon,
                     unsigned flags, void* cuda_stream);

@@ -221,3 +221,71 @@ def test_shard_argument_checks(gf):
     finally:
         a.close()
         b.close()
+
+
+# ---- one process per shard: CUDA IPC mappings and the torch.distributed communicator (gloo), on ONE device ----------
+# (NCCL refuses two ranks on one GPU, so the barrier here is the gloo one — stream synchronisation + host barrier; no
+# kernel of a rank ever waits for another rank.  What this adds to the thread tests: gf_shard_export / gf_shard_attach_ipc,
+# the neighbour's store reached through an IPC mapping by the half-sweep and measure kernels, TorchDistComm.)
+def _ipc_worker(rank, world, port, dims, q):
+    import os
+    import sys
+    os.environ.update({"RANK": str(rank), "WORLD_SIZE": str(world), "LOCAL_RANK": "0",
+                       "MASTER_ADDR": "127.0.0.1", "MASTER_PORT": str(port)})
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    if root not in sys.path:
+        sys.path.insert(0, root)
+    import datetime
+    import torch
+    import torch.distributed as dist
+    from paper_1212_5221_b200 import gf, shards
+    torch.cuda.set_device(0)
+    dist.init_process_group("gloo", rank=rank, world_size=world, timeout=datetime.timedelta(seconds=120))
+    try:
+        Nx, Ny, Nz, Nt = dims
+        L = config(dims, DP, seed=351)
+        stream = torch.cuda.Stream()
+        fx, comm, (t0, n) = shards.make_rank_shard(dist, torch.device("cuda", 0), stream, Nx, Ny, Nz, Nt,
+                                                   precision=DP, recon=18, track_transform=True)
+        fx.set_links(np.ascontiguousarray(L[t0:t0 + n]))
+        r = fx.run(LANDAU, OR, 1.7, max_sweeps=12, eps=-1.0, check_every=4, history=True)
+        nxt = fx.anneal(MAG, 0.9, 0.2, 3, 1, seed=5, first_sweep_index=12)
+        rc = fx.run(COULOMB, OR, 1.7, max_sweeps=6, eps=-1.0, check_every=6)
+        out = (rank, t0, r["history"], nxt, rc["F"], rc["theta"], fx.get_links(), fx.get_gauge_transform(), dict(comm.calls))
+        dist.barrier()          # nobody unmaps a store a neighbour may still be reading
+        fx.close()
+        q.put(out)
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_processes_with_ipc_mapped_stores_bit_for_bit(gf):
+    import socket
+    import torch.multiprocessing as mp
+    dims = (8, 8, 8, 16)
+    L = config(dims, DP, seed=351)
+
+    def body(fx):
+        r = fx.run(LANDAU, OR, 1.7, max_sweeps=12, eps=-1.0, check_every=4, history=True)
+        nxt = fx.anneal(MAG, 0.9, 0.2, 3, 1, seed=5, first_sweep_index=12)
+        rc = fx.run(COULOMB, OR, 1.7, max_sweeps=6, eps=-1.0, check_every=6)
+        return r["history"], nxt, rc["F"], rc["theta"], fx.get_links(), fx.get_gauge_transform()
+
+    ref = run_unsharded(gf, dims, L, body, precision=DP, recon=18, track_transform=True)
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_ipc_worker, args=(r, 2, port, dims, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = sorted((q.get(timeout=300) for _ in procs), key=lambda g: g[0])
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    for g in got:
+        assert np.array_equal(g[2], ref[0]) and g[3] == ref[1] and g[4] == ref[2] and g[5] == ref[3]
+        assert g[8]["barrier"] > 30 and g[8]["allreduce"] >= 4
+    assert np.array_equal(join_t([g[6] for g in got]), ref[4])
+    assert np.array_equal(join_t([g[7] for g in got]), ref[5])
