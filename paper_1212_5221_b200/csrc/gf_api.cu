@@ -71,6 +71,7 @@ struct gf_ctx {
     size_t staging_bytes;
     int64_t device_bytes;
     int block_override;     // 0 = default CTA size
+    int block_auto;         // the default: the largest CTA size that still gives every SM a few CTAs (auto_block)
     int pdl;                // half-sweeps launched with programmatic stream serialization (default 1)
     // kernel timing (gf_kernel_timing)
     bool timing;
@@ -95,6 +96,21 @@ struct gf_ctx {
     std::vector<void*> ipc_opened;   // mappings opened by gf_shard_attach_ipc
     char err[512];
 };
+
+// CTA size of the half-sweep kernels when the caller sets none.  Large lattices: the largest (128 threads for float
+// storage, 64 for double).  A lattice whose half-sweep is only a few hundred CTAs of that size leaves SMs idle or with
+// one CTA where another has two (16^4 SP-12: 256 CTAs on 148 SMs): halve the CTA while the half-sweep has fewer than
+// 512 of them (measured, us per half-sweep, 128 / 64 / 32 threads: 12^4 SP-12 7.1 / 4.8 / 3.9, 16^4 SP-12 7.6 / 5.4 / 6.4,
+// 16^4 MP-12 9.1 / 6.1 / 8.0, 12^4 DP-18 - / 8.7 / 6.4, 20^4 and larger: the largest is best).  Counted on the WHOLE
+// lattice (all copies, all time-slices of all t-shards), so a shard makes the choice of the unsharded context and its
+// fused partial sums keep their order.
+static int auto_block(const gf_ctx* c) {
+    const int maxb = (c->nc == 2 || c->real_bytes == 4) ? 128 : 64;
+    const int64_t Vsh = (int64_t)c->Nx * c->Ny * (c->Nz / 2), units = (int64_t)c->B * c->NtG;
+    int b = maxb;
+    while (b > 32 && ((Vsh + b - 1) / b) * units < 512) b >>= 1;
+    return b;
+}
 
 static int fail(gf_ctx* c, int code, const char* fmt, ...) {
     if (c) {
@@ -214,6 +230,7 @@ static int create_impl(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int n_copie
     ctx->links_dn = nullptr; ctx->Vh_dn = ctx->Vh; ctx->Nt_dn = Nt;
     ctx->gtot_up = ctx->gapp_up = nullptr; ctx->Vh_up = ctx->Vh;
     ctx->attached = !ctx->sharded;
+    ctx->block_auto = auto_block(ctx);
     ctx->have_comm = false;
     memset(&ctx->comm, 0, sizeof(ctx->comm));
 
@@ -689,7 +706,7 @@ static int launch_half(gf_ctx* ctx, int gauge, int algo, double param, uint64_t 
         CU(cudaEventRecord(e0, ctx->stream));
     }
     cudaError_t e;
-    const int blk = ctx->block_override;
+    const int blk = ctx->block_override ? ctx->block_override : ctx->block_auto;
     if (ctx->nc == 2) {
         e = (ctx->precision == GF_DP)   ? launch_sweep_su2<double, double>(a, gauge, track, blk, ctx->stream)
             : (ctx->precision == GF_MP) ? launch_sweep_su2<float, double>(a, gauge, track, blk, ctx->stream)
@@ -975,9 +992,10 @@ static const int GF_RECON12_REUNIT = 16;
 
 static int sweep_gx(const gf_ctx* ctx) {
     const int Vsh = ctx->Nx * ctx->Ny * (ctx->Nz / 2);
-    const int block = (ctx->nc == 2)           ? sweep_su2_block(Vsh, ctx->block_override)
-                      : (ctx->real_bytes == 4) ? sweep_block<float>(Vsh, ctx->block_override)
-                                               : sweep_block<double>(Vsh, ctx->block_override);
+    const int blk = ctx->block_override ? ctx->block_override : ctx->block_auto;
+    const int block = (ctx->nc == 2)           ? sweep_su2_block(Vsh, blk)
+                      : (ctx->real_bytes == 4) ? sweep_block<float>(Vsh, blk)
+                                               : sweep_block<double>(Vsh, blk);
     return (Vsh + block - 1) / block;
 }
 
