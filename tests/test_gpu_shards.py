@@ -289,3 +289,27 @@ def test_two_processes_with_ipc_mapped_stores_bit_for_bit(gf):
         assert g[8]["barrier"] > 30 and g[8]["allreduce"] >= 4
     assert np.array_equal(join_t([g[6] for g in got]), ref[4])
     assert np.array_equal(join_t([g[7] for g in got]), ref[5])
+
+
+@pytest.mark.parametrize("n_shards", [2, 4])
+def test_recipe_and_lagged_stop_on_shards_bit_for_bit(gf, n_shards):
+    # gf_fix (SA -> SR -> OR with per-stage bookkeeping per global slice) and GF_FLAG_LAGGED_STOP (decision from the even
+    # half-sweep's partial sums, summed over the shards) on t-shards
+    dims = (8, 8, 8, 16)
+    L = config(dims, DP, seed=361)
+    kw = dict(precision=DP, recon=12, lagged_stop=True)
+
+    def body(fx):
+        f = fx.fix(MAG, seed=3, sa_steps=5, sa_T_hi=1.0, sa_T_lo=0.1, sa_micro=2, sr_max_sweeps=10, sr_p=0.5, or_omega=1.7,
+                   or_max_sweeps=60, eps=1e-9, check_every=2)
+        r = fx.run(LANDAU, OR, 1.7, max_sweeps=2500, eps=1e-7, check_every=1, reunit_every=200, history=True)
+        return f, r, fx.get_links()
+
+    ref = run_unsharded(gf, dims, L, body, **kw)
+    got = run_sharded(gf, dims, L, n_shards, body, **kw)
+    assert ref[1]["converged"] and ref[1]["sweeps"] < 2500
+    for g in got:
+        assert g[0] == ref[0]
+        assert g[1]["sweeps"] == ref[1]["sweeps"] and g[1]["F"] == ref[1]["F"] and g[1]["theta"] == ref[1]["theta"]
+        assert np.array_equal(g[1]["history"], ref[1]["history"])
+    assert np.array_equal(join_t([g[2] for g in got]), ref[2])
