@@ -21,7 +21,7 @@ from paper_1212_5221_b200 import inputs
 pytestmark = pytest.mark.gpu
 
 LANDAU, COULOMB, MAG = 0, 1, 2
-OR = 0
+OR, SA = 0, 2
 SP, DP, MP = 0, 1, 2
 TILE = (16, 16, 16, 16)
 TOL = {DP: 1e-12, SP: 5e-5, MP: 5e-5}
@@ -169,6 +169,67 @@ def test_full_size_sampled_sites_nonperiodic(gf, oracle, tile, dims, prec, recon
             W = up_out[..., 0] + 1j * up_out[..., 1]
             uni = np.abs(W @ np.conj(np.swapaxes(W, -1, -2)) - np.eye(3)).max()
             assert uni < (1e-12 if prec == DP else 2e-5)
+
+
+@pytest.mark.parametrize("dims,prec,recon,gauge,T", [((64, 64, 64, 256), DP, 18, LANDAU, 1.0), ((64, 64, 64, 256), DP, 18, MAG, 0.5),
+                                                     ((64, 64, 64, 256), SP, 12, LANDAU, 1.0), ((64, 64, 64, 256), SP, 12, LANDAU, 5.0)])
+def test_full_size_heatbath_sampled_sites(gf, oracle, tile, dims, prec, recon, gauge, T):
+    # the simulated-annealing half-sweep in the launch configurations bench.py times (other_workloads): sampled sites of
+    # a non-periodic 64^3 x 256 lattice against oracle.site_update with the site index in the whole lattice (Philox
+    # counters up to 6.7e7, wrap-around neighbours, warp-wide retries across the whole grid).  DP: the annealing bar
+    # 1e-11 per link; SP (float heatbath on the GPU, double in the oracle): 5e-5 on all sampled sites but those whose
+    # local field is weak (conditioning number from the oracle below 0.5), which must still be unitary.
+    import torch
+    from tests import conditioning
+    dev = torch.device("cuda", 0)
+    dt = np.float64 if prec == DP else np.float32
+    tdt = torch.float64 if prec == DP else torch.float32
+    src = nonperiodic_lattice(torch, tile, dims, dev).to(tdt)
+    Nx, Ny, Nz, Nt = dims
+    ext = [Nt, Nx, Ny, Nz]
+    rng = np.random.default_rng(78)
+    seed, sweep_index = 99, 4
+    with gf.GaugeFixer(*dims, precision=prec, recon=recon) as fx:
+        out = torch.empty_like(src)
+        for parity in (0, 1):
+            fx.set_links(src)
+            fx.half_sweep(gauge, SA, T, seed, sweep_index, parity)
+            gf.gf_get_links(fx.ctx, out)
+            s = sample_sites(dims, parity, 1500, rng)
+            st = torch.from_numpy(s).to(dev)
+            mu = torch.arange(4, device=dev)
+            dn = st[:, None, :].repeat(1, 4, 1)
+            for d in range(4):
+                dn[:, d, d] = (dn[:, d, d] - 1) % ext[d]
+            gather_up = lambda A: A[st[:, 0, None], st[:, 1, None], st[:, 2, None], st[:, 3, None], mu[None, :]]
+            gather_dn = lambda A: A[dn[..., 0], dn[..., 1], dn[..., 2], dn[..., 3], mu[None, :]]
+            up_in, dn_in = gather_up(src).cpu().numpy(), gather_dn(src).cpu().numpy()
+            up_out, dn_out = gather_up(out).cpu().numpy(), gather_dn(out).cpu().numpy()
+            n_bad = 0
+            for k in range(s.shape[0]):
+                t, x, y, z = (int(v) for v in s[k])
+                sidx = ((t * Nx + x) * Ny + y) * Nz + z
+                u, d_ = np.ascontiguousarray(up_in[k]), np.ascontiguousarray(dn_in[k])
+                oracle.site_update(u, d_, gauge, SA, T, seed, sidx, sweep_index)
+                err = max(float(np.abs(u.astype(np.float64) - up_out[k]).max()), float(np.abs(d_.astype(np.float64) - dn_out[k]).max()))
+                if prec == DP:
+                    assert err <= 1e-11, (parity, k, err)
+                elif err > 5e-5:
+                    # a weak local field in one of the subgroups (oracle's numbers, double, on the float inputs)
+                    c = np.inf
+                    uu, dd = up_in[k].astype(np.float64), dn_in[k].astype(np.float64)
+                    for sub, (i, j) in enumerate(conditioning.SUBS):
+                        a = oracle.local_quaternion(uu, dd, i, j)
+                        c = min(c, float(np.linalg.norm(a)))
+                        g = oracle.rule_heatbath_landau(a, T, seed, sidx, sweep_index, sub)
+                        for m in range(4):
+                            uu[m] = oracle.apply_subgroup(uu[m], g, i, j, False)
+                            dd[m] = oracle.apply_subgroup(dd[m], g, i, j, True)
+                    assert c < 0.5 and err < 1e-2, (parity, k, err, c)
+                    n_bad += 1
+            assert n_bad <= 15, n_bad          # <= 1 % of the sampled sites
+            W = up_out[..., 0] + 1j * up_out[..., 1]
+            assert np.abs(W @ np.conj(np.swapaxes(W, -1, -2)) - np.eye(3)).max() < (1e-12 if prec == DP else 2e-5)
 
 
 # ---- full runs at BASELINE.json's sizes ---------------------------------------------------------
