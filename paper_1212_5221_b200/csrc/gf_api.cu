@@ -990,12 +990,15 @@ int gf_coulomb_finalize(gf_ctx* ctx) {
 // often (see the comment above anneal_impl and DESIGN.md §7)
 static const int GF_RECON12_REUNIT = 16;
 
-static int sweep_gx(const gf_ctx* ctx) {
+// CTAs per (copy, time-slice) of a half-sweep with the rule `algo` (the stochastic float kernels use smaller CTAs)
+static int sweep_gx(const gf_ctx* ctx, int algo) {
     const int Vsh = ctx->Nx * ctx->Ny * (ctx->Nz / 2);
     const int blk = ctx->block_override ? ctx->block_override : ctx->block_auto;
-    const int block = (ctx->nc == 2)           ? sweep_su2_block(Vsh, blk)
-                      : (ctx->real_bytes == 4) ? sweep_block<float>(Vsh, blk)
-                                               : sweep_block<double>(Vsh, blk);
+    const bool stoch = (algo == GF_SR || algo == GF_SA);
+    const int block = (ctx->nc == 2)              ? sweep_su2_block(Vsh, blk)
+                      : (ctx->precision == GF_SP) ? sweep_block<float, float>(Vsh, blk, stoch)
+                      : (ctx->precision == GF_MP) ? sweep_block<float, double>(Vsh, blk, stoch)
+                                                  : sweep_block<double, double>(Vsh, blk, stoch);
     return (Vsh + block - 1) / block;
 }
 
@@ -1050,7 +1053,7 @@ static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t see
     // otherwise NSG = NS = B * Nt); kernels and device arrays are per local slice
     const int Nt = ctx->NtG, B = ctx->B, NS = ctx->NSG, NSloc = ctx->NS, goff = ctx->t0;
     const int nunits = per_slice ? NS : B, uspan = per_slice ? 1 : Nt;   // unit u = slices [u*uspan, (u+1)*uspan)
-    const int gx = sweep_gx(ctx);
+    const int gx = sweep_gx(ctx, algo);
     const double Vs = (double)ctx->Nx * ctx->Ny * ctx->Nz;
     const double ncd = (double)ctx->nc;
     bool have_exact = false;

@@ -267,14 +267,26 @@ GF_DEV double warp_sum_d(double v) {
 #ifndef GF_MIN_CTAS_MP
 #define GF_MIN_CTAS_MP 4
 #endif
+#ifndef GF_SP_STOCH_BLOCK
+#define GF_SP_STOCH_BLOCK 64    // CTA size of the float kernels with a stochastic rule
+#endif
+#ifndef GF_SP_STOCH_MIN_CTAS
+#define GF_SP_STOCH_MIN_CTAS 9
+#endif
 template <class R, class A = R>
 struct SweepLaunch {   // CTA shape per storage type
     static constexpr int MAX_BLOCK = sizeof(R) == 4 ? GF_SP_BLOCK : 64;
     static constexpr int MIN_CTAS = (sizeof(R) == 4 && sizeof(A) == 8) ? GF_MIN_CTAS_MP : (sizeof(R) == 4 ? GF_SP_MIN_CTAS : 3);
+    // The float kernels with a stochastic rule are bound by arithmetic latency, not by HBM: more warps in flight pay.
+    // The shared-memory slice is laid out for the largest CTA of the instantiation, so a 64-thread maximum halves it
+    // (SP-12 Landau: 24.6 KB) and 9 CTAs = 18 warps fit an SM where four 128-thread CTAs gave 16.
+    __host__ __device__ static constexpr bool small_cta(bool stoch) { return stoch && sizeof(R) == 4 && sizeof(A) == 4; }
+    __host__ __device__ static constexpr int max_block(bool stoch) { return small_cta(stoch) ? GF_SP_STOCH_BLOCK : MAX_BLOCK; }
+    __host__ __device__ static constexpr int min_ctas(bool stoch) { return small_cta(stoch) ? GF_SP_STOCH_MIN_CTAS : MIN_CTAS; }
 };
 
 template <class R, class A, int RECON, int GAUGE, bool STOCH, bool TRACK, bool RED>
-__global__ void __launch_bounds__(SweepLaunch<R, A>::MAX_BLOCK, SweepLaunch<R, A>::MIN_CTAS)
+__global__ void __launch_bounds__(SweepLaunch<R, A>::max_block(STOCH), SweepLaunch<R, A>::min_ctas(STOCH))
 sweep_kernel(const SweepArgs args) {
     typedef Layout<R, RECON> L;
     constexpr int MU0 = (GAUGE == GAUGE_COULOMB) ? 1 : 0;
@@ -327,7 +339,7 @@ sweep_kernel(const SweepArgs args) {
     // ---- a2: stream the 2d links into this thread's shared-memory slice ----
     // slice layout [link][chunk][NTHR] x 16 bytes (+ [link][NTHR] x 8 bytes of SP-18 tails); pointers step
     // by one chunk plane (16 Vh bytes) and one link array (LINK_BYTES Vh bytes)
-    constexpr int NTHR = SweepLaunch<R, A>::MAX_BLOCK;
+    constexpr int NTHR = SweepLaunch<R, A>::max_block(STOCH);
     const int tid = threadIdx.x;
     const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem) + (uint32_t)tid * 16;
     const int64_t plane = 16 * Vh;
@@ -465,10 +477,11 @@ sweep_kernel(const SweepArgs args) {
 }
 
 // CTA size actually used for a slice of Vsh sites per parity (block_override = 0: default)
-template <class R>
-inline int sweep_block(int Vsh, int block_override) {
+template <class R, class A = R>
+inline int sweep_block(int Vsh, int block_override, bool stoch = false) {
     int block = block_override;
-    if (block <= 0 || block > SweepLaunch<R>::MAX_BLOCK) block = SweepLaunch<R>::MAX_BLOCK;
+    const int maxb = SweepLaunch<R, A>::max_block(stoch);
+    if (block <= 0 || block > maxb) block = maxb;
     const int need = ((Vsh + 31) / 32) * 32;
     return block < need ? block : need;
 }

@@ -13,9 +13,9 @@ static cudaError_t launch_one(const SweepArgs& args, int block, cudaStream_t str
     constexpr int ND = (GAUGE == GAUGE_COULOMB) ? 3 : 4;
     auto kern = sweep_kernel<R, A, RECON, GAUGE, STOCH, TRACK, RED>;
     const int Vsh = args.Nx * args.Ny * (args.Nz / 2);
-    block = sweep_block<R>(Vsh, block);
-    // the slice stride is the maximal CTA size whatever the block (sweep.cuh, smem_get)
-    const size_t smem = (size_t)SweepLaunch<R, A>::MAX_BLOCK * 2 * ND * Layout<R, RECON>::LINK_BYTES;
+    block = sweep_block<R, A>(Vsh, block, STOCH);
+    // the slice stride is the maximal CTA size of the instantiation whatever the block (sweep.cuh, smem_get)
+    const size_t smem = (size_t)SweepLaunch<R, A>::max_block(STOCH) * 2 * ND * Layout<R, RECON>::LINK_BYTES;
     // function attributes are per device: remember what was set for this instantiation on each device.  Contexts may
     // be driven from several host threads (one thread per context, gf.h): the cache is atomic, and setting the same
     // attribute twice is harmless.
