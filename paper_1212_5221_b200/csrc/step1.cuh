@@ -175,7 +175,7 @@ GF_DEV void hb_draws_landau(uint64_t seed, uint32_t site, uint32_t sweep, int su
         const S l1 = log_u(r1), l3 = log_u(r3);
         d.v[t ? 6 : 0] = l1 + cos2_2pi(r2) * l3;
         d.v[t ? 7 : 1] = r4 * r4;
-        d.v[t ? 8 : 5] = -(l1 + l3);
+        if (sizeof(S) == 4) d.v[t ? 8 : 5] = -(l1 + l3);   // the guard band of the float decisions only
     }
     // cos th = 2 r5 - 1 = r5 - (1 - r5) and sin^2 th = 4 r5 (1 - r5), with 1 - r5 converted from the complemented
     // Philox word: no cancellation near the poles (in float 1 - cos^2 th would lose sin th there)
