@@ -8,6 +8,9 @@
 
 namespace gf {
 
+#define GF_SMEM_PER_SM (228 * 1024)    // shared memory of an sm_100 SM
+#define GF_SMEM_MAX_CTA (226 * 1024)   // the most one CTA asks for here (227 KB less the kernels' static shared memory)
+
 template <class R, class A, int RECON, int GAUGE, bool STOCH, bool TRACK, bool RED>
 static cudaError_t launch_one(const SweepArgs& args, int block, cudaStream_t stream) {
     constexpr int ND = (GAUGE == GAUGE_COULOMB) ? 3 : 4;
@@ -24,14 +27,35 @@ static cudaError_t launch_one(const SweepArgs& args, int block, cudaStream_t str
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     if (dev < 0 || dev >= 64 || smem > smem_set[dev].load(std::memory_order_acquire)) {
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GF_SMEM_MAX_CTA);
         if (e != cudaSuccess) return e;
         e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
         if (e != cudaSuccess) return e;
         if (dev >= 0 && dev < 64) smem_set[dev].store(smem, std::memory_order_release);
     }
     const dim3 grid((unsigned)((Vsh + block - 1) / block), (unsigned)(args.ncopies * args.Nt));
-    return launch_with_pdl(kern, grid, dim3((unsigned)block), smem, stream, args);
+    // A grid of fewer CTAs than the SMs have slots is not spread evenly by the hardware (measured: 512 CTAs of 64
+    // threads with nine slots per SM run 1.5x slower than with four).  Ask for as much shared memory per CTA as leaves
+    // room for ceil(CTAs / SMs) of them on an SM: the CTAs then spread over all SMs.
+    size_t smem_launch = smem;
+    {
+        static std::atomic<int> sms_of[64];
+        int sms = (dev >= 0 && dev < 64) ? sms_of[dev].load(std::memory_order_relaxed) : 0;
+        if (sms <= 0) {
+            e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            if (e != cudaSuccess) return e;
+            if (dev >= 0 && dev < 64) sms_of[dev].store(sms, std::memory_order_relaxed);
+        }
+        const long long ctas = (long long)grid.x * grid.y;
+        const long long per_sm = (ctas + sms - 1) / sms;
+        const size_t budget = (size_t)GF_SMEM_PER_SM / (size_t)(per_sm > 0 ? per_sm : 1);
+        if (per_sm <= 8 && budget > smem + 1024) {
+            smem_launch = ((budget - 1024) / 1024) * 1024;     // 1 KB per CTA is the driver's
+            if (smem_launch > (size_t)GF_SMEM_MAX_CTA) smem_launch = GF_SMEM_MAX_CTA;
+            if (smem_launch < smem) smem_launch = smem;
+        }
+    }
+    return launch_with_pdl(kern, grid, dim3((unsigned)block), smem_launch, stream, args);
 }
 
 template <class R, class A, int RECON, int GAUGE>
