@@ -406,8 +406,8 @@ const char* gf_version(void);
  *   gf_debug_set_pdl(ctx, 0)    half-sweeps are launched without programmatic dependent launch.
  *   gf_debug_set_block(ctx, n)  CTA size of the half-sweep kernel: a multiple of 32, capped at the kernel's maximum (128
  *                               threads for float storage, 64 for double and for the float stochastic rules); 0 = the
- *                               default, which is that maximum, halved while the whole lattice's half-sweep would have
- *                               fewer than 512 CTAs.  Links are bit-identical for every n, fused partial sums differ in
+ *                               default, which is that maximum, or 32 where the whole lattice's half-sweep would not
+ *                               give every SM a CTA.  Links are bit-identical for every n, fused partial sums differ in
  *                               summation order.
  */
 int gf_debug_set_fused(gf_ctx* ctx, int fused);

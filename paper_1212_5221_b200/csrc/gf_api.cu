@@ -97,19 +97,19 @@ struct gf_ctx {
     char err[512];
 };
 
-// CTA size of the half-sweep kernels when the caller sets none.  Large lattices: the largest (128 threads for float
-// storage, 64 for double).  A lattice whose half-sweep is only a few hundred CTAs of that size leaves SMs idle or with
-// one CTA where another has two (16^4 SP-12: 256 CTAs on 148 SMs): halve the CTA while the half-sweep has fewer than
-// 512 of them (measured, us per half-sweep, 128 / 64 / 32 threads: 12^4 SP-12 7.1 / 4.8 / 3.9, 16^4 SP-12 7.6 / 5.4 / 6.4,
-// 16^4 MP-12 9.1 / 6.1 / 8.0, 12^4 DP-18 - / 8.7 / 6.4, 20^4 and larger: the largest is best).  Counted on the WHOLE
-// lattice (all copies, all time-slices of all t-shards), so a shard makes the choice of the unsharded context and its
-// fused partial sums keep their order.
+// CTA size of the half-sweep kernels when the caller sets none: the largest (128 threads for float storage and SU(2),
+// 64 for double), except on lattices so small that a half-sweep of such CTAs would not give every SM one (float) or
+// two (double) of them — then 32 threads.  Measured with the launches spread over all SMs (sweep_inst.cuh), us per
+// half-sweep, largest CTA / 32 threads: 8^4 SP-12 3.5 / 3.3, DP-18 4.7 / 4.4; 12^4 SP-12 3.8 / 3.6, DP-18 7.5 / 6.4;
+// 16^4 SP-12 5.3 / 6.4, SP-18 6.6 / 10.0, DP-18 11.4 / 13.8; larger lattices: the largest CTA by a growing margin.
+// Counted on the WHOLE lattice (all copies, all time-slices of all t-shards), so a shard makes the choice of the
+// unsharded context and its fused partial sums keep their order.
 static int auto_block(const gf_ctx* c) {
-    const int maxb = (c->nc == 2 || c->real_bytes == 4) ? 128 : 64;
+    const bool dbl = c->nc == 3 && c->real_bytes == 8;
+    const int maxb = dbl ? 64 : 128;
     const int64_t Vsh = (int64_t)c->Nx * c->Ny * (c->Nz / 2), units = (int64_t)c->B * c->NtG;
-    int b = maxb;
-    while (b > 32 && ((Vsh + b - 1) / b) * units < 512) b >>= 1;
-    return b;
+    const int64_t ctas = ((Vsh + maxb - 1) / maxb) * units;
+    return ctas < (dbl ? 300 : 148) ? 32 : maxb;
 }
 
 static int fail(gf_ctx* c, int code, const char* fmt, ...) {
