@@ -397,18 +397,11 @@ __global__ void unitarity_reduce_kernel(const double* partial, int nblocks, doub
 // h(x) Haar-distributed on SU(3): two rows of independent complex standard normals (Box-Muller on
 // Philox uniforms, counter = (site, 0, k | 3 << 8, 0), k = 0..2, key = seed + copy), Gram-Schmidt,
 // third row (u x v)^*.  All in double.  One thread per site; field layout [copy][p][chunk][cb].
-template <class R>
-__global__ void haar_field_kernel(char* field, Dims d, uint64_t seed, int64_t copy_bytes) {
-    const int64_t V = (int64_t)d.Nt * d.Nx * d.Ny * d.Nz;
-    const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= V) return;
-    const int copy = blockIdx.y;
-    int par, cb;
-    site_to_cb(d, s, par, cb);
-    Mat<double> h;
+// h of one site: a function of (seed, lexicographic index of the site in the WHOLE lattice) alone
+GF_DEV void haar_su3(uint64_t seed, uint32_t site, Mat<double>& h) {
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        const u32x4 w = rng_draw(seed + (uint64_t)copy, (uint32_t)s, 0u, k, 3, 0u);
+        const u32x4 w = rng_draw(seed, site, 0u, k, 3, 0u);
         const double r0 = sqrt(-2.0 * log(uniform01(w.x))), r1 = sqrt(-2.0 * log(uniform01(w.z)));
         double s0, c0, s1, c1;
         sincos(6.283185307179586477 * uniform01(w.y), &s0, &c0);
@@ -418,6 +411,19 @@ __global__ void haar_field_kernel(char* field, Dims d, uint64_t seed, int64_t co
 #pragma unroll
     for (int k = 12; k < 18; ++k) h.v[k] = 0.0;
     gram_schmidt(h);
+}
+
+// site_off: lexicographic index of this store's first site in the whole lattice (t-shards: t0 Nx Ny Nz; else 0)
+template <class R>
+__global__ void haar_field_kernel(char* field, Dims d, uint64_t seed, int64_t copy_bytes, int64_t site_off) {
+    const int64_t V = (int64_t)d.Nt * d.Nx * d.Ny * d.Nz;
+    const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= V) return;
+    const int copy = blockIdx.y;
+    int par, cb;
+    site_to_cb(d, s, par, cb);
+    Mat<double> h;
+    haar_su3(seed + (uint64_t)copy, (uint32_t)(s + site_off), h);
     Mat<R> o;
 #pragma unroll
     for (int k = 0; k < 18; ++k) o.v[k] = (R)h.v[k];
@@ -426,9 +432,11 @@ __global__ void haar_field_kernel(char* field, Dims d, uint64_t seed, int64_t co
 
 // U_mu(x) <- h(x) U_mu(x) h(x+mu)^dagger (Eq. (1)) and, when tracked, g(x) <- h(x) g(x).
 // One thread per site (parity blockIdx.z, copy blockIdx.y).
+// t-shards: h(x + t_hat) of the last slice belongs to the store above and is recomputed here from its site index
+// (top_site0 >= 0: lexicographic index, in the whole lattice, of the first site of the slice above; -1: not sharded)
 template <class R, int RECON>
 __global__ void gauge_apply_kernel(char* links, char* gtot, const char* hfield, Dims d, int64_t copy_links_bytes,
-                                   int64_t copy_field_bytes) {
+                                   int64_t copy_field_bytes, uint64_t seed, int64_t top_site0) {
     typedef Layout<R, RECON> L;
     const int Nzh = d.Nz >> 1;
     const int Vsh = d.Nx * d.Ny * Nzh;
@@ -454,7 +462,14 @@ __global__ void gauge_apply_kernel(char* links, char* gtot, const char* hfield, 
     global_get<R, 18>(hfield + Layout<R, 18>::site_offset(par, Vh), Vh, cb, h);
 #pragma unroll 1
     for (int mu = 0; mu < 4; ++mu) {
-        global_get<R, 18>(hfield + Layout<R, 18>::site_offset(1 - par, Vh), Vh, cbf[mu], hf);
+        if (mu == 0 && top_site0 >= 0 && t == d.Nt - 1) {
+            Mat<double> hd;
+            haar_su3(seed + (uint64_t)blockIdx.y, (uint32_t)(top_site0 + ((int64_t)x * d.Ny + y) * d.Nz + 2 * zh + r), hd);
+#pragma unroll
+            for (int k = 0; k < 18; ++k) hf.v[k] = (R)hd.v[k];
+        } else {
+            global_get<R, 18>(hfield + Layout<R, 18>::site_offset(1 - par, Vh), Vh, cbf[mu], hf);
+        }
         char* p0 = links + L::link_offset(par, mu, Vh);
         global_get<R, RECON>(p0, Vh, cb, U);
         mul_left<3>(h, U, T);

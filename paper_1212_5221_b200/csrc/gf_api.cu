@@ -1409,12 +1409,16 @@ int gf_fix(gf_ctx* ctx, const gf_fix_params* p, gf_result* out) {
 // ---- random start on the gauge orbit ------------------------------------------
 #define GAUGE_APPLY(R, RECON, hf)                                                                               \
     gauge_apply_kernel<R, RECON><<<dim3((unsigned)((ctx->Vh + 127) / 128), (unsigned)ctx->B, 2), 128, 0, ctx->stream>>>( \
-        ctx->links, ctx->gtot, (hf), dims_of(ctx), link_store_bytes(ctx), field_store_bytes(ctx))
+        ctx->links, ctx->gtot, (hf), dims_of(ctx), link_store_bytes(ctx), field_store_bytes(ctx), seed, top_site0)
 
 int gf_random_gauge(gf_ctx* ctx, uint64_t seed) {
     if (!ctx) return GF_EINVAL;
     if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_random_gauge: no links set");
-    if (int rcs = not_on_shards(ctx, "gf_random_gauge")) return rcs;
+    // t-shards: h(x) is a function of the site index in the whole lattice, so a shard draws its own sites' h and
+    // recomputes h of the slice above for the temporal links of its last slice; nothing is exchanged
+    const int64_t slice_sites = (int64_t)ctx->Nx * ctx->Ny * ctx->Nz;
+    const int64_t site_off = (int64_t)ctx->t0 * slice_sites;
+    const int64_t top_site0 = ctx->sharded ? (int64_t)((ctx->t0 + ctx->Nt) % ctx->NtG) * slice_sites : -1;
     if (ctx->temporal_stale && ctx->gtot) {
         int rc = gf_coulomb_finalize(ctx);
         if (rc) return rc;
@@ -1436,8 +1440,8 @@ int gf_random_gauge(gf_ctx* ctx, uint64_t seed) {
             e = cudaGetLastError();
         }
     } else {
-        if (ctx->real_bytes == 4) haar_field_kernel<float><<<g, 128, 0, ctx->stream>>>(h, dims_of(ctx), seed, field_store_bytes(ctx));
-        else haar_field_kernel<double><<<g, 128, 0, ctx->stream>>>(h, dims_of(ctx), seed, field_store_bytes(ctx));
+        if (ctx->real_bytes == 4) haar_field_kernel<float><<<g, 128, 0, ctx->stream>>>(h, dims_of(ctx), seed, field_store_bytes(ctx), site_off);
+        else haar_field_kernel<double><<<g, 128, 0, ctx->stream>>>(h, dims_of(ctx), seed, field_store_bytes(ctx), site_off);
         e = cudaGetLastError();
         if (e == cudaSuccess) {
             DISPATCH_RR(ctx, GAUGE_APPLY, h);
@@ -1450,6 +1454,8 @@ int gf_random_gauge(gf_ctx* ctx, uint64_t seed) {
     CU(e);
     // h was applied to all four directions: Coulomb sweeps that follow snapshot g(x) = h g(x) as already applied
     transform_changed(ctx);
+    shard_barrier(ctx);
+    (void)top_site0;
     return GF_OK;
 }
 

@@ -213,8 +213,9 @@ def test_shard_argument_checks(gf):
             a.attach(a, b)                                  # a is not the shard below a
         a.attach(b, b)
         b.attach(a, a)
+        a.set_links(np.zeros(a.shape))
         with pytest.raises(gf.GfError) as e:
-            a.random_gauge(1)
+            a.plaquette()
         assert e.value.code == gf.GF_ESTATE
         h = gf.gf_shard_export(a.ctx)
         assert (h.t0, h.Nt_local, h.has_transform) == (0, 4, 0) and any(h.links)
@@ -300,6 +301,7 @@ def test_recipe_and_lagged_stop_on_shards_bit_for_bit(gf, n_shards):
     kw = dict(precision=DP, recon=12, lagged_stop=True)
 
     def body(fx):
+        fx.random_gauge(seed=77)       # the random start of the recipe: h(x) keyed by the site index in the whole lattice
         f = fx.fix(MAG, seed=3, sa_steps=5, sa_T_hi=1.0, sa_T_lo=0.1, sa_micro=2, sr_max_sweeps=10, sr_p=0.5, or_omega=1.7,
                    or_max_sweeps=60, eps=1e-9, check_every=2)
         r = fx.run(LANDAU, OR, 1.7, max_sweeps=2500, eps=1e-7, check_every=1, reunit_every=200, history=True)
@@ -313,3 +315,25 @@ def test_recipe_and_lagged_stop_on_shards_bit_for_bit(gf, n_shards):
         assert g[1]["sweeps"] == ref[1]["sweeps"] and g[1]["F"] == ref[1]["F"] and g[1]["theta"] == ref[1]["theta"]
         assert np.array_equal(g[1]["history"], ref[1]["history"])
     assert np.array_equal(join_t([g[2] for g in got]), ref[2])
+
+
+@pytest.mark.parametrize("prec,recon", [(DP, 18), (SP, 12)])
+def test_random_gauge_on_shards_bit_for_bit(gf, oracle, prec, recon):
+    dims = (6, 4, 8, 12)
+    L = config(dims, prec, seed=371)
+    dt = L.dtype
+    kw = dict(precision=prec, recon=recon, track_transform=True)
+
+    def body(fx):
+        fx.random_gauge(seed=4242)
+        return fx.get_links(dtype=dt), fx.get_gauge_transform(dtype=dt)
+
+    ref = run_unsharded(gf, dims, L, body, **kw)
+    got = run_sharded(gf, dims, L, 3, body, **kw)           # 12 slices as 4 + 4 + 4
+    assert np.array_equal(join_t([g[0] for g in got]), ref[0])
+    assert np.array_equal(join_t([g[1] for g in got]), ref[1])
+    if prec == DP:      # and the unsharded context against the oracle's random start
+        Lo = L.copy()
+        go = oracle.identity_transform(Lo)
+        oracle.random_gauge(Lo, 4242, go)
+        assert np.abs(ref[0] - Lo).max() <= 1e-12 and np.abs(ref[1] - go).max() <= 1e-12
