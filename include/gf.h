@@ -293,7 +293,8 @@ int gf_fix(gf_ctx* ctx, const gf_fix_params* params, gf_result* out);
  * gf_coulomb_finalize (which reads g(x + t_hat) of its last slice from the shard above) work as on a
  * whole lattice, and so does gf_random_gauge (h(x) is a function of the site index in the whole lattice: a shard
  * recomputes h of the slice above for its last temporal links); gf_get_slice_sweeps has Nt_global entries;
- * gf_unitarity covers the shard's own links; gf_wilson_heatbath and gf_plaquette return GF_ESTATE.  Sweeps and reductions return GF_ESTATE
+ * gf_unitarity covers the shard's own links; gf_plaquette returns the plaquette of the whole lattice (the last slice
+ * reads the first one of the store above); gf_wilson_heatbath returns GF_ESTATE.  Sweeps and reductions return GF_ESTATE
  * until the neighbours are attached.  A single shard spanning the lattice attaches to itself.
  * The tests drive 2 and 4 shards on one device — threads of one process, and two processes with IPC-mapped stores —
  * and compare with the unsharded context bit for bit; mappings of ANOTHER device's memory were not run in this build

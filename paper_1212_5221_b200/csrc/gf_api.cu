@@ -87,6 +87,7 @@ struct gf_ctx {
     char* links_dn;         // store holding slice t0 - 1 as its last slice (not sharded: links)
     int64_t Vh_dn;
     int Nt_dn;
+    char* links_up;         // link store holding slice t0 + Nt as its first slice (not sharded: links)
     char* gtot_up;          // transform stores holding slice t0 + Nt as their first slice (not sharded: gtot / gapplied)
     char* gapp_up;
     int64_t Vh_up;
@@ -228,7 +229,7 @@ static int create_impl(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int n_copie
     ctx->NtG = NtG; ctx->t0 = t0; ctx->NSG = n_copies * NtG;
     ctx->VG = (int64_t)Nx * Ny * Nz * NtG;
     ctx->links_dn = nullptr; ctx->Vh_dn = ctx->Vh; ctx->Nt_dn = Nt;
-    ctx->gtot_up = ctx->gapp_up = nullptr; ctx->Vh_up = ctx->Vh;
+    ctx->gtot_up = ctx->gapp_up = nullptr; ctx->links_up = nullptr; ctx->Vh_up = ctx->Vh;
     ctx->attached = !ctx->sharded;
     ctx->block_auto = auto_block(ctx);
     ctx->have_comm = false;
@@ -268,6 +269,7 @@ static int create_impl(gf_ctx** out, int Nx, int Ny, int Nz, int Nt, int n_copie
     ctx->device_bytes += (int64_t)(npart * 2 + 2 * NS + 2 * nred + 6 * NS) * sizeof(double);
     if (!ctx->sharded) {   // the periodic wrap in t: the store is its own neighbour
         ctx->links_dn = ctx->links;
+        ctx->links_up = ctx->links;
         ctx->gtot_up = ctx->gtot;
     }
     *out = ctx;
@@ -474,6 +476,9 @@ int gf_shard_attach(gf_ctx* ctx, gf_ctx* below, gf_ctx* above) {
     rc = enable_peer_for(ctx, below->links);
     if (rc) return rc;
     ctx->links_dn = below->links; ctx->Vh_dn = below->Vh; ctx->Nt_dn = below->Nt;
+    rc = enable_peer_for(ctx, above->links);
+    if (rc) return rc;
+    ctx->links_up = above->links; ctx->Vh_up = above->Vh;
     if (ctx->gtot) {
         rc = enable_peer_for(ctx, above->gtot);
         if (rc) return rc;
@@ -508,6 +513,14 @@ int gf_shard_attach_ipc(gf_ctx* ctx, const gf_shard_handle* below, const gf_shar
     CU(cudaIpcOpenMemHandle(&p, *(const cudaIpcMemHandle_t*)below->links, cudaIpcMemLazyEnablePeerAccess));
     ctx->ipc_opened.push_back(p);
     ctx->links_dn = (char*)p; ctx->Nt_dn = below->Nt_local; ctx->Vh_dn = Vs2 * below->Nt_local;
+    if (memcmp(below->links, above->links, sizeof(below->links)) == 0) {
+        ctx->links_up = ctx->links_dn;   // two shards: the same store on both sides, mapped once
+    } else {
+        CU(cudaIpcOpenMemHandle(&p, *(const cudaIpcMemHandle_t*)above->links, cudaIpcMemLazyEnablePeerAccess));
+        ctx->ipc_opened.push_back(p);
+        ctx->links_up = (char*)p;
+    }
+    ctx->Vh_up = Vs2 * above->Nt_local;
     if (ctx->gtot) {
         CU(cudaIpcOpenMemHandle(&p, *(const cudaIpcMemHandle_t*)above->gtot, cudaIpcMemLazyEnablePeerAccess));
         ctx->ipc_opened.push_back(p);
@@ -1507,17 +1520,18 @@ int gf_wilson_heatbath(gf_ctx* ctx, double beta, uint64_t seed, uint32_t first_s
 
 #define PLAQUETTE(R, RECON, dummy)                                                                               \
     plaquette_kernel<R, RECON><<<dim3((unsigned)ctx->meas_gx, (unsigned)ctx->NS, 2), ctx->meas_block, 0, ctx->stream>>>( \
-        ctx->links, dims_of(ctx), ctx->partial, link_store_bytes(ctx))
+        ctx->links, dims_of(ctx), ctx->partial, link_store_bytes(ctx), ctx->links_up, ctx->Vh_up)
 
 int gf_plaquette(gf_ctx* ctx, double* plaq) {
     if (!ctx) return GF_EINVAL;
     if (!plaq) return fail(ctx, GF_EINVAL, "gf_plaquette: NULL pointer");
     if (!ctx->have_links) return fail(ctx, GF_ESTATE, "gf_plaquette: no links set");
-    if (int rcs = not_on_shards(ctx, "gf_plaquette")) return rcs;
+    if (int rca = need_attached(ctx, "gf_plaquette")) return rca;
     if (ctx->temporal_stale && ctx->gtot) {
         int rc = gf_coulomb_finalize(ctx);
         if (rc) return rc;
     }
+    shard_barrier(ctx);   // the last slice reads the first one of the store above
     if (ctx->nc == 2) {
         const dim3 g2((unsigned)ctx->meas_gx, (unsigned)ctx->NS, 2);
         if (ctx->real_bytes == 4) plaquette2_kernel<float><<<g2, ctx->meas_block, 0, ctx->stream>>>(ctx->links, dims_of(ctx), ctx->partial, link_store_bytes(ctx));
@@ -1528,13 +1542,19 @@ int gf_plaquette(gf_ctx* ctx, double* plaq) {
     slice_reduce_kernel<<<ctx->NS, 128, 0, ctx->stream>>>(ctx->partial, 2 * ctx->meas_gx, ctx->NS, ctx->slice_dev);
     CU(cudaGetLastError());
     ctx->launches += 2;
-    CU(cudaMemcpyAsync(ctx->slice_host, ctx->slice_dev, (size_t)2 * ctx->NS * sizeof(double), cudaMemcpyDeviceToHost,
-                       ctx->stream));
-    CU(cudaStreamSynchronize(ctx->stream));
+    if (ctx->sharded) {   // per global slice, completed over the shards and summed in slice order on every shard
+        memset(ctx->slice_host, 0, (size_t)2 * ctx->NSG * sizeof(double));
+        CU(cudaMemcpyAsync(ctx->slice_host + ctx->t0, ctx->slice_dev, (size_t)ctx->NS * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    } else {
+        CU(cudaMemcpyAsync(ctx->slice_host, ctx->slice_dev, (size_t)2 * ctx->NS * sizeof(double), cudaMemcpyDeviceToHost,
+                           ctx->stream));
+    }
+    int rcf = finish_enqueued_measure(ctx);
+    if (rcf) return rcf;
     for (int c = 0; c < ctx->B; ++c) {
         double tot = 0.0;
-        for (int t = 0; t < ctx->Nt; ++t) tot += ctx->slice_host[(size_t)c * ctx->Nt + t];
-        plaq[c] = tot / ((double)ctx->nc * 6.0 * (double)ctx->V);
+        for (int t = 0; t < ctx->NtG; ++t) tot += ctx->slice_host[(size_t)c * ctx->NtG + t];
+        plaq[c] = tot / ((double)ctx->nc * 6.0 * (double)ctx->VG);
     }
     return GF_OK;
 }

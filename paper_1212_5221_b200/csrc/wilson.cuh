@@ -135,7 +135,10 @@ __global__ void __launch_bounds__(128, GF_HB_MIN_CTAS) wilson_heatbath_kernel(ch
 // sum over the 6 plaquettes at x of Re tr U_P: grid (ceil(Vsh/block), ncopies*Nt, 2) like measure_kernel;
 // partial[...][0] = sum, [1] = 0
 template <class R, int RECON>
-__global__ void plaquette_kernel(const char* links, Dims d, double* partial, int64_t copy_bytes) {
+// t-shards: U_nu(x + t_hat) of the last slice is the first slice of the link store above (links_up, Vh_up sites per
+// parity; shards hold one copy); not sharded: the store itself (periodic wrap)
+__global__ void plaquette_kernel(const char* links, Dims d, double* partial, int64_t copy_bytes, const char* links_up,
+                                 int64_t Vh_up) {
     typedef Layout<R, RECON> L;
     const int Nzh = d.Nz >> 1;
     const int Vsh = d.Nx * d.Ny * Nzh;
@@ -159,7 +162,10 @@ __global__ void plaquette_kernel(const char* links, Dims d, double* partial, int
             for (int nu = mu + 1; nu < 4; ++nu) {
                 Mat<R> a, b, T1, T2;
                 global_get<R, RECON>(links + L::link_offset(par, mu, Vh), Vh, cb, a);
-                global_get<R, RECON>(links + L::link_offset(1 - par, nu, Vh), Vh, cb_shift(d, s, mu, +1, mu, 0), b);
+                if (mu == 0 && t == d.Nt - 1)     // same (x, y, z) in slice 0 of the store above: in-slice index i
+                    global_get<R, RECON>(links_up + copy * copy_bytes + L::link_offset(1 - par, nu, Vh_up), Vh_up, (int64_t)i, b);
+                else
+                    global_get<R, RECON>(links + L::link_offset(1 - par, nu, Vh), Vh, cb_shift(d, s, mu, +1, mu, 0), b);
                 mul_left<3>(a, b, T1);                                   // U_mu(x) U_nu(x+mu)
                 global_get<R, RECON>(links + L::link_offset(1 - par, mu, Vh), Vh, cb_shift(d, s, nu, +1, nu, 0), a);
                 mul_right_dagger<3>(T1, a, T2);                          // ... U_mu(x+nu)^dag

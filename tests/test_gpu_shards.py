@@ -101,7 +101,7 @@ def test_landau_or_run_bit_for_bit(gf, n_shards, prec, recon):
     def body(fx):
         r = fx.run(LANDAU, OR, 1.7, max_sweeps=60, eps=eps, check_every=3, reunit_every=20 if prec == SP else 0, history=True)
         F, th, ts = fx.measure(LANDAU, slices=True)
-        return r, (F, th, ts), fx.get_links(dtype=dt), fx.get_gauge_transform(dtype=dt), fx.slice_sweeps()
+        return r, (F, th, ts), fx.get_links(dtype=dt), fx.get_gauge_transform(dtype=dt), fx.slice_sweeps(), fx.plaquette()[0]
 
     ref = run_unsharded(gf, dims, L, body, **kw)
     got = run_sharded(gf, dims, L, n_shards, body, **kw)
@@ -111,8 +111,12 @@ def test_landau_or_run_bit_for_bit(gf, n_shards, prec, recon):
         assert np.array_equal(g[0]["history"], ref[0]["history"])
         assert g[1][0] == ref[1][0] and g[1][1] == ref[1][1] and np.array_equal(g[1][2], ref[1][2])
         assert np.array_equal(g[4], ref[4])
+        assert g[5] == ref[5]                                  # the plaquette of the whole lattice, on every shard
     assert np.array_equal(join_t([g[2] for g in got]), ref[2])
     assert np.array_equal(join_t([g[3] for g in got]), ref[3])
+    # gauge invariance (Eq. (1)): the plaquette of the input
+    from tests.helpers import plaquettes
+    assert abs(ref[5] - plaquettes(inputs.as_complex(L.astype(np.float64))).mean()) < (1e-12 if prec == DP else 2e-6)
 
 
 def test_sharded_sweep_matches_oracle(gf, oracle):
@@ -213,9 +217,8 @@ def test_shard_argument_checks(gf):
             a.attach(a, b)                                  # a is not the shard below a
         a.attach(b, b)
         b.attach(a, a)
-        a.set_links(np.zeros(a.shape))
         with pytest.raises(gf.GfError) as e:
-            a.plaquette()
+            a.wilson_heatbath(5.7, 1)                       # the input generator is not sharded
         assert e.value.code == gf.GF_ESTATE
         h = gf.gf_shard_export(a.ctx)
         assert (h.t0, h.Nt_local, h.has_transform) == (0, 4, 0) and any(h.links)
@@ -252,7 +255,8 @@ def _ipc_worker(rank, world, port, dims, q):
         r = fx.run(LANDAU, OR, 1.7, max_sweeps=12, eps=-1.0, check_every=4, history=True)
         nxt = fx.anneal(MAG, 0.9, 0.2, 3, 1, seed=5, first_sweep_index=12)
         rc = fx.run(COULOMB, OR, 1.7, max_sweeps=6, eps=-1.0, check_every=6)
-        out = (rank, t0, r["history"], nxt, rc["F"], rc["theta"], fx.get_links(), fx.get_gauge_transform(), dict(comm.calls))
+        out = (rank, t0, r["history"], nxt, rc["F"], rc["theta"], fx.get_links(), fx.get_gauge_transform(), dict(comm.calls),
+               fx.plaquette()[0])
         dist.barrier()          # nobody unmaps a store a neighbour may still be reading
         fx.close()
         q.put(out)
@@ -270,7 +274,7 @@ def test_two_processes_with_ipc_mapped_stores_bit_for_bit(gf):
         r = fx.run(LANDAU, OR, 1.7, max_sweeps=12, eps=-1.0, check_every=4, history=True)
         nxt = fx.anneal(MAG, 0.9, 0.2, 3, 1, seed=5, first_sweep_index=12)
         rc = fx.run(COULOMB, OR, 1.7, max_sweeps=6, eps=-1.0, check_every=6)
-        return r["history"], nxt, rc["F"], rc["theta"], fx.get_links(), fx.get_gauge_transform()
+        return r["history"], nxt, rc["F"], rc["theta"], fx.get_links(), fx.get_gauge_transform(), fx.plaquette()[0]
 
     ref = run_unsharded(gf, dims, L, body, precision=DP, recon=18, track_transform=True)
     with socket.socket() as s:
@@ -288,6 +292,7 @@ def test_two_processes_with_ipc_mapped_stores_bit_for_bit(gf):
     for g in got:
         assert np.array_equal(g[2], ref[0]) and g[3] == ref[1] and g[4] == ref[2] and g[5] == ref[3]
         assert g[8]["barrier"] > 30 and g[8]["allreduce"] >= 4
+        assert g[9] == ref[6]
     assert np.array_equal(join_t([g[6] for g in got]), ref[4])
     assert np.array_equal(join_t([g[7] for g in got]), ref[5])
 
