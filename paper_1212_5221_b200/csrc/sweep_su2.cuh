@@ -8,6 +8,8 @@
 // (Landau SP 256 B, DP 512 B).  Grid, batching, frozen slices and the fused F / theta partials are those of
 // sweep.cuh.
 #pragma once
+#include <atomic>
+
 #include "su2.cuh"
 #include "sweep.cuh"
 
@@ -163,7 +165,33 @@ static cudaError_t launch_su2_one(const SweepArgs& args, int block, cudaStream_t
     const int Vsh = args.Nx * args.Ny * (args.Nz / 2);
     block = sweep_su2_block(Vsh, block);
     const dim3 grid((unsigned)((Vsh + block - 1) / block), (unsigned)(args.ncopies * args.Nt));
-    return launch_with_pdl(sweep_su2_kernel<R, A, GAUGE, STOCH, TRACK, RED>, grid, dim3((unsigned)block), 0, stream, args);
+    // the kernel uses no dynamic shared memory; a small grid asks for some so that its CTAs spread over all SMs
+    // (sweep_inst.cuh, launch_one)
+    auto kern = sweep_su2_kernel<R, A, GAUGE, STOCH, TRACK, RED>;
+    size_t smem_launch = 0;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    static std::atomic<int> sms_of[64];   // (the attribute query costs microseconds: once per device)
+    int sms = (dev >= 0 && dev < 64) ? sms_of[dev].load(std::memory_order_relaxed) : 0;
+    if (sms <= 0) {
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+        if (dev >= 0 && dev < 64) sms_of[dev].store(sms, std::memory_order_relaxed);
+    }
+    const long long ctas = (long long)grid.x * grid.y, per_sm = (ctas + sms - 1) / sms;
+    if (per_sm <= 8) {
+        smem_launch = ((size_t)(228 * 1024) / (size_t)per_sm - 1024) / 1024 * 1024;
+        if (smem_launch > (size_t)(226 * 1024)) smem_launch = 226 * 1024;
+        static std::atomic<int> attr_set[64];
+        if (dev < 0 || dev >= 64 || !attr_set[dev].load(std::memory_order_acquire)) {
+            e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024);
+            if (e != cudaSuccess) return e;
+            // (no carveout preference: the kernel loads through L1, which large grids want as large as it gets)
+            if (dev >= 0 && dev < 64) attr_set[dev].store(1, std::memory_order_release);
+        }
+    }
+    return launch_with_pdl(kern, grid, dim3((unsigned)block), smem_launch, stream, args);
 }
 template <class R, class A, int GAUGE>
 static cudaError_t launch_su2_gauge(const SweepArgs& args, bool track, int block, cudaStream_t stream) {
