@@ -60,7 +60,9 @@ typedef struct gf_ctx gf_ctx; /* opaque */
 /* Step-1 update rule (Secs. 2.2.3-2.3) */
 #define GF_OR 0    /* overrelaxation g -> g^omega "to first order" = Fig. A.11; param = omega in [1,2) */
 #define GF_SR 1    /* stochastic relaxation: g^2 with probability param = p, else g */
-#define GF_SA 2    /* simulated-annealing heatbath at temperature param = T */
+#define GF_SA 2    /* simulated-annealing heatbath at temperature param = T; its arithmetic is double on
+                      GF_DP / GF_MP contexts and float on GF_SP contexts, where every accept/reject decision that float
+                      cannot settle is re-evaluated in double */
 #define GF_MICRO 3 /* microcanonical step g -> g^2; param ignored */
 
 /* gf_create flags */
