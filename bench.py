@@ -622,7 +622,7 @@ def run_ours(args):
             bench_other((32, 32, 32, 64), 0, "dp", 18, 1, 200, "Landau OR, 32^3x64, DP-18"),
             bench_other((32, 32, 32, 64), 0, "sp", 12, 1, 200, "Landau OR, 32^3x64, SP-12"),
             bench_other((32, 32, 32, 64), 1, "sp", 12, 1, 200, "Coulomb OR, 32^3x64, SP-12 (BASELINE.json configs[2])"),
-            bench_other((16, 16, 16, 16), 0, "dp", 18, 1, 200, "Landau OR, 16^4, DP-18, one copy (configs[1])"),
+            bench_other((16, 16, 16, 16), 0, "dp", 18, 1, 1000, "Landau OR, 16^4, DP-18, one copy (configs[1])"),
             bench_other((16, 16, 16, 16), 0, "dp", 18, 64, 100, "Landau OR, 64 gauge copies of 16^4 per launch, DP-18"),
             bench_other((32, 32, 32, 32), 0, "sp", 12, 16, 100, "Landau OR, 16 gauge copies of 32^4 per launch, SP-12"),
             bench_other((64, 64, 64, 256), 0, "sp", 12, 1, 50, "Landau OR, 64^3x256, SP-12, accumulating g(x) (a8)", track=True),
