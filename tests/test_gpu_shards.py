@@ -6,7 +6,8 @@ the barrier and the sum of the per-slice reduction arrays.  The first slice of a
 of the shard below in place, the Philox counter uses the site index in the whole lattice and the reductions are summed
 per global slice in slice order, so everything — links, g(x), F, theta, histories, sweep counts, annealing draws — must
 equal the unsharded context BIT FOR BIT (integer-exact bar; the unsharded context is held to the oracle elsewhere, and
-once here).  Several devices / processes (peer and IPC mappings) use the same kernels and were not run on hardware.
+once here).  Two PROCESSES on the one device, with IPC-mapped neighbour stores and the torch.distributed (gloo)
+communicator, are run at the end of this file; mappings of another device's memory use the same kernels and were not run.
 """
 import threading
 
