@@ -362,6 +362,41 @@ int gf_plaquette(gf_ctx* ctx, double* plaq);
 int gf_unitarity(gf_ctx* ctx, double* avg, double* max);
 
 /*
+ * gf_unitarity_noalloc — the same measure, Eq. (33), for callers that must not allocate: no context,
+ * and no cudaMalloc, cudaFree or other allocating call inside, on any call.
+ *
+ * Why it exists: gf_unitarity needs a context, i.e. a second copy of the configuration on the GPU, and it takes and
+ * frees two scratch buffers per call (the cudaFree waits for the whole device).  A lattice code whose own fields
+ * already fill the GPU, code that lives inside a memory pool with a fixed budget, or a monitoring step that must not
+ * stall the kernels of other streams cannot use that; here they hand in the buffer they already have.
+ *
+ *   links_device   DEVICE pointer to n_links SU(3) matrices of 18 reals each, row major with re/im innermost (one
+ *                  link of the StandardPattern host layout above; a whole configuration in that layout is
+ *                  n_links = 4 V).  Read only; aligned to 2 * elem_bytes.  The link order plays no role.
+ *   elem_bytes     4 (float) or 8 (double); the determinant is evaluated in double either way.
+ *   n_links        0 <= n_links <= GF_UNITARITY_NOALLOC_MAX_LINKS (2^28 = the 4 V links of 64^3 x 256).  More is
+ *                  rejected with GF_EINVAL: measure the buffer in pieces and combine the averages and maxima.
+ *   result_device  DEVICE pointer to 2 doubles owned by the caller: [0] = (1/n_links) sum |1 - det U|, [1] = max
+ *                  |1 - det U| (both 0 for n_links = 0).  Valid once the work enqueued on cuda_stream has finished.
+ *   cuda_stream    a cudaStream_t or NULL.  The call only enqueues two kernels there (asynchronous).
+ *   errbuf         NULL, or errbuf_len bytes that receive a NUL-terminated description when the return value is not
+ *                  GF_OK (there is no context whose gf_last_error could hold it).
+ * Errors: GF_EINVAL (arguments, size, alignment — checked before the device is touched), GF_ECUDA.
+ *
+ * The scratch memory — one (sum, max) pair per 2048 links — is a fixed array inside libgf.so's device image, 2 MiB
+ * on every GPU that loads the library, held until the process exits.  Consequences:
+ *   - All calls on one device share it.  Calls whose kernels may overlap on the GPU (different streams or host
+ *     threads without an ordering between them) corrupt each other's result; calls on one stream are safe, and so
+ *     are calls on different devices.  Nothing has to be zeroed between calls: every entry a call reads it has
+ *     written itself, whatever the previous call left behind.
+ *   - The first call on each device (with that device current, as for every call) looks up the array's address on
+ *     that device; make that first call before you start capturing a stream.
+ */
+#define GF_UNITARITY_NOALLOC_MAX_LINKS (1 << 28)
+int gf_unitarity_noalloc(const void* links_device, int elem_bytes, int64_t n_links, double* result_device,
+                         void* cuda_stream, char* errbuf, int errbuf_len);
+
+/*
  * gf_reunitarize — reproject every link (and the tracked transform) onto SU(3): Gram-Schmidt on rows
  * 0,1 in double, third row (u x v)^* (R20).  Asynchronous.
  */

@@ -30,9 +30,10 @@ GF_FLAG_TRACK_TRANSFORM = 1
 GF_FLAG_FREEZE_SLICES = 2
 GF_FLAG_SU2 = 4
 GF_FLAG_LAGGED_STOP = 8
+GF_UNITARITY_NOALLOC_MAX_LINKS = 1 << 28
 
 EXPORTS = ["gf_create", "gf_num_colors", "gf_create_batch", "gf_num_copies", "gf_set_links_copy", "gf_get_links_copy",
-           "gf_get_gauge_transform_copy", "gf_measure_batch", "gf_measure_mag_eq16", "gf_run_batch", "gf_fix", "gf_random_gauge", "gf_wilson_heatbath", "gf_plaquette", "gf_unitarity", "gf_destroy", "gf_set_links", "gf_get_links", "gf_get_gauge_transform", "gf_sweep",
+           "gf_get_gauge_transform_copy", "gf_measure_batch", "gf_measure_mag_eq16", "gf_run_batch", "gf_fix", "gf_random_gauge", "gf_wilson_heatbath", "gf_plaquette", "gf_unitarity", "gf_unitarity_noalloc", "gf_destroy", "gf_set_links", "gf_get_links", "gf_get_gauge_transform", "gf_sweep",
            "gf_half_sweep", "gf_measure", "gf_run", "gf_get_slice_sweeps", "gf_anneal", "gf_reunitarize", "gf_coulomb_finalize",
            "gf_sync", "gf_kernel_timing", "gf_kernel_time_ms", "gf_launch_count", "gf_device_bytes", "gf_volume", "gf_last_error", "gf_version",
            "gf_create_shard", "gf_shard_attach", "gf_shard_export", "gf_shard_attach_ipc", "gf_shard_set_comm", "gf_shard_info",
@@ -85,6 +86,7 @@ _lib.gf_random_gauge.argtypes = [_vp, _u64]
 _lib.gf_wilson_heatbath.argtypes = [_vp, _cd, _u64, _u32, _ci]
 _lib.gf_plaquette.argtypes = [_vp, _vp]
 _lib.gf_unitarity.argtypes = [_vp, _vp, _vp]
+_lib.gf_unitarity_noalloc.argtypes = [_vp, _ci, ctypes.c_int64, _vp, _vp, ctypes.c_char_p, _ci]
 _lib.gf_create.argtypes = [ctypes.POINTER(_vp), _ci, _ci, _ci, _ci, _ci, _ci, ctypes.c_uint, _vp]
 _lib.gf_destroy.argtypes = [_vp]
 _lib.gf_set_links.argtypes = [_vp, _vp, _ci, _ci]
@@ -341,6 +343,30 @@ def gf_unitarity(ctx):
     a, m = np.zeros(B), np.zeros(B)
     _check(ctx, _lib.gf_unitarity(ctx, _vp(a.ctypes.data), _vp(m.ctypes.data)))
     return a, m
+
+
+def gf_unitarity_noalloc(links, result, cuda_stream=None):
+    """Eq. (33) on a buffer the caller already has on the GPU, for callers that must not allocate (gf.h,
+    gf_unitarity_noalloc: no context, no cudaMalloc / cudaFree inside; scratch is a fixed 2 MiB array of the library).
+
+    links: CUDA tensor, float32 or float64, contiguous, 18 reals per link (any leading shape; numel / 18 links, at most
+    GF_UNITARITY_NOALLOC_MAX_LINKS).  result: the caller's CUDA float64 tensor with at least 2 elements; it receives
+    (average, maximum) of |1 - det U| once the work enqueued on the stream has run — this wrapper creates no tensor
+    and does not synchronise.  Calls on one device must not overlap on the GPU (they share the scratch array); the first
+    call on a device should come before any stream capture.  Returns `result`."""
+    import torch
+    if not (isinstance(links, torch.Tensor) and links.is_cuda and isinstance(result, torch.Tensor) and result.is_cuda):
+        raise TypeError("gf_unitarity_noalloc: links and result must be CUDA tensors (device memory owned by the caller)")
+    if result.dtype != torch.float64 or result.numel() < 2 or not result.is_contiguous():
+        raise TypeError("gf_unitarity_noalloc: result must be a contiguous float64 tensor with at least 2 elements")
+    ptr, eb, _, n = _buffer(links)
+    if n % 18:
+        raise ValueError("gf_unitarity_noalloc: links must hold 18 reals per link")
+    err = ctypes.create_string_buffer(512)
+    rc = _lib.gf_unitarity_noalloc(_vp(ptr), eb, n // 18, _vp(result.data_ptr()), _vp(_stream_handle(cuda_stream)), err, 512)
+    if rc != GF_OK:
+        raise GfError(rc, err.value.decode())
+    return result
 
 
 def gf_sweep(ctx, gauge, algo, param, seed=0, sweep_index=0):
