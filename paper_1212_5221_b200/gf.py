@@ -273,9 +273,13 @@ def gf_get_gauge_transform_copy(ctx, copy, out):
 
 
 def gf_measure_batch(ctx, gauge, Nt=None):
-    """-> (F[n_copies], theta[n_copies]) or, with Nt given, (F, theta, theta_slice[n_copies, Nt])."""
+    """-> (F[n_copies], theta[n_copies]) or, with Nt given (any true value), (F, theta, theta_slice[n_copies, Nt_global]).
+    The library writes Nt_global entries per copy — on a t-shard more than the shard's own slices — so the buffer is
+    sized from gf_shard_info, never from the caller's number."""
     B = gf_num_copies(ctx)
     F, th = np.zeros(B), np.zeros(B)
+    if Nt:
+        Nt = gf_shard_info(ctx)[2]
     ts = np.zeros((B, Nt)) if Nt else None
     _check(ctx, _lib.gf_measure_batch(ctx, gauge, _vp(F.ctypes.data), _vp(th.ctypes.data),
                                       _vp(ts.ctypes.data) if Nt else None))
@@ -378,8 +382,11 @@ def gf_half_sweep(ctx, gauge, algo, param, seed, sweep_index, parity):
 
 
 def gf_measure(ctx, gauge, Nt=None):
-    """-> (F, theta) or, with Nt given, (F, theta, theta_slice[Nt])."""
+    """-> (F, theta) or, with Nt given (any true value), (F, theta, theta_slice[Nt_global]); the buffer is sized from
+    gf_shard_info (a t-shard reports every slice of the whole lattice)."""
     F, th = _cd(), _cd()
+    if Nt:
+        Nt = gf_shard_info(ctx)[2]
     ts = np.zeros(Nt) if Nt else None
     _check(ctx, _lib.gf_measure(ctx, gauge, ctypes.byref(F), ctypes.byref(th), _vp(ts.ctypes.data) if Nt else None))
     return (F.value, th.value, ts) if Nt else (F.value, th.value)
@@ -400,8 +407,9 @@ def gf_run(ctx, gauge, algo, param, seed=0, first_sweep_index=0, max_sweeps=1000
     return out
 
 
-def gf_get_slice_sweeps(ctx, Nt):
-    out = np.zeros(Nt * gf_num_copies(ctx), dtype=np.int32)
+def gf_get_slice_sweeps(ctx, Nt=None):
+    """-> int32[n_copies * Nt_global] (the size comes from gf_shard_info; Nt is accepted for older callers and ignored)."""
+    out = np.zeros(gf_shard_info(ctx)[2] * gf_num_copies(ctx), dtype=np.int32)
     _check(ctx, _lib.gf_get_slice_sweeps(ctx, _vp(out.ctypes.data)))
     return out
 
@@ -577,7 +585,7 @@ class GaugeFixer:
         return gf_measure_mag_eq16(self.ctx)
 
     def measure_batch(self, gauge, slices=False):
-        return gf_measure_batch(self.ctx, gauge, self.dims[3] if slices else None)
+        return gf_measure_batch(self.ctx, gauge, self.Nt_global if slices else None)
 
     def run_batch(self, gauge, algo, param, **kw):
         return gf_run_batch(self.ctx, gauge, algo, param, **kw)

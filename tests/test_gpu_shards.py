@@ -120,6 +120,29 @@ def test_landau_or_run_bit_for_bit(gf, n_shards, prec, recon):
     assert abs(ref[5] - plaquettes(inputs.as_complex(L.astype(np.float64))).mean()) < (1e-12 if prec == DP else 2e-6)
 
 
+def test_measure_batch_with_slices_on_shards(gf):
+    # the library writes theta_slice for every slice of the WHOLE lattice on each shard; the wrapper once
+    # sized the buffer with the shard's own Nt and the call overran it.  Every wrapper that takes slices must return
+    # Nt_global entries equal to the unsharded context's, whatever Nt the caller names.
+    dims = (4, 6, 4, 16)
+    L = config(dims, DP, seed=305)
+
+    def body(fx):
+        fx.run(COULOMB, OR, 1.7, max_sweeps=2, eps=1e-30, check_every=1)
+        Fb, thb, tsb = fx.measure_batch(COULOMB, slices=True)
+        F1, th1, ts1 = gf.gf_measure(fx.ctx, COULOMB, Nt=2)           # a wrong (too small) Nt cannot under-allocate
+        Fb2, thb2, tsb2 = gf.gf_measure_batch(fx.ctx, COULOMB, Nt=2)
+        return Fb, thb, tsb, (F1, th1, ts1), tsb2, gf.gf_get_slice_sweeps(fx.ctx, 2)
+
+    ref = run_unsharded(gf, dims, L, body, precision=DP)
+    assert ref[2].shape == (1, 16) and ref[2].min() > 0
+    for g in run_sharded(gf, dims, L, 4, body, precision=DP):
+        assert g[2].shape == (1, 16) and g[3][2].shape == (16,) and g[4].shape == (1, 16) and g[5].shape == ref[5].shape
+        assert g[0][0] == ref[0][0] and g[1][0] == ref[1][0] and np.array_equal(g[2], ref[2])
+        assert g[3][0] == ref[3][0] and g[3][1] == ref[3][1] and np.array_equal(g[3][2], ref[3][2])
+        assert np.array_equal(g[4], ref[4])
+
+
 def test_sharded_sweep_matches_oracle(gf, oracle):
     # once against the oracle directly: one Landau OR sweep and one MAG heatbath sweep on 4 shards, DP per-link bars
     dims = (6, 4, 8, 8)
