@@ -309,6 +309,7 @@ int gf_shard_attach(gf_ctx* ctx, gf_ctx* below, gf_ctx* above);
 typedef struct {
     unsigned char links[64], gtot[64], gapplied[64]; /* cudaIpcMemHandle_t of the stores */
     int t0, Nt_local, has_transform;
+    int Nx, Ny, Nz, Nt_global, precision, recon;     /* what the store was created with: checked by gf_shard_attach_ipc */
 } gf_shard_handle;
 int gf_shard_export(gf_ctx* ctx, gf_shard_handle* handle);
 int gf_shard_attach_ipc(gf_ctx* ctx, const gf_shard_handle* below, const gf_shard_handle* above);
@@ -317,6 +318,14 @@ typedef struct {
     void (*allreduce_sum)(void* user, double* buf, int n);
     void* user;
 } gf_comm;
+/*
+ * gf_shard_attach_ipc maps the neighbours' stores only after checking that they were created with this shard's extents,
+ * precision, recon and Nt_global, that they adjoin its slices and that all three track a transform or none does
+ * (GF_EINVAL otherwise, nothing mapped).  A call that fails part-way closes what it had opened, and a repeated call
+ * closes the previous mappings first.  gf_shard_attach (same process) refuses neighbours that live on this shard's
+ * device but use another stream, unless a communicator with a barrier has been set BEFORE the attach: a barrier that
+ * only synchronises host threads orders nothing between two streams.
+ */
 /* comm == NULL: no communicator (all shards on one stream of one process need none for ordering, but still need
  * allreduce_sum for reductions unless there is a single shard) */
 int gf_shard_set_comm(gf_ctx* ctx, const gf_comm* comm);

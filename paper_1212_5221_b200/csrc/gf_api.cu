@@ -110,7 +110,13 @@ static int auto_block(const gf_ctx* c) {
     const int maxb = dbl ? 64 : 128;
     const int64_t Vsh = (int64_t)c->Nx * c->Ny * (c->Nz / 2), units = (int64_t)c->B * c->NtG;
     const int64_t ctas = ((Vsh + maxb - 1) / maxb) * units;
-    return ctas < (dbl ? 300 : 148) ? 32 : maxb;
+    // thresholds calibrated on the 148 SMs of a B200 (one CTA per SM in float, 300 CTAs in double), scaled with the SM
+    // count of the device the context lives on; the t-shards of one lattice must sit on devices of one kind for their
+    // fused partial sums to keep the unsharded order (gf.h, "t-shards")
+    int dev = 0, sms = 148;
+    DevLimits lim;
+    if (cudaGetDevice(&dev) == cudaSuccess && dev_limits(dev, lim) == cudaSuccess) sms = lim.sms;
+    return ctas < (dbl ? (int64_t)300 * sms / 148 : (int64_t)sms) ? 32 : maxb;
 }
 
 static int fail(gf_ctx* c, int code, const char* fmt, ...) {
@@ -473,6 +479,17 @@ int gf_shard_attach(gf_ctx* ctx, gf_ctx* below, gf_ctx* above) {
     if (rc) return rc;
     if ((below->t0 + below->Nt) % ctx->NtG != ctx->t0)
         return fail(ctx, GF_EINVAL, "gf_shard_attach: the shard below ends at slice %d, this one starts at %d", below->t0 + below->Nt, ctx->t0);
+    // shards of one device are ordered by sharing a stream (a host-only barrier orders nothing between two streams)
+    for (const gf_ctx* nb : {below, above}) {
+        if (nb == ctx || nb->stream == ctx->stream || (ctx->have_comm && ctx->comm.barrier)) continue;
+        cudaPointerAttributes at;
+        int dev = 0;
+        CU(cudaPointerGetAttributes(&at, nb->links));
+        CU(cudaGetDevice(&dev));
+        if (at.type == cudaMemoryTypeDevice && at.device == dev)
+            return fail(ctx, GF_EINVAL, "gf_shard_attach: a neighbour on this device uses another stream and no communicator "
+                                        "barrier is set (share one stream, or call gf_shard_set_comm first)");
+    }
     rc = enable_peer_for(ctx, below->links);
     if (rc) return rc;
     ctx->links_dn = below->links; ctx->Vh_dn = below->Vh; ctx->Nt_dn = below->Nt;
@@ -499,36 +516,72 @@ int gf_shard_export(gf_ctx* ctx, gf_shard_handle* h) {
         h->has_transform = 1;
     }
     h->t0 = ctx->t0; h->Nt_local = ctx->Nt;
+    h->Nx = ctx->Nx; h->Ny = ctx->Ny; h->Nz = ctx->Nz; h->Nt_global = ctx->NtG;
+    h->precision = ctx->precision; h->recon = ctx->recon;
+    return GF_OK;
+}
+
+// mappings opened by gf_shard_attach_ipc are closed before a re-attach and when an attach fails part-way
+static void close_ipc_mappings(gf_ctx* ctx) {
+    for (void* q : ctx->ipc_opened) cudaIpcCloseMemHandle(q);
+    ctx->ipc_opened.clear();
+    if (ctx->sharded) {
+        ctx->links_dn = ctx->links_up = nullptr;
+        ctx->gtot_up = ctx->gapp_up = nullptr;
+        ctx->attached = false;
+    }
+}
+static int check_handle(gf_ctx* ctx, const gf_shard_handle* h, const char* what) {
+    if (h->Nx != ctx->Nx || h->Ny != ctx->Ny || h->Nz != ctx->Nz || h->Nt_global != ctx->NtG || h->precision != ctx->precision ||
+        h->recon != ctx->recon)
+        return fail(ctx, GF_EINVAL, "gf_shard_attach_ipc: the %s (%dx%dx%d, Nt_global %d, precision %d, recon %d) does not match this "
+                                    "shard (%dx%dx%d, Nt_global %d, precision %d, recon %d)", what, h->Nx, h->Ny, h->Nz, h->Nt_global,
+                    h->precision, h->recon, ctx->Nx, ctx->Ny, ctx->Nz, ctx->NtG, ctx->precision, ctx->recon);
+    if (h->Nt_local < 2 || h->t0 < 0 || h->t0 + h->Nt_local > ctx->NtG)
+        return fail(ctx, GF_EINVAL, "gf_shard_attach_ipc: the %s holds slices [%d, %d) of %d", what, h->t0, h->t0 + h->Nt_local, ctx->NtG);
+    if ((ctx->gtot != nullptr) != (h->has_transform != 0))
+        return fail(ctx, GF_EINVAL, "gf_shard_attach_ipc: GF_FLAG_TRACK_TRANSFORM differs between this shard and the %s", what);
+    static const unsigned char zero[64] = {0};
+    if (memcmp(h->links, zero, 64) == 0 ||
+        (h->has_transform && (memcmp(h->gtot, zero, 64) == 0 || memcmp(h->gapplied, zero, 64) == 0)))
+        return fail(ctx, GF_EINVAL, "gf_shard_attach_ipc: the %s carries an empty store handle (not filled by gf_shard_export)", what);
     return GF_OK;
 }
 
 int gf_shard_attach_ipc(gf_ctx* ctx, const gf_shard_handle* below, const gf_shard_handle* above) {
     if (!ctx || !below || !above) return GF_EINVAL;
+    if (!ctx->sharded) return fail(ctx, GF_ESTATE, "gf_shard_attach_ipc: not a t-shard (gf_create_shard)");
+    // everything is checked before anything is mapped: a mismatched neighbour would be indexed with this shard's layout
+    int rc = check_handle(ctx, below, "shard below");
+    if (rc) return rc;
+    rc = check_handle(ctx, above, "shard above");
+    if (rc) return rc;
     if ((below->t0 + below->Nt_local) % ctx->NtG != ctx->t0 || above->t0 != (ctx->t0 + ctx->Nt) % ctx->NtG)
         return fail(ctx, GF_EINVAL, "gf_shard_attach_ipc: neighbours do not adjoin slices [%d, %d)", ctx->t0, ctx->t0 + ctx->Nt);
-    if ((ctx->gtot != nullptr) != (above->has_transform != 0))
-        return fail(ctx, GF_EINVAL, "gf_shard_attach_ipc: GF_FLAG_TRACK_TRANSFORM differs between the shards");
+    CU(cudaStreamSynchronize(ctx->stream));
+    close_ipc_mappings(ctx);   // a repeated attach starts from nothing (an open handle cannot be opened twice)
     const int64_t Vs2 = (int64_t)ctx->Nx * ctx->Ny * ctx->Nz / 2;
-    void* p = nullptr;
-    CU(cudaIpcOpenMemHandle(&p, *(const cudaIpcMemHandle_t*)below->links, cudaIpcMemLazyEnablePeerAccess));
-    ctx->ipc_opened.push_back(p);
-    ctx->links_dn = (char*)p; ctx->Nt_dn = below->Nt_local; ctx->Vh_dn = Vs2 * below->Nt_local;
-    if (memcmp(below->links, above->links, sizeof(below->links)) == 0) {
-        ctx->links_up = ctx->links_dn;   // two shards: the same store on both sides, mapped once
-    } else {
-        CU(cudaIpcOpenMemHandle(&p, *(const cudaIpcMemHandle_t*)above->links, cudaIpcMemLazyEnablePeerAccess));
-        ctx->ipc_opened.push_back(p);
-        ctx->links_up = (char*)p;
+    auto open = [&](const unsigned char* h, char** out) -> cudaError_t {
+        void* p = nullptr;
+        cudaError_t e = cudaIpcOpenMemHandle(&p, *(const cudaIpcMemHandle_t*)h, cudaIpcMemLazyEnablePeerAccess);
+        if (e == cudaSuccess) { ctx->ipc_opened.push_back(p); *out = (char*)p; }
+        return e;
+    };
+    cudaError_t e = open(below->links, &ctx->links_dn);
+    ctx->Nt_dn = below->Nt_local; ctx->Vh_dn = Vs2 * below->Nt_local;
+    if (e == cudaSuccess) {
+        if (memcmp(below->links, above->links, sizeof(below->links)) == 0)
+            ctx->links_up = ctx->links_dn;   // two shards: the same store on both sides, mapped once
+        else
+            e = open(above->links, &ctx->links_up);
     }
     ctx->Vh_up = Vs2 * above->Nt_local;
-    if (ctx->gtot) {
-        CU(cudaIpcOpenMemHandle(&p, *(const cudaIpcMemHandle_t*)above->gtot, cudaIpcMemLazyEnablePeerAccess));
-        ctx->ipc_opened.push_back(p);
-        ctx->gtot_up = (char*)p;
-        CU(cudaIpcOpenMemHandle(&p, *(const cudaIpcMemHandle_t*)above->gapplied, cudaIpcMemLazyEnablePeerAccess));
-        ctx->ipc_opened.push_back(p);
-        ctx->gapp_up = (char*)p;
-        ctx->Vh_up = Vs2 * above->Nt_local;
+    if (e == cudaSuccess && ctx->gtot) e = open(above->gtot, &ctx->gtot_up);
+    if (e == cudaSuccess && ctx->gtot) e = open(above->gapplied, &ctx->gapp_up);
+    if (e != cudaSuccess) {
+        close_ipc_mappings(ctx);
+        cudaGetLastError();
+        return fail(ctx, GF_ECUDA, "gf_shard_attach_ipc: cudaIpcOpenMemHandle: %s (mappings opened so far were closed)", cudaGetErrorString(e));
     }
     ctx->attached = true;
     return GF_OK;

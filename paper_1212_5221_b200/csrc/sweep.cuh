@@ -14,6 +14,7 @@
 // Every link is read once and written once per half-sweep; nothing is re-read from HBM.  No
 // __syncthreads: a thread only ever touches its own shared-memory slice.
 #pragma once
+#include <atomic>
 #include <cstdint>
 #include <cuda_runtime.h>
 
@@ -484,6 +485,37 @@ inline int sweep_block(int Vsh, int block_override, bool stoch = false) {
     if (block <= 0 || block > maxb) block = maxb;
     const int need = ((Vsh + 31) / 32) * 32;
     return block < need ? block : need;
+}
+
+// What the launchers need to know about a device, asked once per device: the SM count, the shared memory of an SM and
+// the most dynamic shared memory one CTA may opt into (a B200: 148, 228 KB, 227 KB).  smem_cta_cap leaves 1 KB of the
+// opt-in limit to the kernels' static shared memory (226 KB on a B200).
+struct DevLimits {
+    int sms;
+    size_t smem_per_sm, smem_cta_cap;
+};
+inline cudaError_t dev_limits(int dev, DevLimits& out) {
+    struct Slot {
+        std::atomic<int> ready;
+        DevLimits v;
+    };
+    static Slot cache[64];
+    const bool cached = dev >= 0 && dev < 64;
+    if (cached && cache[dev].ready.load(std::memory_order_acquire)) { out = cache[dev].v; return cudaSuccess; }
+    int sms = 0, per_sm = 0, optin = 0;
+    cudaError_t e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&per_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (e != cudaSuccess) return e;
+    if (sms <= 0 || per_sm <= 0 || optin <= 1024) return cudaErrorInvalidDevice;
+    out.sms = sms;
+    out.smem_per_sm = (size_t)per_sm;
+    out.smem_cta_cap = (size_t)optin - 1024;
+    if (cached) {   // several threads may get here together: they write the same values
+        cache[dev].v = out;
+        cache[dev].ready.store(1, std::memory_order_release);
+    }
+    return cudaSuccess;
 }
 
 // launch a half-sweep kernel, with the programmatic-stream-serialization attribute when args.pdl is set

@@ -172,20 +172,16 @@ static cudaError_t launch_su2_one(const SweepArgs& args, int block, cudaStream_t
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
-    static std::atomic<int> sms_of[64];   // (the attribute query costs microseconds: once per device)
-    int sms = (dev >= 0 && dev < 64) ? sms_of[dev].load(std::memory_order_relaxed) : 0;
-    if (sms <= 0) {
-        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (e != cudaSuccess) return e;
-        if (dev >= 0 && dev < 64) sms_of[dev].store(sms, std::memory_order_relaxed);
-    }
-    const long long ctas = (long long)grid.x * grid.y, per_sm = (ctas + sms - 1) / sms;
-    if (per_sm <= 8) {
-        smem_launch = ((size_t)(228 * 1024) / (size_t)per_sm - 1024) / 1024 * 1024;
-        if (smem_launch > (size_t)(226 * 1024)) smem_launch = 226 * 1024;
+    DevLimits lim;
+    e = dev_limits(dev, lim);   // SM count and shared-memory limits of this device (cached)
+    if (e != cudaSuccess) return e;
+    const long long ctas = (long long)grid.x * grid.y, per_sm = (ctas + lim.sms - 1) / lim.sms;
+    if (per_sm <= 8 && lim.smem_per_sm / (size_t)per_sm > 2048) {
+        smem_launch = (lim.smem_per_sm / (size_t)per_sm - 1024) / 1024 * 1024;
+        if (smem_launch > lim.smem_cta_cap) smem_launch = lim.smem_cta_cap;
         static std::atomic<int> attr_set[64];
         if (dev < 0 || dev >= 64 || !attr_set[dev].load(std::memory_order_acquire)) {
-            e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024);
+            e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lim.smem_cta_cap);
             if (e != cudaSuccess) return e;
             // (no carveout preference: the kernel loads through L1, which large grids want as large as it gets)
             if (dev >= 0 && dev < 64) attr_set[dev].store(1, std::memory_order_release);

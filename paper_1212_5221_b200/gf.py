@@ -54,7 +54,9 @@ class gf_fix_params(ctypes.Structure):
 
 class gf_shard_handle(ctypes.Structure):
     _fields_ = [("links", ctypes.c_ubyte * 64), ("gtot", ctypes.c_ubyte * 64), ("gapplied", ctypes.c_ubyte * 64),
-                ("t0", ctypes.c_int), ("Nt_local", ctypes.c_int), ("has_transform", ctypes.c_int)]
+                ("t0", ctypes.c_int), ("Nt_local", ctypes.c_int), ("has_transform", ctypes.c_int),
+                ("Nx", ctypes.c_int), ("Ny", ctypes.c_int), ("Nz", ctypes.c_int), ("Nt_global", ctypes.c_int),
+                ("precision", ctypes.c_int), ("recon", ctypes.c_int)]
 
 
 GF_BARRIER_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p)

@@ -9,6 +9,7 @@ equal the unsharded context BIT FOR BIT (integer-exact bar; the unsharded contex
 once here).  Two PROCESSES on the one device, with IPC-mapped neighbour stores and the torch.distributed (gloo)
 communicator, are run at the end of this file; mappings of another device's memory use the same kernels and were not run.
 """
+import ctypes
 import threading
 
 import numpy as np
@@ -246,9 +247,44 @@ def test_shard_argument_checks(gf):
         assert e.value.code == gf.GF_ESTATE
         h = gf.gf_shard_export(a.ctx)
         assert (h.t0, h.Nt_local, h.has_transform) == (0, 4, 0) and any(h.links)
+        assert (h.Nx, h.Ny, h.Nz, h.Nt_global, h.precision, h.recon) == (4, 4, 4, 8, a.precision, 18)
+        # gf_shard_attach_ipc checks a neighbour's handle BEFORE it maps anything: a store created with other
+        # extents, precision, recon or flags would be indexed with this shard's layout
+        hb = gf.gf_shard_export(b.ctx)
+        for field, bad in (("Nx", 6), ("Nt_global", 16), ("precision", (a.precision + 1) % 3), ("recon", 12), ("has_transform", 1),
+                           ("t0", 2), ("Nt_local", 0)):
+            hm = gf.gf_shard_handle.from_buffer_copy(bytes(hb))
+            setattr(hm, field, bad)
+            for below, above in ((hm, hb), (hb, hm)):
+                with pytest.raises(gf.GfError) as e:
+                    gf.gf_shard_attach_ipc(a.ctx, below, above)
+                assert e.value.code == gf.GF_EINVAL, field
+        hm = gf.gf_shard_handle.from_buffer_copy(bytes(hb))
+        ctypes.memset(ctypes.addressof(hm), 0, 64)          # a handle that gf_shard_export never filled
+        with pytest.raises(gf.GfError) as e:
+            gf.gf_shard_attach_ipc(a.ctx, hm, hb)
+        assert e.value.code == gf.GF_EINVAL and "empty store handle" in str(e.value)
+        a.sweep(LANDAU, OR, 1.7)                            # the refused calls left the thread attachment alone
+        a.sync()
     finally:
         a.close()
         b.close()
+    # shards of one device on different streams: a host-only barrier orders nothing between them, so the attach is refused
+    # until a communicator with a barrier is set
+    import torch
+    from paper_1212_5221_b200 import shards
+    c = gf.GaugeFixer(4, 4, 4, 4, shard=(0, 8), cuda_stream=torch.cuda.Stream())
+    d = gf.GaugeFixer(4, 4, 4, 4, shard=(4, 8), cuda_stream=torch.cuda.Stream())
+    try:
+        with pytest.raises(gf.GfError) as e:
+            c.attach(d, d)
+        assert e.value.code == gf.GF_EINVAL and "another stream" in str(e.value)
+        comms = shards.ThreadComm.group(2)                  # (any barrier callback: the library cannot look inside it)
+        c.set_comm(comms[0].comm)
+        c.attach(d, d)
+    finally:
+        c.close()
+        d.close()
 
 
 # ---- one process per shard: CUDA IPC mappings and the torch.distributed communicator (gloo), on ONE device ----------
