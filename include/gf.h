@@ -186,8 +186,9 @@ typedef struct {
  * Cost of a check: the odd half-sweep of a check sweep s leaves F(s) and the odd sites' share of theta(s), a lower
  * bound of theta(s), at no extra traffic; only a check at which that bound is below eps runs the stand-alone
  * reduction (one read of every link twice, about one half-sweep), so every stopping decision is the one a reduction
- * after every check would take (Alg. 1).  With GF_FLAG_LAGGED_STOP (single lattice, not with
- * GF_FLAG_FREEZE_SLICES) that reduction is not run either: the even sites' share of theta(s) is what the even
+ * after every check would take (Alg. 1).  With GF_FLAG_LAGGED_STOP (single lattice, GF_DP or GF_MP, not
+ * with GF_FLAG_FREEZE_SLICES; ignored on GF_SP contexts, whose fused sums are formed in float and carry ~1e-12 of
+ * rounding noise in theta: they keep the stand-alone reduction) that reduction is not run either: the even sites' share of theta(s) is what the even
  * half-sweep of sweep s + 1 sees before it updates, so theta(s) is known, exactly and at no cost, half a sweep later.
  * If theta(s) < eps the run stops THERE: out->sweeps = s, and the links returned have received the even half-sweep of
  * sweep s + 1 on top of Alg. 1's s sweeps (out->F, out->theta are those of the links returned; GF_OK).  A check at
@@ -353,8 +354,9 @@ int gf_random_gauge(gf_ctx* ctx, uint64_t seed);
  * sub | purpose << 8, trial), key seed + copy, sweeps first_sweep_index .. first_sweep_index + n_sweeps - 1.
  * The result is a new configuration, so a tracked transform restarts at the identity.  Asynchronous.
  * On contexts with recon = 12 the links are reprojected onto SU(3) after every 16th sweep of the call (as in gf_anneal),
- * on other float contexts after every 100th.  On SP contexts the heatbath arithmetic is float with
- * guard-banded accept decisions, as in GF_SA sweeps.
+ * on other float contexts after every 100th.  On contexts with float storage (GF_SP and GF_MP) the
+ * heatbath arithmetic of this generator is float with guard-banded accept decisions (the kernel works in
+ * the storage type, so GF_MP does not buy a double heatbath here as it does in GF_SA sweeps).
  * On SU(2) contexts the same with the single subgroup and the weight exp((beta/2) Re tr[U A]) (T = 2/beta).
  * gf_plaquette: plaq[n_copies] receives <Re tr U_P> / N_c over the 6 V plaquettes (gauge invariant under
  * Eq. (1): it does not change under any sweep of this library).  Synchronous.

@@ -1224,7 +1224,10 @@ static int run_impl(gf_ctx* ctx, int gauge, int algo, double param, uint64_t see
     // GF_FLAG_LAGGED_STOP (one unit): a check whose lower bound theta_odd(s) falls below eps is not decided by the
     // stand-alone reduction but half a sweep later, from the even sites' share that the even half-sweep of sweep s + 1
     // sees before it updates: exact and free; if theta(s) < eps the run stops there (gf.h)
-    const bool lagged = fused && (ctx->flags & GF_FLAG_LAGGED_STOP) && nunits == 1 && !skip_slice;
+    // Not on GF_SP contexts: there the fused terms are formed from float sums (noise ~1e-12 in theta, see `trig`), a
+    // decision at theta ~ eps could differ from the exact one, and by the time it is taken the links have moved on, so
+    // the exact reduction can no longer settle it.  SP runs keep the margin + exact reduction of the plain path.
+    const bool lagged = fused && (ctx->flags & GF_FLAG_LAGGED_STOP) && nunits == 1 && !skip_slice && ctx->precision != GF_SP;
     bool lag_decide = false, lag_stopped = false;
     // float Step 1 (GF_SP): the fused terms are formed from float sums and carry their rounding noise (~1e-12 in
     // theta); the exact reduction is called for a little earlier so that the bound stays one

@@ -69,3 +69,27 @@ def test_lagged_stop_at_max_sweeps_and_mp(gf, oracle):
             oracle.sweep(ref7, LANDAU, OR, 1.7, 0, k, True)
         assert not r["converged"] and r["sweeps"] == 7
         assert np.abs(fx.get_links(dtype=np.float32).astype(np.float64) - ref7).max() <= 5e-5
+
+
+def test_lagged_stop_is_ignored_on_sp_contexts(gf):
+    """on GF_SP the fused sums are float sums with ~1e-12 of noise in theta, so a lagged decision near eps
+    could contradict the exact reduction after the links have moved on.  The flag therefore does nothing on SP: the run
+    is the plain one bit for bit (sweeps, F, theta, history, links), converged means theta of the RETURNED links < eps,
+    and no extra half-sweep has been applied."""
+    dims = (8, 6, 4, 8)
+    L = inputs.as_real(inputs.make_config(*dims, 0.4, 521, 522), np.float32)
+    for eps in (1e-9, 3e-11):             # the second sits inside the noise band of the fused float sums
+        out = {}
+        for lagged in (True, False):
+            with gf.GaugeFixer(*dims, precision=SP, lagged_stop=lagged) as fx:
+                fx.set_links(L)
+                r = fx.run(LANDAU, OR, 1.7, max_sweeps=600, eps=eps, check_every=1, reunit_every=50, history=True)
+                F, th = fx.measure(LANDAU)
+                out[lagged] = (r, fx.get_links(dtype=np.float32), F, th)
+        r, links, F, th = out[True]
+        r0, links0, F0, th0 = out[False]
+        assert r["sweeps"] == r0["sweeps"] and r["F"] == r0["F"] and r["theta"] == r0["theta"] and r["converged"] == r0["converged"]
+        assert np.array_equal(r["history"], r0["history"]) and np.array_equal(links, links0)
+        assert th == r["theta"] and F == r["F"]                    # what the run reports is the state it returns
+        if r["converged"]:
+            assert th < eps
