@@ -215,7 +215,10 @@ int gf_run_batch(gf_ctx* ctx, int gauge, int algo, double param, uint64_t seed, 
  * sweeping slice t at the first check at which theta_t < eps (the CTAs of a stopped slice exit at
  * once), so the result of slice t is that of a stand-alone run on that slice.  gf_run then returns
  * GF_OK when every slice has stopped; out->theta = max_t theta_t of the final links.  Reprojection
- * (reunit_every) still covers all links.  Landau/MAG runs ignore the flag.
+ * (reunit_every) still covers all links, stopped slices included: on float-storage contexts (GF_SP, GF_MP) a slice
+ * that stopped with theta_t < eps is rounded to float again by every later reprojection and may then read up to
+ * about 3 eps at the final measurement for eps near the float floor (1e-10); the stopping decision itself was taken
+ * on theta_t < eps, and GF_DP contexts return theta_t < eps for every slice.  Landau/MAG runs ignore the flag.
  * gf_get_slice_sweeps: sweeps[n_copies * Nt] (host) receives the number of sweeps applied to every slice
  * of every copy by the last gf_run / gf_run_batch (without the flag or for other gauges: the sweep count
  * of the slice's copy in every entry).

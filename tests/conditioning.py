@@ -43,6 +43,13 @@ def site_conditioning(oracle, Lpre, txyz, gauge, T, seed, sweep_index):
     dirs = (1, 2, 3) if gauge == COULOMB else (0, 1, 2, 3)
     up, dn = _gather(Lpre, t, x, y, z, dirs)
     sidx = ((t * Nx + x) * Ny + y) * Nz + z
+    return gathered_conditioning(oracle, up, dn, gauge, T, seed, sidx, sweep_index)
+
+
+def gathered_conditioning(oracle, up, dn, gauge, T, seed, sidx, sweep_index):
+    """site_conditioning for a site given by its gathered links up[mu] = U_mu(x), dn[mu] = U_mu(x - mu) (float64,
+    modified in place) and its lexicographic index sidx in the whole lattice (the Philox counter)."""
+    dirs = range(up.shape[0])
     c = np.inf
     for s, (i, j) in enumerate(SUBS):
         if gauge == MAG:

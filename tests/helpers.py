@@ -97,3 +97,15 @@ def paper_values():
             if len(line) == 2:
                 out[line[0]] = float(line[1])
     return out
+
+
+def golden_values(name):
+    """key -> float of a `key value` fixture under tests/golden/ (lines starting with # are comments)."""
+    import os
+    out = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", name)) as fh:
+        for line in fh:
+            line = line.split("#")[0].split()
+            if len(line) == 2:
+                out[line[0]] = float(line[1])
+    return out

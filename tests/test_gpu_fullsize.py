@@ -177,8 +177,12 @@ def test_full_size_heatbath_sampled_sites(gf, oracle, tile, dims, prec, recon, g
     # the simulated-annealing half-sweep in the launch configurations bench.py times (other_workloads): sampled sites of
     # a non-periodic 64^3 x 256 lattice against oracle.site_update with the site index in the whole lattice (Philox
     # counters up to 6.7e7, wrap-around neighbours, warp-wide retries across the whole grid).  DP: the annealing bar
-    # 1e-11 per link; SP (float heatbath on the GPU, double in the oracle): 5e-5 on all sampled sites but those whose
-    # local field is weak (conditioning number from the oracle below 0.5), which must still be unitary.
+    # 1e-11 per link; SP (float heatbath on the GPU, double in the oracle): BASELINE.json's 5e-5 on every sampled site,
+    # and a site that exceeds it must be inside ITS OWN first-order bound C 2^-23 (1 + 8 / c(x)) of tests/conditioning.py,
+    # c(x) the site's weakest local field from the oracle and C the constants of
+    # test_sp_heatbath_half_sweep_within_conditioning_bound (4, and 6 in Creutz's regime): the ill-conditioned sites are
+    # accounted for one by one — no blanket allowance, no count of exceptions.  (At c = 0.5 the bound is 8e-6: only
+    # sites with c < 0.08 can exceed 5e-5 at all.)
     import torch
     from tests import conditioning
     dev = torch.device("cuda", 0)
@@ -205,7 +209,8 @@ def test_full_size_heatbath_sampled_sites(gf, oracle, tile, dims, prec, recon, g
             gather_dn = lambda A: A[dn[..., 0], dn[..., 1], dn[..., 2], dn[..., 3], mu[None, :]]
             up_in, dn_in = gather_up(src).cpu().numpy(), gather_dn(src).cpu().numpy()
             up_out, dn_out = gather_up(out).cpu().numpy(), gather_dn(out).cpu().numpy()
-            n_bad = 0
+            C = 4.0 if T < 2.0 else 6.0
+            over = []
             for k in range(s.shape[0]):
                 t, x, y, z = (int(v) for v in s[k])
                 sidx = ((t * Nx + x) * Ny + y) * Nz + z
@@ -215,19 +220,14 @@ def test_full_size_heatbath_sampled_sites(gf, oracle, tile, dims, prec, recon, g
                 if prec == DP:
                     assert err <= 1e-11, (parity, k, err)
                 elif err > 5e-5:
-                    # a weak local field in one of the subgroups (oracle's numbers, double, on the float inputs)
-                    c = np.inf
-                    uu, dd = up_in[k].astype(np.float64), dn_in[k].astype(np.float64)
-                    for sub, (i, j) in enumerate(conditioning.SUBS):
-                        a = oracle.local_quaternion(uu, dd, i, j)
-                        c = min(c, float(np.linalg.norm(a)))
-                        g = oracle.rule_heatbath_landau(a, T, seed, sidx, sweep_index, sub)
-                        for m in range(4):
-                            uu[m] = oracle.apply_subgroup(uu[m], g, i, j, False)
-                            dd[m] = oracle.apply_subgroup(dd[m], g, i, j, True)
-                    assert c < 0.5 and err < 1e-2, (parity, k, err, c)
-                    n_bad += 1
-            assert n_bad <= 15, n_bad          # <= 1 % of the sampled sites
+                    # the site's weakest local field over the three subgroups (oracle's numbers, double, on the float inputs)
+                    c = conditioning.gathered_conditioning(oracle, up_in[k].astype(np.float64), dn_in[k].astype(np.float64),
+                                                           gauge, T, seed, sidx, sweep_index)
+                    bound = C * conditioning.EPS_F * (1.0 + 8.0 / c)
+                    assert err <= bound, (parity, k, err, bound, c)
+                    over.append((err, bound, c))
+            if prec != DP:
+                print(f"T = {T}, parity {parity}: {len(over)} of {s.shape[0]} sampled sites above 5e-5, (err, bound, c) = {over}")
             W = up_out[..., 0] + 1j * up_out[..., 1]
             assert np.abs(W @ np.conj(np.swapaxes(W, -1, -2)) - np.eye(3)).max() < (1e-12 if prec == DP else 2e-5)
 
@@ -255,7 +255,8 @@ def test_config2_full_run_coulomb_32x32x32x64(gf, oracle, prec, recon):
     assert conv and r["converged"]
     assert abs(r["F"] - F) <= 1e-5                      # BASELINE: F to 1e-5 in SP
     assert r["theta"] < 1e-10 and ths.max() < 1e-10
-    assert abs(r["sweeps"] - s) <= 0.1 * s + 20         # SP: rounding decides which check first sees 1e-10
+    print(f"config 2 {('SP', 'DP', 'MP')[prec]}-{recon}: oracle {s} sweeps, GPU {r['sweeps']}")
+    assert abs(r["sweeps"] - s) <= 2 * 10               # SP: rounding decides which check first sees 1e-10: within two checks
     # the 64 slices are 4 periods of the tile's 16: equal slices, equal theta_t
     np.testing.assert_allclose(ths[:16], ths[16:32], rtol=1e-6, atol=1e-16)
 

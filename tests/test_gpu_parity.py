@@ -9,6 +9,8 @@ extents so that any swapped index shows.
 import numpy as np
 import pytest
 
+from tests.helpers import golden_values
+
 from paper_1212_5221_b200 import inputs
 
 pytestmark = pytest.mark.gpu
@@ -397,13 +399,21 @@ def test_mag_anneal_then_or(gf, oracle):
         assert nxt_g == nxt == n_steps * (1 + n_micro)
         Fa, tha = fx.measure(MAG)
         ma = oracle.measure(ref, MAG)
-        assert abs(Fa - ma["F"]) < 0.02          # same ensemble at the end of the schedule
+        # same ensemble at the end of the schedule: both inside the spread that 32 random sequences produce on this
+        # lattice (tests/golden/config3_copy_spread.txt, written from the oracle alone; sigma = 9.9e-4)
+        sp = golden_values("config3_copy_spread.txt")
+        for Fx in (Fa, ma["F"]):
+            assert abs(Fx - sp["F_after_anneal_mean"]) < 4 * sp["F_after_anneal_sigma"], (Fx, sp)
         s, F, th, hist, conv = oracle.run(ref, MAG, OR, 1.7, max_sweeps=8000, eps=1e-12, first_sweep_index=nxt)
         r = fx.run(MAG, OR, 1.7, first_sweep_index=nxt, max_sweeps=8000, eps=1e-12)
         got = fx.get_links()
         g = fx.get_gauge_transform()
     assert conv and r["converged"] and r["theta"] < 1e-12
-    assert abs(r["F"] - F) < 0.02                # two Gribov copies of the same orbit
+    # two trajectories on one orbit.  On this lattice all 32 random sequences of the fixture end in the SAME maximum
+    # (F equal to 1e-12: no copy-to-copy spread left after the overrelaxation), so the full-run bar of BASELINE.json
+    # applies although the annealing trajectories decorrelated: F to 1e-10
+    assert sp["F_final_max"] - sp["F_final_min"] < 1e-11
+    assert abs(r["F"] - F) <= 1e-10 and abs(r["F"] - sp["F_final_mean"]) <= 1e-10
     F0 = oracle.measure(L, MAG)["F"]
     assert r["F"] > F0 + 0.1
     # whatever copy was reached, it is a gauge transform of the input (Eq. 1) by the returned g

@@ -624,3 +624,22 @@ def test_lagged_stop_reading_is_the_plain_run_plus_one_even_half_sweep(oracle):
     assert oracle.run(c, oracle.LANDAU, oracle.OR, 1.7, max_sweeps=6, eps=1e-10)[:3] == \
         oracle.run(d, oracle.LANDAU, oracle.OR, 1.7, max_sweeps=6, eps=1e-10, lagged_stop=True)[:3]
     assert np.array_equal(c, d)
+
+
+def test_config3_copy_spread_fixture_is_the_oracles(oracle):
+    """tests/golden/config3_copy_spread.txt is written by tests/golden/make_config3_copy_spread.py from the oracle alone;
+    two of its 32 random sequences are replayed here (PAPER.md:243, 556 schedule; R25).  On this 6^4 lattice
+    every sequence ends in the same maximum of the maximally Abelian functional, which is what lets the GPU parity test
+    ask for F to 1e-10 after a chaotic annealing trajectory."""
+    from tests.helpers import golden_values
+    from paper_1212_5221_b200 import inputs
+    sp = golden_values("config3_copy_spread.txt")
+    assert sp["n_seeds"] == 32 and sp["F_final_max"] - sp["F_final_min"] < 1e-11 and 5e-4 < sp["F_after_anneal_sigma"] < 2e-3
+    L = inputs.as_real(inputs.make_config(6, 6, 6, 6, 0.5, 350, 351))
+    for k in (0, 17):
+        ref = L.copy()
+        nxt = oracle.anneal(ref, 2, 1.45, 0.01, 12, 3, seed=1234 + k)
+        Fa = oracle.measure(ref, 2)["F"]
+        s, F, th, hist, conv = oracle.run(ref, 2, 0, 1.7, max_sweeps=8000, eps=1e-12, first_sweep_index=nxt)
+        assert conv and abs(F - sp["F_final_mean"]) < 1e-11
+        assert abs(Fa - sp["F_after_anneal_mean"]) < 4 * sp["F_after_anneal_sigma"]
