@@ -514,8 +514,9 @@ def run_ours(args):
                              "bytes_per_site_update": v["roofline"]["bytes_per_site_update"],
                              "kernel_share_of_step": v["kernel_share_of_step"]})
 
-    def bench_other(dims_o, gauge, prec, recon, copies, sweeps, label, su2=False, track=False, algo=OR, param=OMEGA):
-        """Side measurement (not the headline): `sweeps` OR sweeps of `copies` lattices of extent dims_o."""
+    def bench_other(dims_o, gauge, prec, recon, copies, sweeps, label, su2=False, track=False, algo=OR, param=OMEGA, key=None):
+        """Side measurement (not the headline): `sweeps` OR sweeps of `copies` lattices of extent dims_o.
+        key: the name under which the measurement also enters the compact `roofline.modes` summary."""
         ox, oy, oz, ot = dims_o
         Vo = ox * oy * oz * ot
         nd = 3 if gauge == 1 else 4
@@ -554,7 +555,7 @@ def run_ours(args):
         ach = bpsu * (copies * Vo // 2) / (kern_ms / kern_n * 1e-3) / 1e9
         eff = bpsu * copies * Vo * sweeps / (ms * 1e-3) / 1e9        # whole run incl. gaps, reductions, reprojection
         store = copies * Vo * 4 * recon * (8 if prec == "dp" else 4)
-        return {"workload": label, "gauge_group": "SU(2)" if su2 else "SU(3)", "lattice": list(dims_o), "copies": copies, "precision": prec, "recon": recon,
+        return {"workload": label, "key": key, "gauge_group": "SU(2)" if su2 else "SU(3)", "lattice": list(dims_o), "copies": copies, "precision": prec, "recon": recon,
                 "sweeps": sweeps, "value": copies * Vo * sweeps / (ms * 1e-3), "unit": "site-updates/s",
                 "avg_launch_ms": kern_ms / kern_n, "roofline_achieved_gbs": ach, "roofline_frac": ach / peak,
                 "whole_run_gbs": eff, "whole_run_frac": eff / peak,
@@ -619,19 +620,21 @@ def run_ours(args):
         links_dev = None
         torch.cuda.empty_cache()
         others = [
-            bench_other((32, 32, 32, 64), 0, "dp", 18, 1, 200, "Landau OR, 32^3x64, DP-18"),
-            bench_other((32, 32, 32, 64), 0, "sp", 12, 1, 200, "Landau OR, 32^3x64, SP-12"),
-            bench_other((32, 32, 32, 64), 1, "sp", 12, 1, 200, "Coulomb OR, 32^3x64, SP-12 (BASELINE.json configs[2])"),
+            bench_other((32, 32, 32, 64), 0, "dp", 18, 1, 200, "Landau OR, 32^3x64, DP-18", key="dp18_32x32x32x64"),
+            bench_other((32, 32, 32, 64), 0, "sp", 12, 1, 200, "Landau OR, 32^3x64, SP-12", key="sp12_32x32x32x64"),
+            bench_other((32, 32, 32, 64), 1, "sp", 12, 1, 200, "Coulomb OR, 32^3x64, SP-12 (BASELINE.json configs[2])", key="coulomb_sp12_32x32x32x64"),
             bench_other((16, 16, 16, 16), 0, "dp", 18, 1, 1000, "Landau OR, 16^4, DP-18, one copy (configs[1])"),
             bench_other((16, 16, 16, 16), 0, "dp", 18, 64, 100, "Landau OR, 64 gauge copies of 16^4 per launch, DP-18"),
             bench_other((32, 32, 32, 32), 0, "sp", 12, 16, 100, "Landau OR, 16 gauge copies of 32^4 per launch, SP-12"),
             bench_other((64, 64, 64, 256), 0, "sp", 12, 1, 50, "Landau OR, 64^3x256, SP-12, accumulating g(x) (a8)", track=True),
-            bench_other((64, 64, 64, 256), 2, "dp", 18, 1, 30, "MAG OR, 64^3x256, DP-18"),
-            bench_other((64, 64, 64, 256), 0, "sp", 12, 1, 30, "Landau simulated-annealing heatbath T=1 (Philox), 64^3x256, SP-12", algo=2, param=1.0),
-            bench_other((64, 64, 64, 256), 2, "dp", 18, 1, 20, "MAG simulated-annealing heatbath T=0.5 (Philox), 64^3x256, DP-18", algo=2, param=0.5),
-            bench_other((64, 64, 64, 256), 0, "sp", 12, 1, 30, "Landau stochastic relaxation p=0.5 (Philox), 64^3x256, SP-12", algo=1, param=0.5),
-            bench_other((64, 64, 64, 256), 0, "sp", 4, 1, 100, "SU(2) Landau OR, 64^3x256, SP (4 reals per link)", su2=True),
-            bench_other((64, 64, 64, 256), 0, "dp", 4, 1, 100, "SU(2) Landau OR, 64^3x256, DP (4 reals per link)", su2=True),
+            bench_other((64, 64, 64, 256), 2, "dp", 18, 1, 30, "MAG OR, 64^3x256, DP-18", key="mag_dp18"),
+            bench_other((64, 64, 64, 256), 0, "sp", 12, 1, 30, "Landau simulated-annealing heatbath T=1 (Philox), 64^3x256, SP-12", algo=2, param=1.0, key="sa_sp12"),
+            bench_other((64, 64, 64, 256), 0, "dp", 18, 1, 20, "Landau simulated-annealing heatbath T=1 (Philox), 64^3x256, DP-18", algo=2, param=1.0, key="sa_dp18"),
+            bench_other((64, 64, 64, 256), 0, "mp", 12, 1, 20, "Landau simulated-annealing heatbath T=1 (Philox), 64^3x256, MP-12", algo=2, param=1.0, key="sa_mp12"),
+            bench_other((64, 64, 64, 256), 2, "dp", 18, 1, 20, "MAG simulated-annealing heatbath T=0.5 (Philox), 64^3x256, DP-18", algo=2, param=0.5, key="sa_mag_dp18"),
+            bench_other((64, 64, 64, 256), 0, "sp", 12, 1, 30, "Landau stochastic relaxation p=0.5 (Philox), 64^3x256, SP-12", algo=1, param=0.5, key="sr_sp12"),
+            bench_other((64, 64, 64, 256), 0, "sp", 4, 1, 100, "SU(2) Landau OR, 64^3x256, SP (4 reals per link)", su2=True, key="su2_sp"),
+            bench_other((64, 64, 64, 256), 0, "dp", 4, 1, 100, "SU(2) Landau OR, 64^3x256, DP (4 reals per link)", su2=True, key="su2_dp"),
             bench_other((64, 64, 64, 256), 2, "mp", 4, 1, 100, "SU(2) MAG OR, 64^3x256, MP", su2=True),
             bench_shards_one_device((64, 64, 64, 256), "sp", 12, 4, 50,
                                     "Landau OR, 64^3x256, SP-12, ONE lattice as 4 t-shards on one device (one stream)"),
@@ -648,6 +651,17 @@ def run_ours(args):
                          f"{r['seconds']:.1f} s"}
 
     if rank == 0:
+        # compact per-mode summary inside `roofline` (the driver's record keeps that object): per-kernel fraction of
+        # roofline.peak (CUDA events around every half-sweep) and whole-run G site-updates/s; 64^3x256 unless the key
+        # names another lattice; sa_* = simulated-annealing heatbath, sr_* = stochastic relaxation half-sweeps
+        modes = {f"{args.precision}{args.recon}": [round(head["roofline"]["frac"], 4), round(head["value"] / world / 1e9, 3)]}
+        for v in variants:
+            modes[f"{v['precision']}{v['recon']}"] = [round(v["roofline_frac"], 4), round(v["value"] / world / 1e9, 3)]
+        for o in others:
+            if o.get("key"):
+                modes[o["key"]] = [round(o["roofline_frac"], 4), round(o["value"] / 1e9, 3)]
+        head["roofline"]["modes"] = modes
+        head["roofline"]["modes_columns"] = ["kernel_frac_of_peak", "G_site_updates_per_s_per_gpu"]
         line = {
             "metric": "site-updates/s (Landau OR sweep incl. F/theta reductions)", "value": head["value"],
             "unit": "site-updates/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -660,7 +674,8 @@ def run_ours(args):
                                f"{'DP reunitarisation + ' if args.precision != 'dp' else ''}one F/theta reduction",
                        "l2": "link store %.1f GB >> 126 MB L2: every half-sweep streams from HBM, no flush needed"
                              % (V * 4 * args.recon * (8 if args.precision == 'dp' else 4) / 1e9),
-                       "parallelism": "replicas only" if world > 1 else "single GPU"},
+                       "parallelism": ("replicas only" if world > 1 else "single GPU") +
+                                      " (--shard-t instead splits ONE lattice along t over the ranks: DESIGN.md §10, unmeasured on more than one GPU)"},
             "paper_gflops": head["paper_gflops"],
             "paper_context": "3.5 TFlops on 16 Tesla C2070, 64^3x256 SP (PAPER.md:518); other hardware, context only",
             "gpu_launches": head["gpu_launches"], "F": head["F"], "theta": head["theta"],

@@ -123,15 +123,22 @@ def exchange_handles(dist, handle: "gf.gf_shard_handle"):
     return hs[(rank - 1) % world], hs[(rank + 1) % world]
 
 
-def make_rank_shard(dist, device, stream, Nx, Ny, Nz, Nt_global, **kw):
+def make_rank_shard(dist, device, stream, Nx, Ny, Nz, Nt_global, force_comm=False, **kw):
     """One process per GPU: this rank's shard of the lattice, attached to its neighbours' stores through CUDA IPC
-    mappings (NVLink peer access) and wired to torch.distributed.  -> (GaugeFixer, TorchDistComm, (t0, Nt_local))."""
+    mappings (NVLink peer access) and wired to torch.distributed.  -> (GaugeFixer, TorchDistComm, (t0, Nt_local)).
+    A single rank needs no communicator and gets none, unless force_comm asks for it: the whole call path of the
+    multi-rank run (the collective issued from the library's callback once per half-sweep, the device-tensor sum of
+    the slice arrays) then runs on one GPU, which is how it is tested and timed where only one GPU is at hand."""
     world, rank = dist.get_world_size(), dist.get_rank()
     t0, n = partition_t(Nt_global, world)[rank]
     fx = gf.GaugeFixer(Nx, Ny, Nz, n, cuda_stream=stream, shard=(t0, Nt_global), **kw)
     if world == 1:
         fx.attach(fx, fx)
-        return fx, None, (t0, n)
+        if not force_comm:
+            return fx, None, (t0, n)
+        comm = TorchDistComm(dist, device=device, stream=stream)
+        fx.set_comm(comm.comm)
+        return fx, comm, (t0, n)
     below, above = exchange_handles(dist, gf.gf_shard_export(fx.ctx))
     gf.gf_shard_attach_ipc(fx.ctx, below, above)
     comm = TorchDistComm(dist, device=device, stream=stream)
